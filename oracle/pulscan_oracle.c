@@ -1,0 +1,256 @@
+/*
+ * pulscan_oracle.c — CPU ORACLE.  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, double-precision restatement of what the Pulscan boxcar-search hot path computes
+ * (White et al., arXiv 2406.15186; citations are "PAPER.md:L<line>").  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may call it.  It shares no source, header, table or
+ * helper with the CUDA path under paper_2406_15186_b200/csrc/ and neither side includes the other.
+ *
+ * Every step follows the paper's definition in the paper's order; there is no blocking, pruning, fusion or
+ * reordering.  Readings of passages where the paper is silent or garbled are the R-numbers of DESIGN.md §3.
+ *
+ * Parity pins (tests/test_oracle_*.py): numpy.median / scipy MAD / Φ⁻¹(¾); brute-force and closed-form
+ * boxcar sums; mpmath 50-digit χ² tails and normal quantiles (tests/golden/significance_pins.txt);
+ * scipy.special.gammaincc / chi2.sf / norm.isf; Exp(1) statistics of normalised noise; injection recovery.
+ * Parity unpinned: the paper's Bonferroni trial count (R15) — a plan parameter, default 1.
+ *
+ * Precision: float32 inputs are widened to double once; everything else is double.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* κ = 1/Φ⁻¹(3/4): PAPER.md:L142 ("scaled by the factor 1/φ⁻¹(3/4)"); Eq. 8 L147 prints 3/2 (garble, R3);
+ * Alg. 1 L648 prints the 5-digit rounding 1.4826. */
+#define ORC_KAPPA 1.4826022185056018
+
+typedef struct {
+    int32_t spectrum; /* index in the batch                                   */
+    int32_t bin;      /* first bin of the window (R10)                        */
+    int32_t width;    /* boxcar width w in [1, zmax] (R9)                     */
+    int32_t pad_;
+    double power;     /* S(bin, width), mean-1 units (R2)                     */
+    double sigma;     /* Gaussian-equivalent significance (R16)               */
+    double lnp;       /* ln of the (Bonferroni-adjusted) p-value              */
+} orc_candidate;
+
+static int cmp_double(const void* a, const void* b) {
+    double x = *(const double*)a, y = *(const double*)b;
+    return (x > y) - (x < y);
+}
+
+/* Median of n values: middle order statistic, or the mean of the two middle ones for even n (R4;
+ * Alg. 1's local_median).  Sorts a scratch copy (library primitive: qsort). */
+double orc_median(const double* v, int64_t n, double* scratch) {
+    memcpy(scratch, v, (size_t)n * sizeof(double));
+    qsort(scratch, (size_t)n, sizeof(double), cmp_double);
+    if (n & 1) return scratch[n / 2];
+    return 0.5 * (scratch[n / 2 - 1] + scratch[n / 2]);
+}
+
+/* Normalise one real sequence of one block in place: (v − median)/(κ·MAD)  (Eq. 8).
+ * MAD = median(|v − median|) (R5).  If κ·MAD is 0 or not finite the block is set to 0 (R7).
+ * Returns the median; *scale_out receives κ·MAD. */
+double orc_normalise_block(double* v, int64_t n, double* scratch, double* dev, double* scale_out) {
+    double med = orc_median(v, n, scratch);
+    for (int64_t k = 0; k < n; ++k) dev[k] = fabs(v[k] - med);
+    double mad = orc_median(dev, n, scratch);
+    double s = ORC_KAPPA * mad;
+    if (scale_out) *scale_out = s;
+    if (!(s > 0.0) || !isfinite(s)) {
+        for (int64_t k = 0; k < n; ++k) v[k] = 0.0;
+    } else {
+        for (int64_t k = 0; k < n; ++k) v[k] = (v[k] - med) / s;
+    }
+    return med;
+}
+
+/* Steps 1-3: blockwise per-component normalisation, then power.
+ * spec: n interleaved (re, im) float32 pairs.  norm_block = B.  Blocks are [jB, (j+1)B) and the last block
+ * extends to n (R6).  Real and imaginary parts are normalised independently, then
+ * P = (re'^2 + im'^2)/2 (PAPER.md:L150 |X'|^2, halved so that noise has mean 1: R2). */
+void orc_normalise_power(const float* spec, int64_t n, int64_t B, double* P) {
+    int64_t nb = n / B;
+    if (nb < 1) nb = 1;
+#pragma omp parallel
+    {
+        int64_t maxlen = n - (nb - 1) * B; /* the last block is the longest: B + (n mod B), or n if nb = 1 */
+        double* re = (double*)malloc((size_t)maxlen * sizeof(double));
+        double* im = (double*)malloc((size_t)maxlen * sizeof(double));
+        double* scratch = (double*)malloc((size_t)maxlen * sizeof(double));
+        double* dev = (double*)malloc((size_t)maxlen * sizeof(double));
+#pragma omp for schedule(dynamic, 4)
+        for (int64_t j = 0; j < nb; ++j) {
+            int64_t lo = j * B;
+            int64_t hi = (j == nb - 1) ? n : (j + 1) * B;
+            int64_t len = hi - lo;
+            for (int64_t k = 0; k < len; ++k) {
+                re[k] = (double)spec[2 * (lo + k)];
+                im[k] = (double)spec[2 * (lo + k) + 1];
+            }
+            orc_normalise_block(re, len, scratch, dev, NULL);
+            orc_normalise_block(im, len, scratch, dev, NULL);
+            for (int64_t k = 0; k < len; ++k) P[lo + k] = 0.5 * (re[k] * re[k] + im[k] * im[k]);
+        }
+        free(re); free(im); free(scratch); free(dev);
+    }
+}
+
+/* Step 4 on its own, for tiny inputs: every boxcar sum by the paper's recursion
+ * Y_k = Y_{k-1}[:end-1] + X[k:end], i.e. S(i,w) = S(i,w-1) + P[i+w-1].
+ * out is [zmax][n] row-major, out[(w-1)*n + i] = S(i,w) for i + w <= n, NaN where the window does not
+ * exist (output length n-w+1, R11). */
+void orc_boxcar_sums(const double* P, int64_t n, int32_t zmax, double* out) {
+    for (int64_t i = 0; i < n; ++i) out[i] = P[i];
+    for (int32_t w = 2; w <= zmax; ++w) {
+        double* cur = out + (int64_t)(w - 1) * n;
+        const double* prev = out + (int64_t)(w - 2) * n;
+        for (int64_t i = 0; i < n; ++i) cur[i] = (i + w <= n) ? prev[i] + P[i + w - 1] : NAN;
+    }
+}
+
+/* Steps 4-5 for one candidate block c = [cC, min((c+1)C, n)) (R12: a window belongs to the block of its first
+ * bin): running sums by the recursion, per-width maximum M(c,w) and lowest arg-max I(c,w) (R14).
+ * M[w-1] = -1 and I[w-1] = -1 when no window of width w starts in the block (R11).  sums: scratch of C doubles. */
+void orc_block_maxima(const double* P, int64_t n, int32_t zmax, int64_t C, int64_t c, double* sums, double* M,
+                      int64_t* I) {
+    int64_t lo = c * C, hi = lo + C;
+    if (hi > n) hi = n;
+    for (int64_t i = lo; i < hi; ++i) sums[i - lo] = 0.0;
+    for (int32_t w = 1; w <= zmax; ++w) {
+        double best = -1.0;
+        int64_t arg = -1;
+        for (int64_t i = lo; i < hi && i + w <= n; ++i) {
+            sums[i - lo] += P[i + w - 1]; /* S(i,w) = S(i,w-1) + P[i+w-1] */
+            if (sums[i - lo] > best) { best = sums[i - lo]; arg = i; }
+        }
+        M[w - 1] = best;
+        I[w - 1] = arg;
+    }
+}
+
+/* ln Q(w,S), Q(w,S) = e^{-S} Σ_{k=0}^{w-1} S^k/k!: the survival function of a χ² variable with 2w degrees of
+ * freedom evaluated at 2S (Eq. 9; a width-w boxcar is the sum of w χ²(2) powers, and in mean-1
+ * units the χ² statistic is 2S, R2).  Evaluated term by term, normalised at the largest term so that nothing
+ * overflows and every term is positive (no cancellation). */
+double orc_ln_q(int32_t w, double S) {
+    if (!(S > 0.0)) return 0.0;
+    int32_t ks = (S >= (double)(w - 1)) ? (w - 1) : (int32_t)floor(S); /* index of the largest term */
+    double sum = 1.0, t = 1.0;
+    for (int32_t k = ks; k >= 1; --k) { t *= (double)k / S; sum += t; }           /* terms ks-1 … 0 */
+    t = 1.0;
+    for (int32_t k = ks + 1; k <= w - 1; ++k) { t *= S / (double)k; sum += t; }   /* terms ks+1 … w-1 */
+    return -S + (double)ks * log(S) - lgamma((double)ks + 1.0) + log(sum);
+}
+
+/* ln of the one-sided normal survival function, ln(½ erfc(x/√2))  (R16). */
+double orc_ln_sf(double x) {
+    if (x < 0.0) return log1p(-0.5 * erfc(-x / M_SQRT2));
+    if (x < 30.0) return log(0.5 * erfc(x / M_SQRT2));
+    /* erfc underflows near x = 38: asymptotic series sf(x) = φ(x)/x · Σ (-1)^k (2k-1)!!/x^{2k} */
+    double x2 = x * x, term = 1.0, sum = 1.0;
+    for (int k = 1; k < 200; ++k) {
+        double next = -term * (double)(2 * k - 1) / x2;
+        if (fabs(next) >= fabs(term) || fabs(next) < 1e-18) break;
+        term = next;
+        sum += term;
+    }
+    return -0.5 * x2 - log(x) - 0.5 * log(2.0 * M_PI) + log(sum);
+}
+
+/* Gaussian-equivalent σ of a p-value given as ln p: the x with ln sf(x) = ln p (R16).  Plain bisection. */
+double orc_sigma_from_lnp(double lnp) {
+    if (!(lnp < 0.0)) return -INFINITY;
+    double lo = -40.0, hi = 1.0;
+    if (orc_ln_sf(lo) < lnp) return lo;
+    while (orc_ln_sf(hi) > lnp) hi *= 2.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (orc_ln_sf(mid) > lnp) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+/* Power S at which a width-w boxcar reaches ln p = lnp_target (used only to check threshold tables). */
+double orc_power_threshold(int32_t w, double lnp_target) {
+    double lo = 0.0, hi = (double)w + 10.0;
+    while (orc_ln_q(w, hi) > lnp_target) hi *= 2.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (orc_ln_q(w, mid) > lnp_target) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+/* The whole path for a batch (steps 1-8).  spectra: [batch][pitch] complex64 as interleaved float32, n bins used
+ * per row.  Returns the number of candidates found; at most cap are written, ordered by (spectrum, bin) (R19).
+ *   per block c, per width w: ln p(c,w) = ln Q(w, M(c,w));  ln p_adj = min(0, ln p + ln n_trials)        (R15)
+ *   w* = the width with the smallest ln p_adj (= the largest σ, σ being a decreasing function of ln p);
+ *        the smallest such w on exact ties                                                            (R13)
+ *   emit (b, I(c,w*), w*, M(c,w*), σ) iff ln p_adj <= ln sf(sigma_threshold)  (σ >= threshold)          (R17)
+ */
+int64_t orc_search(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                   int64_t C, double sigma_threshold, double n_trials, orc_candidate* out, int64_t cap) {
+    int64_t nblk = (n + C - 1) / C;
+    double ln_trials = log(n_trials);
+    double lnp_thr = orc_ln_sf(sigma_threshold);
+    double* P = (double*)malloc((size_t)n * sizeof(double));
+    orc_candidate* blockbest = (orc_candidate*)malloc((size_t)nblk * sizeof(orc_candidate));
+    int64_t found = 0;
+    for (int64_t b = 0; b < batch; ++b) {
+        orc_normalise_power(spectra + 2 * b * pitch, n, B, P);
+#pragma omp parallel
+        {
+            double* sums = (double*)malloc((size_t)C * sizeof(double));
+            double* M = (double*)malloc((size_t)zmax * sizeof(double));
+            int64_t* I = (int64_t*)malloc((size_t)zmax * sizeof(int64_t));
+#pragma omp for schedule(dynamic, 16)
+            for (int64_t c = 0; c < nblk; ++c) {
+                orc_block_maxima(P, n, zmax, C, c, sums, M, I);
+                double best_lnp = INFINITY;
+                int32_t best_w = 0;
+                for (int32_t w = 1; w <= zmax; ++w) {
+                    if (I[w - 1] < 0) continue; /* no window of this width starts in the block */
+                    double lnp = orc_ln_q(w, M[w - 1]) + ln_trials;
+                    if (lnp > 0.0) lnp = 0.0;
+                    if (lnp < best_lnp) { best_lnp = lnp; best_w = w; } /* strict: smallest w on ties */
+                }
+                orc_candidate r;
+                memset(&r, 0, sizeof r);
+                r.spectrum = -1;
+                if (best_w > 0 && best_lnp <= lnp_thr) {
+                    r.spectrum = (int32_t)b;
+                    r.bin = (int32_t)I[best_w - 1];
+                    r.width = best_w;
+                    r.power = M[best_w - 1];
+                    r.lnp = best_lnp;
+                    r.sigma = orc_sigma_from_lnp(best_lnp);
+                }
+                blockbest[c] = r;
+            }
+            free(sums); free(M); free(I);
+        }
+        for (int64_t c = 0; c < nblk; ++c) { /* blocks in order: the list comes out sorted by (spectrum, bin) */
+            if (blockbest[c].spectrum < 0) continue;
+            if (found < cap) out[found] = blockbest[c];
+            ++found;
+        }
+    }
+    free(P); free(blockbest);
+    return found;
+}
+
+int orc_num_threads(void) {
+    int n = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp master
+        n = __builtin_omp_get_num_threads();
+    }
+#endif
+    return n;
+}
+
+double orc_kappa(void) { return ORC_KAPPA; }
