@@ -1,0 +1,131 @@
+/*
+ * pulscan.h — C ABI of libpulscan: the data-parallel hot path of Pulscan (White et al., arXiv 2406.15186),
+ * the unmatched-filter (boxcar) acceleration search over the Fourier spectrum of a dedispersed observation,
+ * as hand-written sm_100a CUDA.  Citations are PAPER.md line numbers; "R<n>" are the readings in DESIGN.md §3.
+ *
+ * What one search computes, per spectrum of a batch (§2.2.3-2.2.5):
+ *   1. per normalisation block, per component (re, im independently): v' = (v − median)/(κ·MAD), κ = 1/Φ⁻¹(¾)
+ *      (L140-148, Eq. 8); exact medians; the last block absorbs n_bins mod norm_block (R6); MAD = 0 → block = 0 (R7)
+ *   2. power P = (re'² + im'²)/2 (L150; halved so that noise has mean 1, R2)
+ *   3. boxcar sums S(i,w) = Σ_{j<w} P[i+j] for every width w in [1, zmax] and every bin i with i + w ≤ n_bins
+ *      (L152, L169-199; R9-R11)
+ *   4. per candidate block c = [c·block_width, (c+1)·block_width) of start bins and per width: the maximum and
+ *      its lowest arg-max (Alg. 4; R12, R14)
+ *   5. ln p = ln Q(w, S): χ² survival with 2w degrees of freedom at 2S (L154-158, Eq. 9), plus ln n_trials
+ *      (Bonferroni, L158, R15); σ = the Gaussian-equivalent significance (L114, L158; R16)
+ *   6. per block the width with the smallest ln p (largest σ; smallest width on ties, R13); the candidate
+ *      (spectrum, bin, width, power, sigma) is emitted iff σ ≥ sigma_threshold (L342-344, L361; R17)
+ * so at most one candidate per (spectrum, candidate block).
+ *
+ * Conventions.  All `d_` pointers are DEVICE pointers, all `h_` pointers are HOST pointers; the library never
+ * takes ownership of either.  Every function returns PULSCAN_OK (0) or a negative error code and never throws;
+ * pulscan_last_error() describes the last failure on the calling thread.  There is no CPU fallback: without a
+ * CUDA device of compute capability 10.x the search functions return PULSCAN_ECUDA / PULSCAN_EARCH.
+ */
+#ifndef PULSCAN_H
+#define PULSCAN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PULSCAN_OK 0
+#define PULSCAN_EINVAL (-1)       /* bad argument (range, null, alignment, plan state)                   */
+#define PULSCAN_ENOWORKSPACE (-2) /* no workspace attached, or it is too small                           */
+#define PULSCAN_ECUDA (-3)        /* a CUDA runtime call or kernel launch failed                         */
+#define PULSCAN_EARCH (-4)        /* the current device is not compute capability 10.x (B200, sm_100a)   */
+
+/* Limits of this build (PULSCAN_EINVAL beyond them). */
+#define PULSCAN_MAX_ZMAX 4096
+#define PULSCAN_MAX_NORM_BLOCK 16384
+#define PULSCAN_MAX_BLOCK_PLUS_ZMAX 24576 /* block_width + zmax: one candidate block + halo in shared memory */
+
+typedef struct pulscan_plan pulscan_plan; /* opaque */
+
+/* One candidate: 20 bytes, no padding.  `bin` is the first bin of the window (R10), `width` = w (the paper's
+ * drift z = w − 1, R9), `power` = S(bin, width) in mean-1 units, `sigma` single-precision (R21). */
+typedef struct {
+    int32_t spectrum;
+    int32_t bin;
+    int32_t width;
+    float power;
+    float sigma;
+} pulscan_candidate;
+
+/* Create a plan for `batch` spectra of `n_bins` complex64 bins each, boxcar widths 1..zmax, candidate blocks of
+ * `block_width` start bins (Alg. 4's chunk_size; L224 "block width is a user defined parameter") and a
+ * Gaussian-σ threshold (L361).  Host-only: touches no CUDA device.  Defaults: norm_block = next power of two
+ * ≥ 16·block_width clamped to [1024, 8192]; n_trials = 1; pitch = n_bins.
+ * Returns NULL on error (n_bins < 2, batch < 1, zmax < 1 or ≥ n_bins or > PULSCAN_MAX_ZMAX, block_width < 1,
+ * block_width + zmax > PULSCAN_MAX_BLOCK_PLUS_ZMAX, sigma_threshold ≤ 0 or not finite, batch·blocks ≥ 2³¹). */
+pulscan_plan* pulscan_plan_create(int64_t n_bins, int32_t batch, int32_t zmax, int32_t block_width,
+                                  float sigma_threshold);
+
+/* Normalisation block B in bins (L142 "the input data is divided into blocks"): 2 ≤ B ≤ PULSCAN_MAX_NORM_BLOCK. */
+int pulscan_plan_set_norm_block(pulscan_plan* plan, int32_t norm_block);
+
+/* Bonferroni trial count N ≥ 1 (L158): p_adj = min(1, N·p).  Default 1 = single-trial σ (R15). */
+int pulscan_plan_set_trials(pulscan_plan* plan, double n_trials);
+
+/* Row stride of the input in complex64 bins, ≥ n_bins.  Default n_bins (dense rows). */
+int pulscan_plan_set_pitch(pulscan_plan* plan, int64_t pitch_bins);
+
+/* Search mode: 0 = pruned sweep (default; exact — cover-sum upper bounds only discard windows that cannot reach
+ * their width's power threshold), 1 = exhaustive sweep (every (bin, width) evaluated; the cross-check). */
+int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode);
+
+/* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
+ * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
+int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);
+
+/* Capacity the caller must give d_candidates: batch · ceil(n_bins / block_width) records. */
+int64_t pulscan_plan_max_candidates(const pulscan_plan* plan);
+
+/* Scratch the caller must provide (device memory, 256-byte aligned): the float32 power intermediate
+ * [batch][power_pitch], the flagged-block list and counters.  With host staging enabled it also holds a device
+ * copy of the input for pulscan_search_host. */
+size_t pulscan_plan_workspace_bytes(const pulscan_plan* plan);
+int pulscan_plan_enable_host_staging(pulscan_plan* plan, int32_t enable);
+int pulscan_plan_set_workspace(pulscan_plan* plan, void* d_workspace, size_t bytes);
+
+/* Run the whole path on the device.  d_spectra: complex64 [batch][pitch] (interleaved re, im float32; 8-byte
+ * aligned; read-only).  d_candidates: pulscan_plan_max_candidates() records.  d_count: one uint32, zeroed by the
+ * call, then the number of candidates.  Enqueues kernels on `cuda_stream` (a cudaStream_t; NULL = default
+ * stream), allocates nothing and does not synchronise; the order of the records is unspecified (R19). */
+int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate* d_candidates, uint32_t* d_count,
+                   void* cuda_stream);
+
+/* The same search from HOST buffers: copies h_spectra (complex64 [batch][pitch]; pinned memory recommended) to
+ * the staging area of the workspace, searches, copies the count and the records back to h_count /
+ * h_candidates (capacity pulscan_plan_max_candidates()) and synchronises the stream before returning.
+ * Requires pulscan_plan_enable_host_staging(plan, 1) before the workspace was sized and attached. */
+int pulscan_search_host(pulscan_plan* plan, const void* h_spectra, pulscan_candidate* h_candidates,
+                        uint32_t* h_count, void* cuda_stream);
+
+/* Steps 1-2 only (normalise + power), for unit tests and profiling: d_power receives float32
+ * [batch][pulscan_plan_power_pitch()] (bins ≥ n_bins of a row are unspecified). */
+int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_power, void* cuda_stream);
+int64_t pulscan_plan_power_pitch(const pulscan_plan* plan);
+
+/* Introspection (host only).  thresholds: h_T[w−1] = the power at which width w reaches the σ threshold
+ * (zmax doubles).  describe: a human-readable dump of the plan (levels of the pruned sweep, sizes); returns the
+ * number of bytes needed including the terminator.  stats: after the stream has been synchronised, h_stats[0] =
+ * candidate blocks flagged by the sweep in the last search, h_stats[1..7] reserved. */
+int pulscan_plan_get_thresholds(const pulscan_plan* plan, double* h_T);
+int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf_bytes);
+int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_stream);
+/* Kernels one pulscan_search() enqueues for this plan (memsets not counted). */
+int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan);
+
+int pulscan_plan_destroy(pulscan_plan* plan);
+
+const char* pulscan_last_error(void);
+const char* pulscan_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PULSCAN_H */

@@ -1,0 +1,572 @@
+// pulscan_api.cu — the C ABI of libpulscan (include/pulscan.h): plan construction (host only), workspace layout,
+// and the enqueue of the three kernels of one search.  No PyTorch, no allocation and no synchronisation on the
+// search path; there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/pulscan.h"
+#include "block_exact.cuh"
+#include "boxcar_sweep.cuh"
+#include "norm_power.cuh"
+#include "significance.cuh"
+
+using namespace pulscan;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_last_error = buf;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                                       \
+    do {                                                                                                     \
+        cudaError_t e_ = (expr);                                                                             \
+        if (e_ != cudaSuccess) return fail(PULSCAN_ECUDA, "%s failed: %s", #expr, cudaGetErrorString(e_));  \
+    } while (0)
+
+// PULSCAN_DEBUG_SYNC=1 in the environment: synchronise after every launch so that a device fault is reported by the
+// launch that caused it (debugging aid; never set on a timed path).
+int debug_sync(const char* what) {
+    static const bool on = std::getenv("PULSCAN_DEBUG_SYNC") != nullptr;
+    if (!on) return PULSCAN_OK;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return fail(PULSCAN_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+    return PULSCAN_OK;
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline int pow2_ceil(int x) { int p = 1; while (p < x) p <<= 1; return p; }
+
+} // namespace
+
+struct pulscan_plan {
+    // user parameters
+    int64_t n = 0;
+    int32_t batch = 0, zmax = 0, C = 0, B = 0;
+    double sigma_thr = 0, n_trials = 1.0;
+    int64_t pitch = 0;
+    int32_t mode = 0;
+    int32_t tile_user = 0;
+    double log10_p_flag = -5.0;
+    bool host_staging = false;
+    // derived (host)
+    bool dirty = true;         // derived tables need (re)building
+    int64_t nblk = 0;          // candidate blocks per spectrum
+    int32_t nb = 0;            // normalisation blocks per spectrum
+    int64_t pitchP = 0;
+    double lnp_thr = 0, ln_trials = 0;
+    std::vector<double> T;     // T_w
+    std::vector<float> Tp;     // conservative float thresholds for the float32 sweep
+    std::vector<float> tau;    // per-level cover thresholds
+    SweepParams sp{};
+    int tiles_per_row = 0;
+    size_t smem_sweep = 0, smem_exh = 0, smem_exact = 0;
+    int exh_len = 0;
+    // normalisation launch shapes
+    int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
+    bool has_tail = false;
+    // workspace (device, caller-owned)
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_stage_in = 0, off_stage_cand = 0,
+           off_stage_count = 0, bitmap_bytes = 0, need_bytes = 0;
+    // device tables (plan-owned, small)
+    double* d_T = nullptr;
+    float* d_Tp = nullptr;
+    float* d_tau = nullptr;
+    bool device_ready = false;
+    int sm_count = 148;
+};
+
+namespace {
+
+// ---------------------------------------------------------------- host-side plan derivation
+float round_down_float(double x) {
+    float f = (float)x;
+    if ((double)f > x) f = std::nextafterf(f, -INFINITY);
+    return f;
+}
+
+// Conservative float32 threshold for a sum of `terms` non-negative float32 addends that must not miss a true
+// (double-precision) sum ≥ T: any summation order loses at most (terms−1)·2⁻²⁴ relative; 2e-6 covers the
+// float32 rounding of the addends themselves.
+float conservative_threshold(double T, int terms) {
+    return round_down_float(T * (1.0 - 2.0 * (double)terms * 5.9604644775390625e-8 - 2e-6));
+}
+
+int derive(pulscan_plan& p) {
+    if (!p.dirty) return PULSCAN_OK;
+    p.nblk = (p.n + p.C - 1) / p.C;
+    p.nb = (int32_t)std::max<int64_t>(1, p.n / p.B);
+    p.pitchP = (int64_t)align_up((size_t)p.n, 4);
+    p.lnp_thr = ln_sf(p.sigma_thr);
+    p.ln_trials = std::log(p.n_trials);
+    const double lnp_target = p.lnp_thr - p.ln_trials; // ln p_adj ≤ lnp_thr ⇔ ln p ≤ lnp_thr − ln N  (R15, R17)
+    p.T.resize(p.zmax);
+    p.Tp.resize(p.zmax);
+    for (int w = 1; w <= p.zmax; ++w) {
+        p.T[w - 1] = power_threshold(w, lnp_target);
+        p.Tp[w - 1] = conservative_threshold(p.T[w - 1], w);
+    }
+
+    // ---- sweep tile
+    int tile = p.tile_user ? p.tile_user : (p.zmax <= 512 ? 4096 : 8192);
+    // ---- group size per width: the largest g = 2^lg whose worst cover (w + 2g − 2 bins) of pure noise passes the
+    //      width's threshold with probability ≤ p_flag; made non-decreasing in w by a suffix minimum.
+    const double ln_pflag = p.log10_p_flag * 2.302585092994046;
+    const int lg_cap = 6;
+    std::vector<int> lgw(p.zmax + 2, 0);
+    for (int w = 1; w <= p.zmax; ++w) {
+        int best = 0;
+        for (int lg = 1; lg <= lg_cap; ++lg) {
+            const int g = 1 << lg, Lc = w + 2 * g - 2;
+            if ((tile >> lg) % kSweepR != 0) break;
+            if (ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
+        }
+        lgw[w] = best;
+    }
+    for (int w = p.zmax - 1; w >= 1; --w) lgw[w] = std::min(lgw[w], lgw[w + 1]);
+
+    SweepParams& sp = p.sp;
+    std::memset(&sp, 0, sizeof sp);
+    p.tau.clear();
+    int nlev = 0, lgmax = 0;
+    for (int w = 1; w <= p.zmax;) {
+        int w2 = w;
+        while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lgw[w]) ++w2;
+        if (nlev >= kMaxLevels) return fail(PULSCAN_EINVAL, "internal: too many sweep levels");
+        SweepLevel& lv = sp.lv[nlev++];
+        lv.lg = lgw[w];
+        lv.wlo = w;
+        lv.whi = w2;
+        const int g = 1 << lv.lg;
+        if (g == 1) { lv.m_lo = w; lv.m_hi = w2; }
+        else {
+            lv.m_lo = (w + g - 1) / g;
+            lv.m_hi = (w2 >= 2) ? (w2 - 2) / g + 2 : 1;
+        }
+        lv.tau_off = (int)p.tau.size();
+        for (int m = 1; m <= lv.m_hi; ++m) {
+            if (m < lv.m_lo) { p.tau.push_back(INFINITY); continue; }
+            const int wmin = (g == 1) ? m : (m == 1 ? 1 : (m - 2) * g + 2);
+            const int wq = std::min(std::max(lv.wlo, wmin), lv.whi);
+            p.tau.push_back(conservative_threshold(p.T[wq - 1], m * g));
+        }
+        lgmax = std::max(lgmax, lv.lg);
+        w = w2 + 1;
+    }
+    sp.nlevels = nlev;
+    sp.lgmax = lgmax;
+    sp.tile = tile;
+    const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
+    sp.len = tile + halo;
+    int off = 0;
+    for (int lg = 0; lg <= lgmax; ++lg) {
+        sp.g_off[lg] = off;
+        off += (int)align_up((size_t)((sp.len >> lg) + kSweepPad), 4);
+    }
+    sp.smem_floats = off;
+    int task = 0;
+    for (int l = 0; l < nlev; ++l) {
+        SweepLevel& lv = sp.lv[l];
+        lv.g_off = sp.g_off[lv.lg];
+        lv.task_off = task;
+        lv.ntasks = ((tile >> lv.lg) + kSweepR - 1) / kSweepR;
+        task += lv.ntasks;
+    }
+    sp.ntasks = task;
+    sp.ntau = (int)p.tau.size();
+    p.tiles_per_row = (int)((p.n + tile - 1) / tile);
+    const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
+    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + 16 + flag_bytes;
+    p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
+    p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
+    p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
+
+    // ---- normalisation launch shapes
+    const int64_t len_last = p.n - (int64_t)(p.nb - 1) * p.B;
+    if (p.B <= 8192) { p.nt_main = 256; p.ept_main = pow2_ceil((p.B + 255) / 256); }
+    else { p.nt_main = 1024; p.ept_main = pow2_ceil((p.B + 1023) / 1024); }
+    p.has_tail = len_last > (int64_t)p.ept_main * p.nt_main || p.nb == 1;
+    if (p.has_tail) {
+        p.nt_tail = len_last <= 256 * 32 ? 256 : 1024;
+        p.ept_tail = pow2_ceil((int)((len_last + p.nt_tail - 1) / p.nt_tail));
+        if (p.ept_tail > 32) return fail(PULSCAN_EINVAL, "last normalisation block too long (%lld bins)", (long long)len_last);
+        p.main_blocks_per_row = p.nb - 1;
+    } else {
+        p.main_blocks_per_row = p.nb;
+    }
+
+    // ---- workspace layout
+    size_t o = 0;
+    p.off_P = o; o += align_up((size_t)p.batch * p.pitchP * 4, 256);
+    p.bitmap_bytes = align_up((size_t)((p.batch * p.nblk + 31) / 32) * 4, 256);
+    p.off_bitmap = o; o += p.bitmap_bytes;
+    p.off_flagged = o; o += align_up((size_t)p.batch * p.nblk * 4, 256);
+    p.off_counters = o; o += 256;
+    if (p.host_staging) {
+        p.off_stage_in = o; o += align_up((size_t)p.batch * p.pitch * 8, 256);
+        p.off_stage_cand = o; o += align_up((size_t)p.batch * p.nblk * sizeof(pulscan_candidate), 256);
+        p.off_stage_count = o; o += 256;
+    }
+    p.need_bytes = o;
+    p.dirty = false;
+    return PULSCAN_OK;
+}
+
+int ensure_device(pulscan_plan& p) {
+    if (p.device_ready) return PULSCAN_OK;
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10)
+        return fail(PULSCAN_EARCH, "device %s is compute capability %d.%d; libpulscan is built for sm_100a only", prop.name,
+                    prop.major, prop.minor);
+    p.sm_count = prop.multiProcessorCount;
+    CUDA_TRY(cudaMalloc(&p.d_T, p.T.size() * sizeof(double)));
+    CUDA_TRY(cudaMalloc(&p.d_Tp, p.Tp.size() * sizeof(float)));
+    CUDA_TRY(cudaMalloc(&p.d_tau, std::max<size_t>(1, p.tau.size()) * sizeof(float)));
+    CUDA_TRY(cudaMemcpy(p.d_T, p.T.data(), p.T.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(p.d_Tp, p.Tp.data(), p.Tp.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(p.d_tau, p.tau.data(), p.tau.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_sweep));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exh));
+    CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exact));
+    p.device_ready = true;
+    return PULSCAN_OK;
+}
+
+void release_device(pulscan_plan& p) {
+    if (p.d_T) cudaFree(p.d_T);
+    if (p.d_Tp) cudaFree(p.d_Tp);
+    if (p.d_tau) cudaFree(p.d_tau);
+    p.d_T = nullptr; p.d_Tp = nullptr; p.d_tau = nullptr;
+    p.device_ready = false;
+}
+
+template <int NT>
+int launch_norm(int ept, int grid, cudaStream_t st, const float2* spectra, long long pitch_in, long long n, int B, int nb,
+                int first_block, int blocks_per_row, float* P, long long pitchP) {
+#define PULSCAN_NORM_CASE(E)                                                                                      \
+    case E:                                                                                                       \
+        norm_power_kernel<E, NT><<<grid, NT, 0, st>>>(spectra, pitch_in, n, B, nb, first_block, blocks_per_row, P, \
+                                                      pitchP);                                                    \
+        break;
+    switch (ept) {
+        PULSCAN_NORM_CASE(1)
+        PULSCAN_NORM_CASE(2)
+        PULSCAN_NORM_CASE(4)
+        PULSCAN_NORM_CASE(8)
+        PULSCAN_NORM_CASE(16)
+        PULSCAN_NORM_CASE(32)
+        default: return fail(PULSCAN_EINVAL, "internal: unsupported elements-per-thread %d", ept);
+    }
+#undef PULSCAN_NORM_CASE
+    CUDA_TRY(cudaGetLastError());
+    char what[64];
+    snprintf(what, sizeof what, "norm_power_kernel<%d,%d> grid %d", ept, NT, grid);
+    return debug_sync(what);
+}
+
+int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStream_t st) {
+    const float2* spec = reinterpret_cast<const float2*>(d_spectra);
+    int rc = PULSCAN_OK;
+    if (p.main_blocks_per_row > 0) {
+        const long long grid = (long long)p.main_blocks_per_row * p.batch;
+        if (grid > 2147483647LL) return fail(PULSCAN_EINVAL, "too many normalisation blocks for one launch");
+        rc = (p.nt_main == 256)
+                 ? launch_norm<256>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP)
+                 : launch_norm<1024>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP);
+        if (rc) return rc;
+    }
+    if (p.has_tail) {
+        rc = (p.nt_tail == 256)
+                 ? launch_norm<256>(p.ept_tail, p.batch, st, spec, p.pitch, p.n, p.B, p.nb, p.nb - 1, 1, d_power, p.pitchP)
+                 : launch_norm<1024>(p.ept_tail, p.batch, st, spec, p.pitch, p.n, p.B, p.nb, p.nb - 1, 1, d_power, p.pitchP);
+    }
+    return rc;
+}
+
+int check_plan_ready(pulscan_plan* plan) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    int rc = derive(*plan);
+    if (rc) return rc;
+    if (!plan->ws) return fail(PULSCAN_ENOWORKSPACE, "no workspace attached (pulscan_plan_set_workspace)");
+    if (plan->ws_bytes < plan->need_bytes)
+        return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes attached, %zu needed", plan->ws_bytes, plan->need_bytes);
+    return ensure_device(*plan);
+}
+
+} // namespace
+
+// ---------------------------------------------------------------------------------------------------- C ABI
+extern "C" {
+
+pulscan_plan* pulscan_plan_create(int64_t n_bins, int32_t batch, int32_t zmax, int32_t block_width,
+                                  float sigma_threshold) {
+    auto bad = [](const char* fmt, auto... a) -> pulscan_plan* { fail(PULSCAN_EINVAL, fmt, a...); return nullptr; };
+    if (n_bins < 2 || n_bins > 2147483647LL) return bad("n_bins = %lld out of range [2, 2^31)", (long long)n_bins);
+    if (batch < 1) return bad("batch = %d < 1", batch);
+    if (zmax < 1 || zmax > PULSCAN_MAX_ZMAX) return bad("zmax = %d out of range [1, %d]", zmax, PULSCAN_MAX_ZMAX);
+    if ((int64_t)zmax >= n_bins) return bad("zmax = %d must be < n_bins = %lld", zmax, (long long)n_bins);
+    if (block_width < 1) return bad("block_width = %d < 1", block_width);
+    if ((int64_t)block_width + zmax > PULSCAN_MAX_BLOCK_PLUS_ZMAX)
+        return bad("block_width + zmax = %lld exceeds %d", (long long)block_width + zmax, PULSCAN_MAX_BLOCK_PLUS_ZMAX);
+    if (!(sigma_threshold > 0.f) || !std::isfinite(sigma_threshold)) return bad("sigma_threshold must be finite and > 0");
+    const int64_t nblk = (n_bins + block_width - 1) / block_width;
+    if (nblk * batch >= 2147483648LL) return bad("batch · candidate blocks = %lld ≥ 2^31", (long long)(nblk * batch));
+    pulscan_plan* p = new (std::nothrow) pulscan_plan;
+    if (!p) return bad("out of host memory");
+    p->n = n_bins; p->batch = batch; p->zmax = zmax; p->C = block_width; p->sigma_thr = sigma_threshold;
+    p->pitch = n_bins;
+    int nbk = pow2_ceil(16 * block_width);
+    p->B = std::min(8192, std::max(1024, nbk));
+    g_last_error.clear();
+    return p;
+}
+
+int pulscan_plan_set_norm_block(pulscan_plan* plan, int32_t norm_block) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (norm_block < 2 || norm_block > PULSCAN_MAX_NORM_BLOCK)
+        return fail(PULSCAN_EINVAL, "norm_block = %d out of range [2, %d]", norm_block, PULSCAN_MAX_NORM_BLOCK);
+    plan->B = norm_block; plan->dirty = true; release_device(*plan);
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_trials(pulscan_plan* plan, double n_trials) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (!(n_trials >= 1.0) || !std::isfinite(n_trials)) return fail(PULSCAN_EINVAL, "n_trials must be finite and ≥ 1");
+    plan->n_trials = n_trials; plan->dirty = true; release_device(*plan);
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_pitch(pulscan_plan* plan, int64_t pitch_bins) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (pitch_bins < plan->n) return fail(PULSCAN_EINVAL, "pitch = %lld < n_bins = %lld", (long long)pitch_bins, (long long)plan->n);
+    plan->pitch = pitch_bins; plan->dirty = true;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (mode != 0 && mode != 1) return fail(PULSCAN_EINVAL, "mode must be 0 (pruned) or 1 (exhaustive)");
+    plan->mode = mode;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (tile_bins != 0 && (tile_bins < 1024 || tile_bins > 16384 || tile_bins % 512 != 0))
+        return fail(PULSCAN_EINVAL, "tile_bins must be 0 or a multiple of 512 in [1024, 16384]");
+    if (log10_p_flag != 0.0 && !(log10_p_flag <= -2.0 && log10_p_flag >= -9.0))
+        return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -2]");
+    plan->tile_user = tile_bins;
+    plan->log10_p_flag = (log10_p_flag == 0.0) ? -5.0 : log10_p_flag;
+    plan->dirty = true; release_device(*plan);
+    return PULSCAN_OK;
+}
+
+int64_t pulscan_plan_max_candidates(const pulscan_plan* plan) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    return (int64_t)plan->batch * ((plan->n + plan->C - 1) / plan->C);
+}
+
+size_t pulscan_plan_workspace_bytes(const pulscan_plan* plan) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return 0; }
+    if (derive(*const_cast<pulscan_plan*>(plan))) return 0;
+    return plan->need_bytes;
+}
+
+int pulscan_plan_enable_host_staging(pulscan_plan* plan, int32_t enable) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    plan->host_staging = enable != 0; plan->dirty = true;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_workspace(pulscan_plan* plan, void* d_workspace, size_t bytes) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    int rc = derive(*plan);
+    if (rc) return rc;
+    if (!d_workspace) return fail(PULSCAN_EINVAL, "null workspace");
+    if (reinterpret_cast<uintptr_t>(d_workspace) & 255) return fail(PULSCAN_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < plan->need_bytes)
+        return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes given, %zu needed", bytes, plan->need_bytes);
+    plan->ws = d_workspace; plan->ws_bytes = bytes;
+    return PULSCAN_OK;
+}
+
+int64_t pulscan_plan_power_pitch(const pulscan_plan* plan) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    return (int64_t)align_up((size_t)plan->n, 4);
+}
+
+int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_power, void* cuda_stream) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    int rc = derive(*plan);
+    if (rc) return rc;
+    if (!d_spectra || !d_power) return fail(PULSCAN_EINVAL, "null pointer");
+    if (reinterpret_cast<uintptr_t>(d_spectra) & 7) return fail(PULSCAN_EINVAL, "d_spectra must be 8-byte aligned");
+    if (reinterpret_cast<uintptr_t>(d_power) & 15) return fail(PULSCAN_EINVAL, "d_power must be 16-byte aligned");
+    rc = ensure_device(*plan);
+    if (rc) return rc;
+    return enqueue_norm(*plan, d_spectra, d_power, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate* d_candidates, uint32_t* d_count,
+                   void* cuda_stream) {
+    int rc = check_plan_ready(plan);
+    if (rc) return rc;
+    if (!d_spectra || !d_candidates || !d_count) return fail(PULSCAN_EINVAL, "null pointer");
+    if (reinterpret_cast<uintptr_t>(d_spectra) & 7) return fail(PULSCAN_EINVAL, "d_spectra must be 8-byte aligned");
+    if (reinterpret_cast<uintptr_t>(d_candidates) & 3 || reinterpret_cast<uintptr_t>(d_count) & 3)
+        return fail(PULSCAN_EINVAL, "d_candidates / d_count must be 4-byte aligned");
+    pulscan_plan& p = *plan;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char* ws = static_cast<char*>(p.ws);
+    float* d_P = reinterpret_cast<float*>(ws + p.off_P);
+    unsigned* d_bitmap = reinterpret_cast<unsigned*>(ws + p.off_bitmap);
+    unsigned* d_flagged = reinterpret_cast<unsigned*>(ws + p.off_flagged);
+    unsigned* d_counters = reinterpret_cast<unsigned*>(ws + p.off_counters);
+
+    CUDA_TRY(cudaMemsetAsync(d_bitmap, 0, p.bitmap_bytes, st));
+    CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
+    CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
+
+    rc = enqueue_norm(p, d_spectra, d_P, st);                                     // (a)
+    if (rc) return rc;
+
+    const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
+    if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
+    if (p.mode == 0) {
+        boxcar_sweep_kernel<<<(int)grid_b, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
+                                                                             p.nblk, p.d_tau, p.d_Tp, d_bitmap, d_flagged,
+                                                                             d_counters);
+    } else {
+        boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_P, p.pitchP,
+                                                                                p.n, p.tiles_per_row, p.C, p.nblk, p.d_Tp,
+                                                                                d_bitmap, d_flagged, d_counters);
+    }
+    CUDA_TRY(cudaGetLastError());
+    if ((rc = debug_sync(p.mode ? "boxcar_exhaustive_kernel" : "boxcar_sweep_kernel"))) return rc;
+
+    const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
+    const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
+    block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
+                                                                   p.lnp_thr, d_flagged, d_counters, d_candidates, d_count);
+    CUDA_TRY(cudaGetLastError());
+    return debug_sync("block_exact_kernel");
+}
+
+int pulscan_search_host(pulscan_plan* plan, const void* h_spectra, pulscan_candidate* h_candidates, uint32_t* h_count,
+                        void* cuda_stream) {
+    int rc = check_plan_ready(plan);
+    if (rc) return rc;
+    if (!plan->host_staging) return fail(PULSCAN_EINVAL, "host staging not enabled (pulscan_plan_enable_host_staging)");
+    if (!h_spectra || !h_candidates || !h_count) return fail(PULSCAN_EINVAL, "null pointer");
+    pulscan_plan& p = *plan;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char* ws = static_cast<char*>(p.ws);
+    void* d_in = ws + p.off_stage_in;
+    pulscan_candidate* d_cand = reinterpret_cast<pulscan_candidate*>(ws + p.off_stage_cand);
+    uint32_t* d_cnt = reinterpret_cast<uint32_t*>(ws + p.off_stage_count);
+    CUDA_TRY(cudaMemcpyAsync(d_in, h_spectra, (size_t)p.batch * p.pitch * 8, cudaMemcpyHostToDevice, st));
+    rc = pulscan_search(plan, d_in, d_cand, d_cnt, cuda_stream);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(h_count, d_cnt, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (*h_count)
+        CUDA_TRY(cudaMemcpyAsync(h_candidates, d_cand, (size_t)*h_count * sizeof(pulscan_candidate), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_get_thresholds(const pulscan_plan* plan, double* h_T) {
+    if (!plan || !h_T) return fail(PULSCAN_EINVAL, "null pointer");
+    int rc = derive(*const_cast<pulscan_plan*>(plan));
+    if (rc) return rc;
+    std::memcpy(h_T, plan->T.data(), plan->T.size() * sizeof(double));
+    return PULSCAN_OK;
+}
+
+int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf_bytes) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    if (derive(*const_cast<pulscan_plan*>(plan))) return -1;
+    const pulscan_plan& p = *plan;
+    std::string s;
+    char line[512];
+    snprintf(line, sizeof line,
+             "pulscan plan: n_bins=%lld batch=%d zmax=%d block_width=%d norm_block=%d sigma_threshold=%g n_trials=%g pitch=%lld mode=%s\n",
+             (long long)p.n, p.batch, p.zmax, p.C, p.B, p.sigma_thr, p.n_trials, (long long)p.pitch, p.mode ? "exhaustive" : "pruned");
+    s += line;
+    snprintf(line, sizeof line, "norm: %d blocks/row, main <EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.ept_main, p.nt_main,
+             p.main_blocks_per_row, p.has_tail ? "" : " (no tail launch)");
+    s += line;
+    if (p.has_tail) { snprintf(line, sizeof line, "norm tail: <EPT=%d,NT=%d> x 1/row\n", p.ept_tail, p.nt_tail); s += line; }
+    double evals = 0;
+    for (int l = 0; l < p.sp.nlevels; ++l) {
+        const SweepLevel& lv = p.sp.lv[l];
+        const double ev = (double)lv.m_hi / (double)(1 << lv.lg);
+        evals += ev;
+        snprintf(line, sizeof line, "sweep level %d: g=%d widths [%d,%d] covers m=[%d,%d] tasks/tile=%d  (%.3f cover sums per bin)\n", l,
+                 1 << lv.lg, lv.wlo, lv.whi, lv.m_lo, lv.m_hi, lv.ntasks, ev);
+        s += line;
+    }
+    snprintf(line, sizeof line,
+             "sweep: tile=%d len=%d tiles/row=%d smem=%zu B, %.3f cover sums per bin (exhaustive: %d), p_flag=1e%g\n", p.sp.tile,
+             p.sp.len, p.tiles_per_row, p.smem_sweep, evals, p.zmax, p.log10_p_flag);
+    s += line;
+    snprintf(line, sizeof line, "exact: smem=%zu B; workspace=%zu B; T_1=%.4f T_zmax=%.4f\n", p.smem_exact, p.need_bytes, p.T.front(), p.T.back());
+    s += line;
+    const int64_t need = (int64_t)s.size() + 1;
+    if (h_buf && buf_bytes > 0) {
+        const size_t ncopy = (size_t)std::min<int64_t>(buf_bytes - 1, (int64_t)s.size());
+        std::memcpy(h_buf, s.data(), ncopy);
+        h_buf[ncopy] = 0;
+    }
+    return need;
+}
+
+int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_stream) {
+    int rc = check_plan_ready(plan);
+    if (rc) return rc;
+    if (!h_stats) return fail(PULSCAN_EINVAL, "null pointer");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    CUDA_TRY(cudaMemcpyAsync(h_stats, static_cast<char*>(plan->ws) + plan->off_counters, 8 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return PULSCAN_OK;
+}
+
+int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    if (derive(*const_cast<pulscan_plan*>(plan))) return -1;
+    return (plan->main_blocks_per_row > 0 ? 1 : 0) + (plan->has_tail ? 1 : 0) + 2;
+}
+
+int pulscan_plan_destroy(pulscan_plan* plan) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    release_device(*plan);
+    delete plan;
+    return PULSCAN_OK;
+}
+
+const char* pulscan_last_error(void) { return g_last_error.c_str(); }
+const char* pulscan_version(void) { return "pulscan-b200 0.1.0 (sm_100a)"; }
+
+} // extern "C"

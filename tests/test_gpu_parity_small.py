@@ -1,0 +1,162 @@
+"""GPU parity (through the C ABI) against the oracle at sizes the oracle finishes in seconds: several tiles, ragged
+tails, both sweep modes, edge and degenerate cases.  Bins/widths bit-exact, power rel 1e-5, sigma abs 1e-3."""
+import numpy as np
+import pytest
+import torch
+
+from _parity import assert_same_candidates, gpu_search, oracle_search
+from paper_2406_15186_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def noise_spectra(batch, n, seed, scale=50.0, device="cuda"):
+    g = torch.Generator(device="cpu").manual_seed(seed)
+    x = torch.randn(batch, n, 2, generator=g, dtype=torch.float32) * scale
+    return torch.view_as_complex(x).to(device)
+
+
+def bump(spec, row, start, width, factor):
+    spec[row, start:start + width] *= factor
+
+
+@pytest.mark.parametrize("n,B", [(1000, 256), (4097, 1024), (12289, 4096), (8192, 4096), (16385, 8192), (300, 512),
+                                 (40000, 16384), (5000, 100), (2049, 2)])
+def test_normalise_power_matches_oracle(orc, n, B):
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(3, n, seed=n + B)
+    spec[1] = spec[1] * 1e-3 + (5.0 - 2.0j)     # offset and scale differ per row
+    plan = binding.Plan(n, 3, min(8, n - 1), 16, 6.0, norm_block=B)
+    P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
+    plan.destroy()
+    for b in range(3):
+        ref = orc.normalise_power(spec[b].cpu().numpy(), B)
+        err = np.abs(P[b] - ref)
+        # bins whose component sits next to the block median cancel in v − m: absolute floor
+        assert np.all(err <= 1e-5 * ref + 1e-6), f"row {b}: max err {err.max()} at {err.argmax()}"
+
+
+def test_normalise_power_degenerate_blocks(orc):
+    from paper_2406_15186_b200 import binding
+    n, B = 3 * 512 + 7, 512
+    spec = noise_spectra(1, n, seed=5)
+    spec[0, :512] = 3.0 + 4.0j                       # MAD = 0 in both components → power 0 (R7)
+    spec[0, 512:1024].imag.round_()                  # heavy duplicates (quantised) in one component
+    spec.real[0, 1024:1024 + 300] = 7.0              # > half the block identical → MAD = 0 for re only
+    plan = binding.Plan(n, 1, 8, 16, 6.0, norm_block=B)
+    P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
+    plan.destroy()
+    ref = orc.normalise_power(spec[0].cpu().numpy(), B)
+    assert np.all(P[0, :512] == 0)
+    assert np.all(np.abs(P[0] - ref) <= 1e-5 * ref + 1e-6)
+
+
+def test_normalise_power_extreme_ranges(orc):
+    from paper_2406_15186_b200 import binding
+    n, B = 4096, 1024
+    spec = noise_spectra(1, n, seed=6, scale=1.0)
+    spec[0, :1024] *= 1e-30                           # tiny values: linear bucketing scale overflows → key path
+    spec[0, 1024:2048] *= 1e30
+    spec.real[0, 2048] = 3e38                         # one huge outlier stretches the range
+    spec.real[0, 2049] = -3e38
+    plan = binding.Plan(n, 1, 8, 16, 6.0, norm_block=B)
+    P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
+    plan.destroy()
+    ref = orc.normalise_power(spec[0].cpu().numpy(), B)
+    ok = ref < 1e30                                   # the two outliers' own powers (~1e76) overflow float32
+    assert ok.sum() == n - 2
+    bad = np.flatnonzero(np.abs(P[0][ok] - ref[ok]) > 2e-5 * ref[ok] + 1e-6)
+    assert bad.size == 0, f"{bad[:10]} gpu {P[0][ok][bad[:5]]} ref {ref[ok][bad[:5]]}"
+
+
+CASES = [
+    # n, batch, zmax, B, C, thr
+    (4097, 2, 16, 1024, 64, 4.0),
+    (20001, 3, 40, 2048, 100, 4.5),
+    (32769, 1, 32, 1024, 64, 4.0),
+    (9000, 2, 200, 4096, 200, 4.0),
+    (30011, 1, 300, 8192, 1200, 4.0),
+    (5000, 4, 7, 512, 1, 3.5),
+    (777, 2, 100, 256, 5000, 3.0),
+    (2100, 1, 2000, 1024, 50, 3.5),
+]
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,batch,zmax,B,C,thr", CASES)
+def test_search_matches_oracle(orc, n, batch, zmax, B, C, thr, mode):
+    spec = noise_spectra(batch, n, seed=n * 7 + zmax)
+    bump(spec, 0, n // 3, 6, 3.0)
+    bump(spec, batch - 1, n // 2, min(zmax, 60), 1.8)
+    bump(spec, batch - 1, n - 5, 5, 4.0)             # at the very end of the row: truncated windows (R11)
+    gpu, stats = gpu_search(spec, zmax, B, C, thr, mode=mode)
+    ora = oracle_search(orc, spec, zmax, B, C, thr)
+    assert len(ora) > 0
+    assert_same_candidates(gpu, ora, f"n={n} zmax={zmax} mode={mode}")
+    assert stats[0] >= len(ora)                      # every emitting block was flagged by the sweep
+
+
+def test_pruned_equals_exhaustive_on_noise_with_low_threshold(orc):
+    spec = noise_spectra(2, 50001, seed=99)
+    a, _ = gpu_search(spec, 64, 2048, 128, 3.0, mode=0)
+    b, _ = gpu_search(spec, 64, 2048, 128, 3.0, mode=1)
+    assert np.array_equal(a, b) and len(a) > 50
+    assert_same_candidates(a, oracle_search(orc, spec, 64, 2048, 128, 3.0), "thr=3 noise")
+
+
+@pytest.mark.parametrize("tile,lpf", [(1024, -2.0), (2048, -3.0), (8192, -7.0), (16384, -9.0)])
+def test_tuning_never_changes_results(orc, tile, lpf):
+    spec = noise_spectra(1, 40000, seed=123)
+    bump(spec, 0, 17000, 90, 1.7)
+    ref, _ = gpu_search(spec, 150, 4096, 200, 4.0)
+    got, _ = gpu_search(spec, 150, 4096, 200, 4.0, tile=tile, log10_p_flag=lpf)
+    assert np.array_equal(ref, got)
+
+
+def test_pitch_and_trials(orc):
+    spec = noise_spectra(3, 6000, seed=321)
+    bump(spec, 1, 1000, 12, 3.5)
+    gpu, _ = gpu_search(spec, 24, 1024, 50, 3.5, n_bins=5555, n_trials=40.0)
+    ora = oracle_search(orc, spec, 24, 1024, 50, 3.5, n_bins=5555, n_trials=40.0)
+    assert_same_candidates(gpu, ora, "pitch>n, trials=40")
+
+
+def test_empty_result_and_all_zero_input():
+    spec = noise_spectra(2, 30000, seed=8)
+    gpu, stats = gpu_search(spec, 32, 2048, 64, 9.5)
+    assert len(gpu) == 0
+    zeros = torch.zeros(1, 5000, dtype=torch.complex64, device="cuda")
+    gpu, _ = gpu_search(zeros, 32, 1024, 64, 3.0)
+    assert len(gpu) == 0                               # MAD = 0 everywhere → power 0 → nothing (R7)
+
+
+def test_strong_signal_many_flagged_blocks(orc):
+    wl = synth.CONFIGS[2].scaled(n_samples=1 << 18, zmax=200, norm_block=4096, block_width=200, n_fixed_random=0,
+                                 fixed=(synth.Injection(0, 201.3, 0.3, 150.0), synth.Injection(0, 411.0, 0.2, 0.0)), seed=5)
+    X, _ = synth.make_spectra(wl, device="cuda")
+    gpu, _ = gpu_search(X, wl.zmax, wl.norm_block, wl.block_width, 6.0)
+    ora = oracle_search(orc, X, wl.zmax, wl.norm_block, wl.block_width, 6.0)
+    assert len(ora) >= 2
+    assert_same_candidates(gpu, ora, "strong signals")
+
+
+def test_batch_rows_independent_on_gpu():
+    spec = noise_spectra(4, 20000, seed=77)
+    bump(spec, 2, 5000, 20, 2.5)
+    full, _ = gpu_search(spec, 48, 2048, 100, 3.5)
+    for b in range(4):
+        alone, _ = gpu_search(spec[b:b + 1].contiguous(), 48, 2048, 100, 3.5)
+        sub = full[full["spectrum"] == b]
+        assert np.array_equal(alone["bin"], sub["bin"]) and np.array_equal(alone["width"], sub["width"])
+        assert np.array_equal(alone["power"], sub["power"]) and np.array_equal(alone["sigma"], sub["sigma"])
+
+
+def test_config1_full(orc):
+    wl = synth.CONFIGS[1]
+    X, inj = synth.make_spectra(wl)                     # host float64 FFT, as BASELINE config 1 specifies
+    Xd = X.cuda()
+    gpu, _ = gpu_search(Xd, wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    ora = oracle_search(orc, Xd, wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    assert_same_candidates(gpu, ora, "config 1")
+    top = gpu[np.argmax(gpu["sigma"])]
+    assert (int(top["bin"]), int(top["width"])) == (727, 14)
