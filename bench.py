@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Pulscan boxcar-search hot path on B200 (one JSON line on stdout, rank 0).
+
+A "step" is one pass of the whole path (normalise + power, boxcar sweep over every width 1..zmax, exact evaluation of
+marked blocks, significance, threshold, compaction) over one batch of synthetic spectra through `pulscan_search`.
+Workload: BASELINE.json configs[2], the batched 2^22-bin DM-trial config the north_star quotes its target on
+(256 × 4,194,305 complex64 bins = 8.59 GB: larger than L2, so consecutive steps cannot be served from cache).
+`--config k` (1-5) selects another BASELINE config.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+N > 1: one process per GPU under torchrun; every rank searches its own full-size batch (weak scaling, no data-path
+collective: spectra are independent); time = max over ranks, value = all ranks' bins / time.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "fourier_bins_searched_per_sec_at_zmax"
+UNIT = "bins/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config, 1-based (default 3 = configs[2])")
+    ap.add_argument("--batch", type=int, default=0, help="override the config's batch (debugging only)")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--log10-p-flag", type=float, default=0.0)
+    return ap.parse_args()
+
+
+def workload(args):
+    from paper_2406_15186_b200 import synth
+    wl = synth.CONFIGS[args.config]
+    if args.batch:
+        wl = wl.scaled(batch=args.batch)
+    return wl
+
+
+def config_dict(wl, n_gpus):
+    return {
+        "workload": f"BASELINE.json configs[{int(wl.name[3]) - 1}] ({wl.name}): {wl.batch} spectra x {wl.n_bins} complex64 bins "
+                    f"per GPU, zmax={wl.zmax}, norm_block={wl.norm_block}, block_width={wl.block_width}, "
+                    f"sigma_threshold={wl.sigma_threshold}",
+        "n_bins": wl.n_bins, "batch_per_gpu": wl.batch, "zmax": wl.zmax, "norm_block": wl.norm_block,
+        "block_width": wl.block_width, "sigma_threshold": wl.sigma_threshold,
+        "input_bytes_per_gpu": wl.batch * wl.n_bins * 8,
+        "cache": "inputs larger than L2 (no flush needed)" if wl.batch * wl.n_bins * 8 > 256e6 else "L2 flushed between steps",
+        "parallelism": f"dp{n_gpus} over spectra, no collective on the data path",
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=lambda: [self.lines.append(l) for l in self.proc.stdout], daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            p = [x.strip() for x in l.split(",")]
+            if len(p) < 6:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, p[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_hbm_peak():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        try:
+            return float(json.loads(f.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except (ValueError, KeyError):
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def recorded_traffic(kernel: str, cfg: int):
+    """dram bytes per launch of `kernel` from the committed ncu summary (profiles/traffic.json), scaled per bin."""
+    f = ROOT / "profiles" / "traffic.json"
+    if not f.exists():
+        return None
+    try:
+        t = json.loads(f.read_text())
+        return t.get(f"cfg{cfg}", {}).get(kernel)
+    except ValueError:
+        return None
+
+
+def cpu_baseline(wl, X_host_rows, budget_s=15.0):
+    """The oracle, as it stands, on a bounded sample of the same spectra (host rows already in memory)."""
+    import oracle
+    import numpy as np
+    oracle.build()
+    t0 = time.perf_counter()
+    oracle.search(X_host_rows[0], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    t1 = time.perf_counter() - t0
+    extra = int(max(0, min(len(X_host_rows) - 1, round(budget_s / max(t1, 1e-3)) - 1)))
+    t_all, n_sp = t1, 1
+    if extra:
+        t0 = time.perf_counter()
+        oracle.search(np.ascontiguousarray(X_host_rows[1:1 + extra]), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+        t_all += time.perf_counter() - t0
+        n_sp += extra
+    return {"value": n_sp * wl.n_bins / t_all, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{n_sp} of {wl.batch} spectra of the workload ({n_sp * wl.n_bins} bins, all {wl.zmax} widths), "
+                      f"{t_all:.1f} s wall"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores; each step is one spectrum of the workload."""
+    from paper_2406_15186_b200 import dist as pdist, synth
+    rank, _, world = pdist.env_rank_world()
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    wl = workload(args)
+    X, _ = synth.make_spectra(wl, device="cpu", spectra=range(min(wl.batch, 2)))
+    rows = X.numpy()
+    per_step = 1
+    for _ in range(args.warmup):
+        oracle.search(rows[0], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        oracle.search(rows[i % len(rows)], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    dt = time.perf_counter() - t0
+    value = args.steps * per_step * wl.n_bins / dt
+    sample = f"{per_step} spectrum of the workload per step ({wl.n_bins} bins x {wl.zmax} widths)"
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(wl, args.gpus),
+        "bin_widths_per_sec": value * wl.zmax,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as tdist
+    from paper_2406_15186_b200 import binding, dist as pdist, synth
+
+    rank, local_rank, world = pdist.env_rank_world()
+    if world > 1:
+        torch.cuda.set_device(local_rank)
+        tdist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", torch.cuda.current_device())
+    wl = workload(args).scaled(seed=workload(args).seed + 1000 * rank)  # every rank its own spectra
+    X, _ = synth.make_spectra(wl, device=dev)
+    bins = wl.batch * wl.n_bins
+    steps, warm = args.steps, max(args.warmup, 3)
+
+    plan = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
+                        tile=args.tile, log10_p_flag=args.log10_p_flag)
+    plan.attach(dev)
+    plan.set_profiling(warm + steps)
+    stream = torch.cuda.current_stream()
+    for _ in range(warm):
+        plan.search(X, stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(); pdist.barrier(); torch.cuda.synchronize()
+    with ClockSampler(torch.cuda.current_device()) as clk:
+        e0.record(stream)
+        for _ in range(steps):
+            plan.search(X, stream)
+        e1.record(stream)
+        torch.cuda.synchronize(); pdist.barrier(); torch.cuda.synchronize()
+    ms_total = pdist.max_over_ranks(e0.elapsed_time(e1))
+    total_bins = pdist.sum_over_ranks(bins)
+    ms_step = ms_total / steps
+    value = total_bins / (ms_step * 1e-3)
+    n_cand = int(plan.d_count.item())
+    flagged = int(plan.stats()[0])
+
+    # per-kernel device times of the timed steps (CUDA events recorded by the library on the launching stream)
+    prof = np.array([plan.profile(s) for s in range(warm, warm + steps)], dtype=np.float64).mean(axis=0)
+    kernels = {"norm_power_kernel": (prof[1], 12 * bins), "boxcar_sweep_kernel": (prof[2], 4 * bins),
+               "block_exact_kernel": (prof[3], None)}
+    dom = max(("norm_power_kernel", "boxcar_sweep_kernel"), key=lambda k: kernels[k][0])
+    peak, peak_src = measured_hbm_peak()
+    dom_ms, dom_bytes = kernels[dom]
+    achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
+    traffic_per_bin = recorded_traffic(dom, args.config)
+    roofline = {
+        "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": (traffic_per_bin * bins) if traffic_per_bin else None, "peak_source": peak_src,
+        "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": dom_ms,
+        "kernel_ms_all": {"memsets": prof[0], "norm_power_kernel": prof[1], "boxcar_sweep_kernel": prof[2],
+                          "block_exact_kernel": prof[3]},
+        "sweep_achieved": 4 * bins / (prof[2] * 1e-3) / 1e9, "sweep_frac": 4 * bins / (prof[2] * 1e-3) / 1e9 / peak,
+        "path_algorithmic_GBps": 8 * bins / (ms_step * 1e-3) / 1e9 if world == 1 else None,
+        "path_frac": 8 * bins / (ms_step * 1e-3) / 1e9 / peak if world == 1 else None,
+    }
+    launches = plan.launches_per_search * steps
+
+    # end to end through the C ABI with host buffers (H2D of the spectra + D2H of count and records inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        plan_h = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
+                              tile=args.tile, log10_p_flag=args.log10_p_flag, host_staging=True)
+        plan_h.attach(dev)
+        Xh = torch.empty(X.shape, dtype=X.dtype, pin_memory=True)
+        Xh.copy_(X)
+        hc = np.empty(plan_h.max_candidates, dtype=binding.CANDIDATE_DTYPE)
+        rec = plan_h.search_host(Xh, hc)  # warm-up
+        torch.cuda.synchronize(); pdist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            rec = plan_h.search_host(Xh, hc)
+        dt = pdist.max_over_ranks(time.perf_counter() - t0)
+        assert len(rec) == n_cand, "host-buffer search disagrees with device-buffer search"
+        e2e = {"value": total_bins * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(Xh.numel() * 8),
+               "d2h_bytes_per_step": int(4 + 20 * len(rec)), "steps": args.e2e_steps, "ms_per_step": 1e3 * dt / args.e2e_steps}
+        plan_h.destroy()
+        del plan_h
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(wl, X[: min(wl.batch, 96)].cpu().numpy())
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": config_dict(wl, world), "bin_widths_per_sec": value * wl.zmax,
+            "candidates_per_step": n_cand, "blocks_flagged_by_sweep": flagged, "clocks": clk.summary(),
+            "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(out), flush=True)
+    plan.destroy()
+    if world > 1:
+        tdist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and world == 1 and args.impl == "ours":
+        # not under torchrun: launch one process per GPU ourselves
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000), str(Path(__file__).resolve())] + sys.argv[1:]
+        return subprocess.call(cmd)
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -120,6 +120,13 @@ int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_str
 /* Kernels one pulscan_search() enqueues for this plan (memsets not counted). */
 int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan);
 
+/* Per-kernel timing.  set_profiling(n_slots > 0) makes every pulscan_search record CUDA events on its stream
+ * around its stages into slot (search index mod n_slots); get_profile waits for that search and returns
+ * h_ms[0..3] = milliseconds of {workspace memsets, kernel (a) normalise+power, kernel (b) sweep, kernel (c) exact
+ * evaluation + significance + compaction}.  n_slots = 0 (default) records nothing. */
+int pulscan_plan_set_profiling(pulscan_plan* plan, int32_t n_slots);
+int pulscan_plan_get_profile(pulscan_plan* plan, int32_t slot, float* h_ms);
+
 int pulscan_plan_destroy(pulscan_plan* plan);
 
 const char* pulscan_last_error(void);

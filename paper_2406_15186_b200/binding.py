@@ -41,6 +41,8 @@ SIGNATURES = {
     "pulscan_plan_describe": (ctypes.c_int64, [_P, _P, ctypes.c_int64]),
     "pulscan_plan_get_stats": (ctypes.c_int, [_P, _P, _P]),
     "pulscan_plan_launches_per_search": (ctypes.c_int32, [_P]),
+    "pulscan_plan_set_profiling": (ctypes.c_int, [_P, ctypes.c_int32]),
+    "pulscan_plan_get_profile": (ctypes.c_int, [_P, ctypes.c_int32, _P]),
     "pulscan_plan_destroy": (ctypes.c_int, [_P]),
     "pulscan_last_error": (ctypes.c_char_p, []),
     "pulscan_version": (ctypes.c_char_p, []),
@@ -196,6 +198,15 @@ class Plan:
         h = np.zeros(8, dtype=np.uint32)
         _check(self.lib.pulscan_plan_get_stats(self.handle, h.ctypes.data, _stream_ptr(stream)))
         return h
+
+    def set_profiling(self, n_slots: int) -> None:
+        _check(self.lib.pulscan_plan_set_profiling(self.handle, n_slots))
+
+    def profile(self, slot: int) -> np.ndarray:
+        """Milliseconds of {memsets, kernel (a), kernel (b), kernel (c)} of the search recorded in `slot`."""
+        ms = np.zeros(4, dtype=np.float32)
+        _check(self.lib.pulscan_plan_get_profile(self.handle, slot, ms.ctypes.data))
+        return ms
 
     def destroy(self) -> None:
         if getattr(self, "handle", None):

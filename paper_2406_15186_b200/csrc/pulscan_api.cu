@@ -92,6 +92,9 @@ struct pulscan_plan {
     float* d_tau = nullptr;
     bool device_ready = false;
     int sm_count = 148;
+    // optional per-kernel timing: 5 events per slot (start, memsets done, (a) done, (b) done, (c) done)
+    int prof_slots = 0, prof_next = 0;
+    std::vector<cudaEvent_t> prof_events;
 };
 
 namespace {
@@ -251,6 +254,12 @@ int ensure_device(pulscan_plan& p) {
     CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exact));
     p.device_ready = true;
     return PULSCAN_OK;
+}
+
+void release_profiling(pulscan_plan& p) {
+    for (cudaEvent_t e : p.prof_events) cudaEventDestroy(e);
+    p.prof_events.clear();
+    p.prof_next = 0;
 }
 
 void release_device(pulscan_plan& p) {
@@ -445,12 +454,24 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     unsigned* d_flagged = reinterpret_cast<unsigned*>(ws + p.off_flagged);
     unsigned* d_counters = reinterpret_cast<unsigned*>(ws + p.off_counters);
 
+    cudaEvent_t* ev = nullptr;
+    if (p.prof_slots > 0) {
+        if (p.prof_events.empty()) {
+            p.prof_events.resize((size_t)p.prof_slots * 5);
+            for (cudaEvent_t& e : p.prof_events) CUDA_TRY(cudaEventCreate(&e));
+        }
+        ev = &p.prof_events[(size_t)(p.prof_next % p.prof_slots) * 5];
+        ++p.prof_next;
+        CUDA_TRY(cudaEventRecord(ev[0], st));
+    }
     CUDA_TRY(cudaMemsetAsync(d_bitmap, 0, p.bitmap_bytes, st));
     CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
     CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
 
+    if (ev) CUDA_TRY(cudaEventRecord(ev[1], st));
     rc = enqueue_norm(p, d_spectra, d_P, st);                                     // (a)
     if (rc) return rc;
+    if (ev) CUDA_TRY(cudaEventRecord(ev[2], st));
 
     const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
     if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
@@ -465,12 +486,14 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     }
     CUDA_TRY(cudaGetLastError());
     if ((rc = debug_sync(p.mode ? "boxcar_exhaustive_kernel" : "boxcar_sweep_kernel"))) return rc;
+    if (ev) CUDA_TRY(cudaEventRecord(ev[3], st));
 
     const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
     const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
     block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
                                                                    p.lnp_thr, d_flagged, d_counters, d_candidates, d_count);
     CUDA_TRY(cudaGetLastError());
+    if (ev) CUDA_TRY(cudaEventRecord(ev[4], st));
     return debug_sync("block_exact_kernel");
 }
 
@@ -559,8 +582,27 @@ int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan) {
     return (plan->main_blocks_per_row > 0 ? 1 : 0) + (plan->has_tail ? 1 : 0) + 2;
 }
 
+int pulscan_plan_set_profiling(pulscan_plan* plan, int32_t n_slots) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (n_slots < 0 || n_slots > 65536) return fail(PULSCAN_EINVAL, "n_slots out of range [0, 65536]");
+    release_profiling(*plan);
+    plan->prof_slots = n_slots;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_get_profile(pulscan_plan* plan, int32_t slot, float* h_ms) {
+    if (!plan || !h_ms) return fail(PULSCAN_EINVAL, "null pointer");
+    if (slot < 0 || slot >= plan->prof_slots || plan->prof_events.empty() || slot >= plan->prof_next)
+        return fail(PULSCAN_EINVAL, "profiling slot %d not recorded", slot);
+    cudaEvent_t* ev = &plan->prof_events[(size_t)slot * 5];
+    CUDA_TRY(cudaEventSynchronize(ev[4]));
+    for (int k = 0; k < 4; ++k) CUDA_TRY(cudaEventElapsedTime(&h_ms[k], ev[k], ev[k + 1]));
+    return PULSCAN_OK;
+}
+
 int pulscan_plan_destroy(pulscan_plan* plan) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    release_profiling(*plan);
     release_device(*plan);
     delete plan;
     return PULSCAN_OK;

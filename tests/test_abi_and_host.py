@@ -1,0 +1,146 @@
+"""CPU-only checks of the boundary: libpulscan.so loads, exports every symbol include/pulscan.h declares, validates
+its arguments, and its host-side plan logic (thresholds, sweep levels, workspace sizes) is sound.  No compute calls."""
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2406_15186_b200 import build as pbuild
+    pbuild.build()
+    from paper_2406_15186_b200 import binding as b
+    b.load_library()
+    return b
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "pulscan.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(pulscan_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(binding):
+    lib = binding.load_library()
+    names = declared_symbols()
+    assert len(names) >= 20
+    for n in names:
+        assert hasattr(lib, n), f"libpulscan.so does not export {n}"
+    assert sorted(binding.SIGNATURES) == names      # the binding marshals exactly the declared functions
+    assert "sm_100a" in binding.version()
+
+
+def test_candidate_record_layout(binding):
+    assert binding.CANDIDATE_DTYPE.itemsize == 20
+    assert [binding.CANDIDATE_DTYPE.fields[k][1] for k in ("spectrum", "bin", "width", "power", "sigma")] == [0, 4, 8, 12, 16]
+
+
+@pytest.mark.parametrize("args", [
+    (1, 1, 1, 1, 6.0),            # n_bins < 2
+    (100, 0, 8, 10, 6.0),         # batch < 1
+    (100, 1, 0, 10, 6.0),         # zmax < 1
+    (100, 1, 100, 10, 6.0),       # zmax >= n_bins
+    (100000, 1, 5000, 10, 6.0),   # zmax > PULSCAN_MAX_ZMAX
+    (100, 1, 8, 0, 6.0),          # block_width < 1
+    (100000, 1, 4000, 30000, 6.0),  # block_width + zmax too large
+    (100, 1, 8, 10, 0.0),         # sigma_threshold <= 0
+    (100, 1, 8, 10, float("nan")),
+    (2 ** 31 + 5, 1, 8, 10, 6.0),
+])
+def test_plan_create_rejects_bad_arguments(binding, args):
+    with pytest.raises(binding.PulscanError) as e:
+        binding.Plan(*args)
+    assert e.value.code == binding.PULSCAN_EINVAL and len(str(e.value)) > 20
+
+
+def test_setters_validate(binding):
+    p = binding.Plan(10000, 2, 16, 50, 6.0)
+    lib = p.lib
+    assert lib.pulscan_plan_set_norm_block(p.handle, 1) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_norm_block(p.handle, 1 << 20) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_trials(p.handle, 0.5) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_pitch(p.handle, 9999) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_mode(p.handle, 7) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_tuning(p.handle, 1000, 0.0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_tuning(p.handle, 2048, -1.0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_workspace(p.handle, None, 1 << 30) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_workspace(p.handle, 4096 + 8, 1 << 30) == binding.PULSCAN_EINVAL      # misaligned
+    assert lib.pulscan_plan_set_workspace(p.handle, 4096, 16) == binding.PULSCAN_ENOWORKSPACE
+    assert lib.pulscan_search(p.handle, 4096, 4096, 4096, None) == binding.PULSCAN_ENOWORKSPACE         # nothing attached
+    assert lib.pulscan_search(None, 4096, 4096, 4096, None) == binding.PULSCAN_EINVAL
+    assert "workspace" in binding.last_error() or "null" in binding.last_error()
+    assert lib.pulscan_plan_set_norm_block(p.handle, 1024) == 0 and lib.pulscan_plan_set_trials(p.handle, 1e6) == 0
+    p.destroy()
+
+
+def test_default_norm_block_reproduces_baseline_configs(binding):
+    # next power of two >= 16·block_width clamped to [1024, 8192]: 64→1024, 200→4096, 1200→8192, 100→2048
+    for C, B in [(64, 1024), (200, 4096), (1200, 8192), (100, 2048)]:
+        d = binding.Plan(1 << 20, 1, 32, C, 6.0).describe()
+        assert f"norm_block={B} " in d
+
+
+def test_sizes(binding):
+    p = binding.Plan(4194305, 256, 200, 200, 6.0, norm_block=4096)
+    assert p.max_candidates == 256 * 20972
+    assert p.power_pitch == 4194308
+    ws = p.workspace_bytes
+    assert 256 * 4194308 * 4 <= ws <= 256 * 4194308 * 4 + 64e6
+    ph = binding.Plan(4194305, 256, 200, 200, 6.0, norm_block=4096, host_staging=True)
+    assert ph.workspace_bytes >= ws + 256 * 4194305 * 8
+    assert p.launches_per_search == 4      # (a) main + (a) last blocks + (b) + (c)
+    assert binding.Plan(4096 * 8, 2, 16, 64, 6.0, norm_block=4096).launches_per_search == 3   # no ragged last block
+
+
+def test_thresholds_match_survival_function(binding):
+    from scipy import special, stats
+    for thr, trials in [(6.0, 1.0), (7.0, 1.0), (6.0, 1e6)]:
+        p = binding.Plan(100000, 1, 1200, 100, thr, n_trials=trials)
+        T = p.thresholds()
+        assert np.all(np.diff(T) > 0)
+        target = special.log_ndtr(-thr) - np.log(trials)
+        for w in (1, 2, 13, 100, 200, 1200):
+            assert stats.chi2.logsf(2 * T[w - 1], 2 * w) == pytest.approx(target, abs=1e-7)
+        p.destroy()
+    T6 = binding.Plan(100000, 1, 1200, 100, 6.0).thresholds()
+    assert T6[0] == pytest.approx(20.7368, abs=1e-4) and T6[1199] == pytest.approx(1419.6481, abs=1e-4)
+
+
+def _levels(desc):
+    out = []
+    for m in re.finditer(r"sweep level \d+: g=(\d+) widths \[(\d+),(\d+)\] covers m=\[(\d+),(\d+)\]", desc):
+        out.append(tuple(int(x) for x in m.groups()))
+    return out
+
+
+@pytest.mark.parametrize("zmax,thr,lpf", [(32, 6.0, 0.0), (200, 6.0, 0.0), (1200, 6.0, -3.0), (100, 7.0, -8.0), (4096, 3.0, 0.0), (1, 6.0, 0.0)])
+def test_sweep_levels_cover_every_width_exactly_once(binding, zmax, thr, lpf):
+    p = binding.Plan(1 << 22, 1, zmax, 200, thr, log10_p_flag=lpf)
+    lv = _levels(p.describe())
+    assert lv and lv[0][1] == 1 and lv[-1][2] == zmax
+    for a, b in zip(lv, lv[1:]):
+        assert b[1] == a[2] + 1 and b[0] > a[0]          # contiguous widths, growing group size
+    for g, wlo, whi, mlo, mhi in lv:
+        # every window of width w in [wlo, whi] at any alignment is covered by between m_lo and m_hi groups
+        for w in {wlo, whi, (wlo + whi) // 2}:
+            for a in range(g):
+                m = (a + w - 1) // g + 1
+                assert mlo <= m <= mhi
+    p.destroy()
+
+
+def test_pruning_bound_is_an_upper_bound_property():
+    # the sweep's premise: P >= 0, so a window's sum is bounded by the sum of the aligned groups covering it
+    rng = np.random.default_rng(0)
+    P = rng.exponential(size=4096)
+    pre = np.concatenate([[0.0], np.cumsum(P)])
+    for g in (2, 4, 8, 16, 32):
+        for _ in range(200):
+            w = int(rng.integers(1, 300)); i = int(rng.integers(0, 4096 - w))
+            k0, k1 = i // g, (i + w - 1) // g
+            lo, hi = k0 * g, min((k1 + 1) * g, 4096)
+            assert pre[hi] - pre[lo] >= pre[i + w] - pre[i] - 1e-9

@@ -1,0 +1,94 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (one pulscan_search over the
+whole batch), checked against the oracle on sampled spectra (every spectrum of configs 1-2; a seeded sample that
+always includes injected spectra for configs 3-5) plus properties that hold for the whole batch."""
+import numpy as np
+import pytest
+import torch
+
+from _parity import assert_same_candidates
+from paper_2406_15186_b200 import binding, synth
+
+pytestmark = pytest.mark.gpu
+
+
+def full_search(wl, X):
+    plan = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block)
+    plan.attach(X.device)
+    plan.search(X)
+    rec = plan.candidates()
+    flagged = int(plan.stats()[0])
+    plan.destroy()
+    return rec, flagged
+
+
+def check_sample(orc, wl, X, rec, inj, n_noise, seed):
+    injected = sorted({i.spectrum for i in inj})
+    rng = np.random.default_rng(seed)
+    noise = [b for b in rng.permutation(wl.batch).tolist() if b not in injected][:n_noise]
+    sample = sorted(set(injected[:12] + noise))
+    for b in sample:
+        ora = orc.search(X[b].cpu().numpy(), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+        ora["spectrum"] = b
+        assert_same_candidates(rec[rec["spectrum"] == b], ora, f"{wl.name} spectrum {b}")
+    return sample
+
+
+def check_properties(wl, rec, inj):
+    # at most one record per (spectrum, candidate block); every field in range; sigma above the threshold
+    key = rec["spectrum"].astype(np.int64) * (1 << 32) + rec["bin"] // wl.block_width
+    assert len(np.unique(key)) == len(rec)
+    assert rec["bin"].min() >= 0 and np.all(rec["bin"] + rec["width"] <= wl.n_bins)
+    assert rec["width"].min() >= 1 and rec["width"].max() <= wl.zmax
+    assert np.all(rec["sigma"] >= wl.sigma_threshold - 1e-3) and np.all(rec["power"] > 0)
+    # injected signals strong enough to matter are recovered as the top candidate of their spectrum near the expected bin
+    for i in inj:
+        mine = rec[rec["spectrum"] == i.spectrum]
+        expected_power = i.amp ** 2 * wl.n_samples / 4
+        if expected_power < 150 or abs(i.z) + 1 > wl.zmax or abs(i.jerk) > 0:
+            continue
+        assert len(mine), f"injection {i} not detected"
+        top = mine[np.argmax(mine["sigma"])]
+        assert abs(top["bin"] - i.expected_start_bin(wl.t_obs)) <= max(8, 0.15 * abs(i.z)), (i, top)
+
+
+def test_config2_full(orc):
+    wl = synth.CONFIGS[2]
+    X, inj = synth.make_spectra(wl)                     # host float64 FFT (BASELINE config 2)
+    Xd = X.cuda()
+    rec, flagged = full_search(wl, Xd)
+    ora = orc.search(X.numpy(), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    assert_same_candidates(rec, ora, "config 2")
+    assert len(inj) == 3 and sorted(abs(i.z) for i in inj) == [20.0, 80.0, 180.0]
+    check_properties(wl, rec, inj)
+    assert flagged >= len(rec)
+
+
+@pytest.mark.parametrize("cfg,n_noise", [(3, 6), (4, 0), (5, 10)])
+def test_batched_configs_full(orc, cfg, n_noise):
+    wl = synth.CONFIGS[cfg]
+    X, inj = synth.make_spectra(wl, device="cuda")
+    rec, flagged = full_search(wl, X)
+    sample = check_sample(orc, wl, X, rec, inj, n_noise, seed=cfg)
+    assert len(sample) >= min(12, len({i.spectrum for i in inj}))
+    check_properties(wl, rec, inj)
+    # noise-only false alarms: <= n·zmax·sf(thr) per spectrum is an upper bound (overlapping windows are correlated)
+    from scipy import stats
+    injected = {i.spectrum for i in inj}
+    n_noise_cands = int(np.sum(~np.isin(rec["spectrum"], list(injected))))
+    bound = (wl.batch - len(injected)) * wl.n_bins * wl.zmax * stats.norm.sf(wl.sigma_threshold)
+    assert n_noise_cands <= max(3.0, 1.5 * bound + 3 * np.sqrt(bound))
+    del X
+    torch.cuda.empty_cache()
+
+
+def test_host_buffer_entry_point_matches_device_entry_point():
+    wl = synth.CONFIGS[3].scaled(batch=6, frac_injected=0.5)
+    X, _ = synth.make_spectra(wl, device="cuda")
+    rec, _ = full_search(wl, X)
+    plan = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
+                        host_staging=True)
+    plan.attach("cuda")
+    Xh = X.cpu().pin_memory()
+    got = plan.search_host(Xh)
+    plan.destroy()
+    assert np.array_equal(got, rec)
