@@ -33,6 +33,8 @@ struct SelectSmem {
     float out_next;
 };
 
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
 __device__ __forceinline__ unsigned float_key(float v) {
     unsigned b = __float_as_uint(v);
     return b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u);
@@ -213,23 +215,11 @@ __device__ __forceinline__ float normalise_component(float (&v)[EPT], int len, S
     return (s > 0.0 && isfinite(s)) ? (float)(0.70710678118654752440 / s) : 0.f;
 }
 
-// One CTA per normalisation block.  Grid: blocks_per_row · batch CTAs; block j = first_block + (blockIdx.x mod
-// blocks_per_row) of spectrum blockIdx.x / blocks_per_row.  Block j covers bins [jB, (j+1)B), the last block of a
-// row extends to n (R6).  Output: P[row·pitchP + bin] = ((re−m_re)/s_re)² /2 + ((im−m_im)/s_im)² /2, s = κ·MAD;
-// s = 0 or not finite → 0 (R7).
+// One normalisation block by the general path: len values at src → powers at dst.
 template <int EPT, int NT>
-__global__ void __launch_bounds__(NT)
-norm_power_kernel(const float2* __restrict__ spectra, long long pitch_in, long long n, int B, int nb, int first_block,
-                  int blocks_per_row, float* __restrict__ P, long long pitchP) {
-    __shared__ SelectSmem sm;
+__device__ __forceinline__ void norm_block_general(const float2* __restrict__ src, int len, float* __restrict__ dst,
+                                                   SelectSmem& sm) {
     const int tid = threadIdx.x;
-    const long long row = blockIdx.x / blocks_per_row;
-    const int j = first_block + (int)(blockIdx.x % blocks_per_row);
-    const long long lo = (long long)j * B;
-    const long long hi = (j == nb - 1) ? n : lo + B;
-    const int len = (int)(hi - lo);
-    const float2* src = spectra + row * pitch_in + lo;
-
     float re[EPT], im[EPT];
 #pragma unroll
     for (int r = 0; r < EPT; ++r) {
@@ -241,7 +231,6 @@ norm_power_kernel(const float2* __restrict__ spectra, long long pitch_in, long l
     }
     const float inv_re = normalise_component<EPT, NT>(re, len, sm);
     const float inv_im = normalise_component<EPT, NT>(im, len, sm);
-    float* dst = P + row * pitchP + lo;
 #pragma unroll
     for (int r = 0; r < EPT; ++r) {
         const int idx = tid + r * NT;
@@ -249,6 +238,40 @@ norm_power_kernel(const float2* __restrict__ spectra, long long pitch_in, long l
             const float x = re[r] * inv_re, y = im[r] * inv_im;
             dst[idx] = fmaf(x, x, y * y);
         }
+    }
+}
+
+// General kernel: one CTA per normalisation block.  Grid: blocks_per_row · batch CTAs; block j = first_block +
+// (blockIdx.x mod blocks_per_row) of spectrum blockIdx.x / blocks_per_row.  Block j covers bins [jB, (j+1)B), the
+// last block of a row extends to n (R6).  Output: P[row·pitchP + bin] = ((re−m_re)/s_re)²/2 + ((im−m_im)/s_im)²/2,
+// s = κ·MAD; s = 0 or not finite → 0 (R7).  Handles any block length up to EPT·NT.
+template <int EPT, int NT>
+__global__ void __launch_bounds__(NT)
+norm_power_kernel(const float2* __restrict__ spectra, long long pitch_in, long long n, int B, int nb, int first_block,
+                  int blocks_per_row, float* __restrict__ P, long long pitchP) {
+    __shared__ SelectSmem sm;
+    const long long row = blockIdx.x / blocks_per_row;
+    const int j = first_block + (int)(blockIdx.x % blocks_per_row);
+    const long long lo = (long long)j * B;
+    const long long hi = (j == nb - 1) ? n : lo + B;
+    norm_block_general<EPT, NT>(spectra + row * pitch_in + lo, (int)(hi - lo), P + row * pitchP + lo, sm);
+}
+
+// Redo kernel: the blocks the fast kernel declined (redo[e] = row·blocks_per_row + j, all of length B), by the general
+// path.  A fixed small grid loops over the list, whose length is only known on the device.
+template <int EPT, int NT>
+__global__ void __launch_bounds__(NT)
+norm_power_redo_kernel(const float2* __restrict__ spectra, long long pitch_in, int B, int blocks_per_row,
+                       float* __restrict__ P, long long pitchP, const unsigned* __restrict__ redo,
+                       const unsigned* __restrict__ redo_count) {
+    __shared__ SelectSmem sm;
+    const unsigned cnt = *redo_count;
+    for (unsigned e = blockIdx.x; e < cnt; e += gridDim.x) {
+        const unsigned id = redo[e];
+        const long long row = id / (unsigned)blocks_per_row;
+        const long long lo = (long long)(id % (unsigned)blocks_per_row) * B;
+        norm_block_general<EPT, NT>(spectra + row * pitch_in + lo, B, P + row * pitchP + lo, sm);
+        __syncthreads();
     }
 }
 

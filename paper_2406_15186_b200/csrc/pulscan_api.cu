@@ -16,6 +16,7 @@
 #include "block_exact.cuh"
 #include "boxcar_sweep.cuh"
 #include "norm_power.cuh"
+#include "norm_power_fast.cuh"
 #include "significance.cuh"
 
 using namespace pulscan;
@@ -81,10 +82,11 @@ struct pulscan_plan {
     // normalisation launch shapes
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
     bool has_tail = false;
+    bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_fast_kernel
     // workspace (device, caller-owned)
     void* ws = nullptr;
     size_t ws_bytes = 0;
-    size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_stage_in = 0, off_stage_cand = 0,
+    size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_redo = 0, off_stage_in = 0, off_stage_cand = 0,
            off_stage_count = 0, bitmap_bytes = 0, need_bytes = 0;
     // device tables (plan-owned, small)
     double* d_T = nullptr;
@@ -216,6 +218,9 @@ int derive(pulscan_plan& p) {
         p.main_blocks_per_row = p.nb;
     }
 
+    p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.main_blocks_per_row > 0 &&
+                 std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
+
     // ---- workspace layout
     size_t o = 0;
     p.off_P = o; o += align_up((size_t)p.batch * p.pitchP * 4, 256);
@@ -223,6 +228,7 @@ int derive(pulscan_plan& p) {
     p.off_bitmap = o; o += p.bitmap_bytes;
     p.off_flagged = o; o += align_up((size_t)p.batch * p.nblk * 4, 256);
     p.off_counters = o; o += 256;
+    p.off_redo = o; o += align_up((size_t)p.batch * p.nb * 4, 256);
     if (p.host_staging) {
         p.off_stage_in = o; o += align_up((size_t)p.batch * p.pitch * 8, 256);
         p.off_stage_cand = o; o += align_up((size_t)p.batch * p.nblk * sizeof(pulscan_candidate), 256);
@@ -294,15 +300,47 @@ int launch_norm(int ept, int grid, cudaStream_t st, const float2* spectra, long 
     return debug_sync(what);
 }
 
-int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStream_t st) {
+constexpr int kRedoGrid = 148;
+
+// Fast kernel for the full blocks + redo kernel (general path) for the blocks it declined.
+int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* spec, float* P, unsigned* redo,
+                     unsigned* redo_count) {
+#define PULSCAN_FAST_CASE(E)                                                                                          \
+    case E:                                                                                                           \
+        norm_power_fast_kernel<E, 256><<<grid, 256, 0, st>>>(spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo,  \
+                                                             redo_count);                                             \
+        norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P,        \
+                                                                  p.pitchP, redo, redo_count);                        \
+        break;
+    switch (p.ept_main) {
+        PULSCAN_FAST_CASE(1)
+        PULSCAN_FAST_CASE(2)
+        PULSCAN_FAST_CASE(4)
+        PULSCAN_FAST_CASE(8)
+        PULSCAN_FAST_CASE(16)
+        PULSCAN_FAST_CASE(32)
+        default: return fail(PULSCAN_EINVAL, "internal: unsupported elements-per-thread %d", p.ept_main);
+    }
+#undef PULSCAN_FAST_CASE
+    CUDA_TRY(cudaGetLastError());
+    return debug_sync("norm_power_fast_kernel + norm_power_redo_kernel");
+}
+
+// d_scratch: the redo list and its counter (inside the workspace for pulscan_search; a temporary for the stand-alone
+// pulscan_normalise_power, which has no workspace).  redo_count must be zero on entry.
+int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStream_t st, unsigned* d_redo,
+                 unsigned* d_redo_count) {
     const float2* spec = reinterpret_cast<const float2*>(d_spectra);
     int rc = PULSCAN_OK;
     if (p.main_blocks_per_row > 0) {
         const long long grid = (long long)p.main_blocks_per_row * p.batch;
         if (grid > 2147483647LL) return fail(PULSCAN_EINVAL, "too many normalisation blocks for one launch");
-        rc = (p.nt_main == 256)
-                 ? launch_norm<256>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP)
-                 : launch_norm<1024>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP);
+        if (p.use_fast && d_redo)
+            rc = launch_norm_fast(p, (int)grid, st, spec, d_power, d_redo, d_redo_count);
+        else
+            rc = (p.nt_main == 256)
+                     ? launch_norm<256>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP)
+                     : launch_norm<1024>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP);
         if (rc) return rc;
     }
     if (p.has_tail) {
@@ -435,7 +473,14 @@ int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_
     if (reinterpret_cast<uintptr_t>(d_power) & 15) return fail(PULSCAN_EINVAL, "d_power must be 16-byte aligned");
     rc = ensure_device(*plan);
     if (rc) return rc;
-    return enqueue_norm(*plan, d_spectra, d_power, static_cast<cudaStream_t>(cuda_stream));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (plan->ws && plan->ws_bytes >= plan->need_bytes) { // workspace attached: same kernels as pulscan_search
+        char* ws = static_cast<char*>(plan->ws);
+        unsigned* d_counters = reinterpret_cast<unsigned*>(ws + plan->off_counters);
+        CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
+        return enqueue_norm(*plan, d_spectra, d_power, st, reinterpret_cast<unsigned*>(ws + plan->off_redo), d_counters + 1);
+    }
+    return enqueue_norm(*plan, d_spectra, d_power, st, nullptr, nullptr); // no workspace: general kernels only
 }
 
 int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate* d_candidates, uint32_t* d_count,
@@ -469,7 +514,7 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
 
     if (ev) CUDA_TRY(cudaEventRecord(ev[1], st));
-    rc = enqueue_norm(p, d_spectra, d_P, st);                                     // (a)
+    rc = enqueue_norm(p, d_spectra, d_P, st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1); // (a)
     if (rc) return rc;
     if (ev) CUDA_TRY(cudaEventRecord(ev[2], st));
 
@@ -538,8 +583,8 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
              "pulscan plan: n_bins=%lld batch=%d zmax=%d block_width=%d norm_block=%d sigma_threshold=%g n_trials=%g pitch=%lld mode=%s\n",
              (long long)p.n, p.batch, p.zmax, p.C, p.B, p.sigma_thr, p.n_trials, (long long)p.pitch, p.mode ? "exhaustive" : "pruned");
     s += line;
-    snprintf(line, sizeof line, "norm: %d blocks/row, main <EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.ept_main, p.nt_main,
-             p.main_blocks_per_row, p.has_tail ? "" : " (no tail launch)");
+    snprintf(line, sizeof line, "norm: %d blocks/row, main %s<EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.use_fast ? "fast" : "general",
+             p.ept_main, p.nt_main, p.main_blocks_per_row, p.has_tail ? "" : " (no tail launch)");
     s += line;
     if (p.has_tail) { snprintf(line, sizeof line, "norm tail: <EPT=%d,NT=%d> x 1/row\n", p.ept_tail, p.nt_tail); s += line; }
     double evals = 0;
@@ -579,7 +624,7 @@ int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_str
 int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan) {
     if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
     if (derive(*const_cast<pulscan_plan*>(plan))) return -1;
-    return (plan->main_blocks_per_row > 0 ? 1 : 0) + (plan->has_tail ? 1 : 0) + 2;
+    return (plan->main_blocks_per_row > 0 ? (plan->use_fast ? 2 : 1) : 0) + (plan->has_tail ? 1 : 0) + 2;
 }
 
 int pulscan_plan_set_profiling(pulscan_plan* plan, int32_t n_slots) {

@@ -27,11 +27,16 @@ def test_normalise_power_matches_oracle(orc, n, B):
     spec = noise_spectra(3, n, seed=n + B)
     spec[1] = spec[1] * 1e-3 + (5.0 - 2.0j)     # offset and scale differ per row
     plan = binding.Plan(n, 3, min(8, n - 1), 16, 6.0, norm_block=B)
-    P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
+    P_general = plan.normalise_power(spec).cpu().numpy().astype(np.float64)   # no workspace: general kernels
+    plan.attach("cuda")
+    P_fast = plan.normalise_power(spec).cpu().numpy().astype(np.float64)      # as in pulscan_search: fast + redo kernels
+    stats = plan.stats()
     plan.destroy()
+    assert np.array_equal(P_general, P_fast)           # both paths select exactly, then share the arithmetic
+    assert stats[1] <= 1                               # fast-path blocks sent to the redo list
     for b in range(3):
         ref = orc.normalise_power(spec[b].cpu().numpy(), B)
-        err = np.abs(P[b] - ref)
+        err = np.abs(P_fast[b] - ref)
         # bins whose component sits next to the block median cancel in v − m: absolute floor
         assert np.all(err <= 1e-5 * ref + 1e-6), f"row {b}: max err {err.max()} at {err.argmax()}"
 
@@ -44,7 +49,9 @@ def test_normalise_power_degenerate_blocks(orc):
     spec[0, 512:1024].imag.round_()                  # heavy duplicates (quantised) in one component
     spec.real[0, 1024:1024 + 300] = 7.0              # > half the block identical → MAD = 0 for re only
     plan = binding.Plan(n, 1, 8, 16, 6.0, norm_block=B)
+    plan.attach("cuda")
     P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
+    assert plan.stats()[1] >= 1                        # degenerate blocks leave the fast path for the general one
     plan.destroy()
     ref = orc.normalise_power(spec[0].cpu().numpy(), B)
     assert np.all(P[0, :512] == 0)
@@ -60,6 +67,7 @@ def test_normalise_power_extreme_ranges(orc):
     spec.real[0, 2048] = 3e38                         # one huge outlier stretches the range
     spec.real[0, 2049] = -3e38
     plan = binding.Plan(n, 1, 8, 16, 6.0, norm_block=B)
+    plan.attach("cuda")
     P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
     plan.destroy()
     ref = orc.normalise_power(spec[0].cpu().numpy(), B)
