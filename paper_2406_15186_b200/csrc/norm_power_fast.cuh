@@ -31,7 +31,7 @@ struct FastSmem {
     float wmin[2][32], wmax[2][32];
     int sel[2], nb2[2];
     unsigned excl[2], cnt[2];
-    float res_a[2], res_b[2];
+    unsigned res_key[2][2][2];        // [phase][component][rank k, rank k+1] as order-preserving keys
     int fail;
 };
 
@@ -113,38 +113,60 @@ __device__ __forceinline__ void fast_scan(const unsigned* __restrict__ hist, uns
     }
 }
 
+__device__ __forceinline__ unsigned atom_shared_inc(unsigned addr) { // one ATOMS, no compiler-side warp aggregation
+    unsigned old;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(addr) : "memory");
+    return old;
+}
+
+// Copy the values whose packed bucket byte equals `sel` (or `nb2`) to list[].  Per 4-value word one XOR and the
+// zero-byte test (x − 0x01010101) & ~x & 0x80808080; only words with a hit (≈ 4 % of them) do more.
 template <int EPT>
 __device__ __forceinline__ void fast_gather(const float (&v)[EPT], const unsigned (&idx)[(EPT + 3) / 4], int sel, int nb2,
-                                            float* list, unsigned* list_n) {
+                                            float* list, unsigned list_n_addr) {
     const unsigned s4 = (unsigned)sel * 0x01010101u, n4 = (unsigned)nb2 * 0x01010101u;
+    const bool two = nb2 != sel;
 #pragma unroll
     for (int q = 0; q < (EPT + 3) / 4; ++q) {
-        const unsigned m = __vcmpeq4(idx[q], s4) | __vcmpeq4(idx[q], n4);
-        if (m) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (4 * q + j < EPT && (m & (0xFFu << (8 * j)))) {
-                    const unsigned slot = atomicAdd(list_n, 1u);
-                    if (slot < (unsigned)kFastListCap) list[slot] = v[4 * q + j];
-                }
+        const unsigned x = idx[q] ^ s4;
+        unsigned has = (x - 0x01010101u) & ~x & 0x80808080u;
+        if (two) {
+            const unsigned y = idx[q] ^ n4;
+            has |= (y - 0x01010101u) & ~y & 0x80808080u;
+        }
+        while (has) {                                   // lowest flagged byte is always a true match
+            const int j = (__ffs(has) - 1) >> 3;
+            has &= has - 1;
+            const unsigned byte = (idx[q] >> (8 * j)) & 0xFFu;
+            if (byte != (unsigned)sel && byte != (unsigned)nb2) continue;   // borrow artefact above a true match
+            float val = v[4 * q];
+            if (4 * q + 1 < EPT && j == 1) val = v[4 * q + 1];
+            if (4 * q + 2 < EPT && j == 2) val = v[4 * q + 2];
+            if (4 * q + 3 < EPT && j == 3) val = v[4 * q + 3];
+            const unsigned slot = atom_shared_inc(list_n_addr);
+            if (slot < (unsigned)kFastListCap) list[slot] = val;
         }
     }
 }
 
 // Threads [0, NT/2) rank the members of component 0, threads [NT/2, NT) those of component 1 (NT/2 ≥ kFastListCap).
-__device__ __forceinline__ void fast_rank(FastSmem& sm, int c, int t, unsigned kk) {
+// The value of rank r is max{x : #{y < x} ≤ r}; each member counts the members below it and the qualifying ones
+// race with atomicMax on the order-preserving key of the float.  res_key[c][0..1] must be 0 on entry.
+__device__ __forceinline__ void fast_rank(FastSmem& sm, int c, int t, unsigned kk, int phase) {
     const unsigned cnt = sm.cnt[c];
     if ((unsigned)t < cnt) {
         const float x = sm.list[c][t];
-        unsigned rank = 0;
-        for (unsigned j = 0; j < cnt; ++j) {
-            const float y = sm.list[c][j];
-            rank += (y < x || (y == x && j < (unsigned)t)) ? 1u : 0u;
-        }
+        unsigned below = 0;
+        for (unsigned j = 0; j < cnt; ++j) below += (sm.list[c][j] < x) ? 1u : 0u;
         const unsigned target = kk - sm.excl[c];
-        if (rank == target) sm.res_a[c] = x;
-        if (rank == target + 1) sm.res_b[c] = x;
+        const unsigned key = float_key(x);
+        if (below <= target) atomicMax(&sm.res_key[phase][c][0], key);
+        if (below <= target + 1) atomicMax(&sm.res_key[phase][c][1], key);
     }
+}
+
+__device__ __forceinline__ float key_float(unsigned k) {
+    return __uint_as_float(k ^ ((k >> 31) ? 0x80000000u : 0xFFFFFFFFu));
 }
 
 template <int EPT, int NT>
@@ -187,6 +209,7 @@ norm_power_fast_kernel(const float2* __restrict__ spectra, long long pitch_in, i
     // zero the four histograms and the counters; publish the warp extrema
     for (int i = tid; i < 4 * kSelBuckets; i += NT) (&sm.hist[0][0][0])[i] = 0;
     if (tid < 4) (&sm.list_n[0][0])[tid] = 0;
+    if (tid < 8) (&sm.res_key[0][0][0])[tid] = 0;
     if (tid == 0) sm.fail = 0;
     if (lane == 0) {
         sm.wmin[0][warp] = vmin[0]; sm.wmax[0][warp] = vmax[0];
@@ -217,15 +240,15 @@ norm_power_fast_kernel(const float2* __restrict__ spectra, long long pitch_in, i
     }
     if (!bad) {
 #pragma unroll
-        for (int c = 0; c < 2; ++c) fast_gather<EPT>(v[c], idx[c], sm.sel[c], sm.nb2[c], sm.list[c], &sm.list_n[0][c]);
+        for (int c = 0; c < 2; ++c) fast_gather<EPT>(v[c], idx[c], sm.sel[c], sm.nb2[c], sm.list[c], smem_addr(&sm.list_n[0][c]));
         __syncthreads();                                                                 // S4
-        fast_rank(sm, tid >= NT / 2, tid & (NT / 2 - 1), kRank);
+        fast_rank(sm, tid >= NT / 2, tid & (NT / 2 - 1), kRank, 0);
         __syncthreads();                                                                 // S5
         // ---------------- |v − median| and its median (the MAD)
         float dscale[2];
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            const float a = sm.res_a[c], b = kEven ? sm.res_b[c] : a;
+            const float a = key_float(sm.res_key[0][c][0]), b = kEven ? key_float(sm.res_key[0][c][1]) : a;
             const float h = 0.5f * __fsub_rn(b, a);
 #pragma unroll
             for (int r = 0; r < EPT; ++r) v[c][r] = fabsf(__fsub_rn(__fsub_rn(v[c][r], a), h));
@@ -244,13 +267,13 @@ norm_power_fast_kernel(const float2* __restrict__ spectra, long long pitch_in, i
     }
     if (!bad) {
 #pragma unroll
-        for (int c = 0; c < 2; ++c) fast_gather<EPT>(v[c], idx[c], sm.sel[c], sm.nb2[c], sm.list[c], &sm.list_n[1][c]);
+        for (int c = 0; c < 2; ++c) fast_gather<EPT>(v[c], idx[c], sm.sel[c], sm.nb2[c], sm.list[c], smem_addr(&sm.list_n[1][c]));
         __syncthreads();                                                                 // S8
-        fast_rank(sm, tid >= NT / 2, tid & (NT / 2 - 1), kRank);
+        fast_rank(sm, tid >= NT / 2, tid & (NT / 2 - 1), kRank, 1);
         __syncthreads();                                                                 // S9
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            const float a = sm.res_a[c], b = kEven ? sm.res_b[c] : a;
+            const float a = key_float(sm.res_key[1][c][0]), b = kEven ? key_float(sm.res_key[1][c][1]) : a;
             const double s = kKappa * (0.5 * ((double)a + (double)b));
             inv[c] = (s > 0.0 && isfinite(s)) ? (float)(0.70710678118654752440 / s) : 0.f;
         }
