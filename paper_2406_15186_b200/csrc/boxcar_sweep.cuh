@@ -8,12 +8,18 @@
 // blocks in double precision.  Nothing a marked block could emit is lost and an unmarked block cannot emit.
 //
 // The paper's kernel (Alg. 4) does one shared-memory add per (bin, width) — issue-bound, ~2·zmax instructions per
-// bin.  Here the tile (+ zmax halo) is staged in shared memory by one TMA bulk copy and swept with COVER SUMS:
-// P ≥ 0, so a window of width w is bounded above by the sum of the aligned g-bin groups that cover it.  For a level
-// (g, [wlo, whi]) thread t accumulates U(k0,m) = Σ_{k<m} G_g[k0+k] for R consecutive group starts k0 in registers
-// and compares with τ(m) = T'_{max(wlo, (m−2)g+2)} — (n/g)·(whi/g+2) additions instead of n·(whi−wlo+1).  g grows
-// like √w (chosen on the host so that a noise cover passes with probability ≤ p_flag), which makes every level cost
-// O(n).  A cover that passes is refined exactly (its ≤ g² windows summed and compared with their own T'_w).
+// bin.  Here the tile (+ zmax halo) is staged in shared memory by one TMA bulk copy, turned into its prefix sum
+// PP[i] = Σ_{j<i} P[j] once, and swept with COVER SUMS: P ≥ 0, so a window of width w is bounded above by the sum of
+// the aligned g-bin groups that cover it, U(k0,m) = PP[(k0+m)·g] − PP[k0·g].  For a level (g, [wlo, whi]) a thread
+// holds PP at 8 consecutive group starts in registers and slides over m: one FADD + half an FMNMX3 per cover sum,
+// (n/g)·(whi/g+2) cover sums instead of n·(whi−wlo+1) window sums.  g grows like √w (chosen on the host so that a
+// cover of pure noise passes with probability ≤ p_flag), which makes every level cost O(n).  Covers that pass go to a
+// shared-memory work list and are refined afterwards by whole warps: their ≤ g² windows are summed from PP and
+// compared with their own T'_w.
+//
+// Float safety.  PP is a float32 scan; every PP[i] carries at most ~36 roundings of magnitude
+// ≤ 2⁻²⁴·PP[len], so a difference of two entries is off by < slack = kSlackUlps·2⁻²⁴·PP[len] from the exact sum of
+// the float32 powers.  Every comparison adds the slack on the side that keeps the cover / window.
 //
 // Exhaustive mode (the cross-check) evaluates every (i, w) by the paper's recursion instead.
 #pragma once
@@ -23,30 +29,39 @@
 namespace pulscan {
 
 constexpr int kMaxLevels = 8;
-constexpr int kSweepR = 8;      // consecutive group starts per thread (register sliding window)
 constexpr int kSweepThreads = 256;
-constexpr int kSweepPad = 2 * kSweepR; // zero entries after each group array (sliding-window over-read)
+constexpr int kSweepR = 8;                 // consecutive group starts per thread
+constexpr int kScanPer = 20;               // floats per thread per scan pass: 80-byte lane stride is bank-conflict-free
+constexpr int kScanPass = kScanPer * kSweepThreads;
+constexpr int kWorkCap = 384;              // flagged (8 group starts × 4 cover lengths) cells per tile before giving up
+constexpr int kPadG = 16;                  // replicated entries after each decimated prefix array (window over-read)
+constexpr float kSlackUlps = 96.f;         // ≥ 2·(19 + 5 + 7 + 3 + passes) + 1 roundings, see above
 
 struct SweepLevel {
     int lg;        // log2 of the group size g
     int wlo, whi;  // widths this level answers for
     int m_lo;      // smallest number of groups a cover of a width-wlo window has
     int m_hi;      // largest number of groups a cover of a width-whi window has
-    int tau_off;   // offset of τ[0..m_hi) in the τ table (τ[m−1] ↔ cover of m groups; +inf below m_lo)
-    int g_off;     // offset (floats) of this level's group array in shared memory
-    int task_off;  // first flattened task index of this level
-    int ntasks;    // ceil(tile/g / R)
+    int m_start;   // m_lo rounded down to a multiple of 4 (16-byte alignment of the sliding window's vector loads)
+    int nsteps;    // 4-wide steps over m: m_start + 4·nsteps > m_hi; ≤ 33; τ = +inf below m_lo and above m_hi
+    int tau_off;   // offset of τ[m_start ..] in the τ table (4·nsteps entries)
+    int pg_off;    // offset (floats) of this level's decimated prefix array PG[k] = PP[k·g] in shared memory
+    int nk;        // group starts per tile = tile / g
+    int wt_off;    // first warp-task of this level; a warp-task is 32 lanes × 8 group starts
+    int nwt;       // warp-tasks of this level
 };
 
 struct SweepParams {
     int nlevels;
-    int lgmax;      // arrays for lg = 0..lgmax are built
-    int tile;       // start bins per CTA
-    int len;        // tile + halo, multiple of 64
-    int ntasks;
+    int tile;        // start bins per CTA
+    int len;         // tile + halo, multiple of 64; halo ≥ zmax + 2·g_max
+    int ntasks;      // warp-tasks per tile (levels are ordered by decreasing cost)
     int ntau;
-    int smem_floats; // data floats (group arrays incl. pads)
-    int g_off[8];    // offsets of the group arrays for lg = 0..7
+    int narr;        // decimated arrays: one per distinct group size
+    int arr_lg[kMaxLevels];
+    int arr_off[kMaxLevels];
+    int z_floats;    // floats of the PP region (4 + len + pad)
+    int smem_floats; // PP region + decimated arrays
     SweepLevel lv[kMaxLevels];
 };
 
@@ -95,82 +110,190 @@ __device__ __forceinline__ void load_tile(float* sP, const float* __restrict__ P
     __syncthreads();
 }
 
-// U(k0,m) for R consecutive k0 = base..base+R−1 and m = 1..m_hi; returns max over (k0, m) of U − τ[m−1].
-template <int R>
-__device__ __forceinline__ float sweep_task(const float* __restrict__ G, int base, int m_hi,
-                                            const float* __restrict__ tau) {
-    float buf[R], U[R];
+// ---------------------------------------------------------------------------------------------------------------
+// Prefix scan.  Z is the PP region: Z[3] = PP[0] = 0 and Z[4+i] = Σ_{j≤i} P[j], i.e. PP[i] = Z[3+i] for i ∈ [0, len].
+// `fetch(i4)` returns the four powers P[4·i4 .. 4·i4+3] of the tile (zeros beyond the row's end); for the in-place
+// variant it reads Z+4 itself, which is safe because every read of a pass happens before the pass's barrier and every
+// write after it, and a pass only writes where it (or an earlier pass) has read.
+// The decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg], are written straight from the scan registers
+// (each thread owns 20 consecutive entries, so the multiples of g among them are known), followed by kPadG copies of
+// PP[len]: a cover that reaches past the staged bins gains nothing.
+// Returns PP[len] (the largest entry) in every thread.  Ends with a CTA barrier.
+struct ScanSmem {
+    float wtot[kSweepThreads / 32];
+};
+
+template <class Fetch>
+__device__ __forceinline__ float scan_tile(const SweepParams& sp, float* Z, float* sG, ScanSmem& ss, Fetch fetch) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int len = sp.len;
+    float carry = 0.f;
+    if (tid == 0) Z[3] = 0.f;
+    if (tid < sp.narr) sG[sp.arr_off[tid]] = 0.f;
+    for (int base = 0; base < len; base += kScanPass) {
+        const int i0 = base + kScanPer * tid;
+        float x[kScanPer];
 #pragma unroll
-    for (int j = 0; j < R; ++j) { buf[j] = G[base + j]; U[j] = 0.f; }
-    float flag = -INFINITY;
-    for (int m0 = 0; m0 < m_hi; m0 += R) {
+        for (int q = 0; q < kScanPer / 4; ++q) {
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (i0 + 4 * q < len) v = fetch((i0 >> 2) + q);
+            x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+        }
 #pragma unroll
-        for (int s = 0; s < R; ++s) {
-            const int m = m0 + s;
-            if (m < m_hi) {
+        for (int j = 1; j < kScanPer; ++j) x[j] += x[j - 1];
+        float incl = x[kScanPer - 1];
 #pragma unroll
-                for (int r = 0; r < R; ++r) U[r] += buf[(r + s) % R];
-                float mx = U[0];
+        for (int off = 1; off < 32; off <<= 1) {
+            const float t = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += t;
+        }
+        float excl = __shfl_up_sync(0xffffffffu, incl, 1);
+        if (lane == 0) excl = 0.f;
+        if (lane == 31) ss.wtot[warp] = incl;
+        __syncthreads();
+        float wbase = 0.f, total = 0.f;
 #pragma unroll
-                for (int r = 1; r < R; ++r) mx = fmaxf(mx, U[r]);
-                flag = fmaxf(flag, mx - tau[m]);
-                buf[s] = G[base + R + m];
+        for (int w = 0; w < kSweepThreads / 32; ++w) {
+            const float t = ss.wtot[w];
+            if (w < warp) wbase += t;
+            total += t;
+        }
+        const float off = carry + (wbase + excl);
+#pragma unroll
+        for (int j = 0; j < kScanPer; ++j) x[j] += off;     // x[j] = PP[i0 + j + 1]
+        if (i0 < len) {
+#pragma unroll
+            for (int q = 0; q < kScanPer / 4; ++q)
+                if (i0 + 4 * q < len)
+                    reinterpret_cast<float4*>(Z + 4)[(i0 >> 2) + q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
+            for (int a = 0; a < sp.narr; ++a) {
+                const int lg = sp.arr_lg[a];
+                float* dst = sG + sp.arr_off[a];
+                if (lg >= 2) {              // candidates: PP[i0 + 4q + 4]
+                    const int gm = (1 << lg) - 1;
+#pragma unroll
+                    for (int q = 0; q < kScanPer / 4; ++q) {
+                        const int pos = i0 + 4 * q + 4;
+                        if ((pos & gm) == 0 && pos <= len) dst[pos >> lg] = x[4 * q + 3];
+                    }
+                } else if (lg == 1) {
+#pragma unroll
+                    for (int q = 0; q < kScanPer / 2; ++q) {
+                        const int pos = i0 + 2 * q + 2;
+                        if (pos <= len) dst[pos >> 1] = x[2 * q + 1];
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < kScanPer; ++j)
+                        if (i0 + j + 1 <= len) dst[i0 + j + 1] = x[j];
+                }
             }
         }
+        carry += total;
+        if (base + kScanPass >= len && tid < kPadG * sp.narr) {   // last pass: carry = PP[len]
+            const int a = tid / kPadG;
+            sG[sp.arr_off[a] + (len >> sp.arr_lg[a]) + 1 + (tid % kPadG)] = carry;
+        }
+        __syncthreads();
     }
-    return flag;
+    return carry;
+}
+
+// One 4-wide step over m for 8 group starts.  O is the rotation of the 12-entry window W (compile time, so that the
+// window never moves between registers): W[(O + j) % 12] = PG[k0b + m + j], j = 0..11 after the load below.
+template <int O>
+__device__ __forceinline__ bool sweep_step(const float (&A)[kSweepR], float (&W)[12], const float* __restrict__ pg_next,
+                                           const float* __restrict__ tau4) {
+    const float4 nw = *reinterpret_cast<const float4*>(pg_next);
+    W[(O + 8) % 12] = nw.x; W[(O + 9) % 12] = nw.y; W[(O + 10) % 12] = nw.z; W[(O + 11) % 12] = nw.w;
+    const float4 t = *reinterpret_cast<const float4*>(tau4);
+    const float tq[4] = {t.x, t.y, t.z, t.w};
+    bool hit = false;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        float u[kSweepR];
+#pragma unroll
+        for (int r = 0; r < kSweepR; ++r) u[r] = W[(O + q + r) % 12] - A[r];
+        const float m0 = fmaxf(fmaxf(u[0], u[1]), u[2]);
+        const float m1 = fmaxf(fmaxf(u[3], u[4]), u[5]);
+        const float m2 = fmaxf(fmaxf(u[6], u[7]), m0);
+        hit = hit || (fmaxf(m1, m2) >= tq[q]);
+    }
+    return hit;
+}
+
+// All covers of one level for 8 consecutive group starts k0b..k0b+7: returns the bit mask of the 4-wide m steps in
+// which some cover reached its threshold (slack already folded into A).
+__device__ __forceinline__ unsigned sweep_task(const float* __restrict__ PG, int k0b, int m_start, int nsteps,
+                                               const float* __restrict__ tau, float slack) {
+    float A[kSweepR], W[12];
+    {
+        const float4 a0 = *reinterpret_cast<const float4*>(PG + k0b);
+        const float4 a1 = *reinterpret_cast<const float4*>(PG + k0b + 4);
+        A[0] = a0.x - slack; A[1] = a0.y - slack; A[2] = a0.z - slack; A[3] = a0.w - slack;
+        A[4] = a1.x - slack; A[5] = a1.y - slack; A[6] = a1.z - slack; A[7] = a1.w - slack;
+        const float* p = PG + k0b + m_start;
+        const float4 w0 = *reinterpret_cast<const float4*>(p);
+        const float4 w1 = *reinterpret_cast<const float4*>(p + 4);
+        W[0] = w0.x; W[1] = w0.y; W[2] = w0.z; W[3] = w0.w; W[4] = w1.x; W[5] = w1.y; W[6] = w1.z; W[7] = w1.w;
+        W[8] = W[9] = W[10] = W[11] = 0.f;
+    }
+    unsigned mask = 0;
+    const float* p = PG + k0b + m_start + 8;
+    for (int s = 0; s < nsteps; s += 3) {
+        if (sweep_step<0>(A, W, p, tau)) mask |= 1u << s;
+        if (s + 1 < nsteps && sweep_step<4>(A, W, p + 4, tau + 4)) mask |= 2u << s;
+        if (s + 2 < nsteps && sweep_step<8>(A, W, p + 8, tau + 8)) mask |= 4u << s;
+        p += 12; tau += 12;
+    }
+    return mask;
 }
 
 struct SweepCtx {
-    const float* sP;
+    const float* Z;         // PP region (PP[i] = Z[3+i])
     const float* Tp;        // global: T'_w, w = 1..zmax (conservative float thresholds)
     unsigned char* sflag;   // shared: one byte per candidate block touched by the tile
-    long long t0, n;
+    int t0, n;              // n_bins < 2^31 (pulscan_plan_create)
     int tile, C;
-    long long c_first;      // first candidate block of the tile
+    int c_first;            // first candidate block of the tile
+    float slack;
 };
 
-// A cover of m+1 groups starting at group k0 passed its bound: sum its windows exactly (float32) and mark the
-// candidate block of every start bin that owns a window with S ≥ T'_w.
-__device__ __noinline__ void refine_cover(const SweepCtx& cx, const SweepLevel& lv, const float* __restrict__ G,
-                                          int k0, int m) {
+// One work-list cell (level L, group starts k0b..k0b+7, cover lengths m4..m4+3), one cover per lane: re-test it and sum
+// the windows of every cover that passes, all 32 lanes sharing the ≤ g² (start, end) pairs.
+__device__ __forceinline__ void refine_cell(const SweepCtx& cx, const SweepLevel& lv, const float* __restrict__ PG,
+                                            const float* __restrict__ tau, int k0b, int step) {
+    const int lane = threadIdx.x & 31;
+    const int k0 = k0b + (lane & 7);
+    const int m = lv.m_start + 4 * step + (lane >> 3);
+    const float U = PG[k0 + m] - PG[k0];
     const int g = 1 << lv.lg;
-    const int i_lo = k0 * g;
-    long long lim = cx.n - cx.t0;
-    int i_hi = i_lo + g;
-    if (i_hi > cx.tile) i_hi = cx.tile;
-    if ((long long)i_hi > lim) i_hi = (int)lim;
-    float inner = 0.f;
-    for (int k = k0 + 1; k < k0 + m; ++k) inner += G[k];
-    const int e_lo = (m == 0) ? i_lo : (k0 + m) * g; // first bin of the last group of the cover
-    for (int i = i_lo; i < i_hi; ++i) {
-        const int cb = (int)((cx.t0 + i) / cx.C - cx.c_first);
-        if (cx.sflag[cb]) continue;
-        float s = inner;
-        if (m > 0)
-            for (int j = i; j < i_lo + g; ++j) s += cx.sP[j];
-        const int e_first = (m == 0) ? i : e_lo;
-        for (int e = e_first; e < e_lo + g; ++e) { // window [i, e]
-            s += cx.sP[e];
-            const int w = e - i + 1;
-            if (w < lv.wlo) continue;
-            if (w > lv.whi || cx.t0 + e >= cx.n) break;
-            if (s >= __ldg(cx.Tp + (w - 1))) { cx.sflag[cb] = 1; break; }
-        }
+    bool live = U + cx.slack >= tau[4 * step + (lane >> 3)];
+    if (live && g <= cx.C) {   // nothing left to find if the (one or two) blocks owning the cover's start bins are marked
+        const int b0 = cx.t0 + (k0 << lv.lg);
+        live = !(cx.sflag[(int)(b0 / cx.C - cx.c_first)] && cx.sflag[(int)((b0 + g - 1) / cx.C - cx.c_first)]);
     }
-}
-
-template <int R>
-__device__ __noinline__ void refine_task(const SweepCtx& cx, const SweepLevel& lv, const float* __restrict__ G,
-                                         int base, const float* __restrict__ tau) {
-    const int g = 1 << lv.lg;
-    for (int r = 0; r < R; ++r) {
-        const int k0 = base + r;
-        if (k0 * g >= cx.tile || cx.t0 + (long long)k0 * g >= cx.n) break;
-        float U = 0.f;
-        for (int m = 0; m < lv.m_hi; ++m) {
-            U += G[k0 + m];
-            if (U >= tau[m]) refine_cover(cx, lv, G, k0, m);
+    unsigned hits = __ballot_sync(0xffffffffu, live);
+    while (hits) {
+        const int src = __ffs(hits) - 1;
+        hits &= hits - 1;
+        const int kk = k0b + (src & 7), mm = lv.m_start + 4 * step + (src >> 3);
+        const int i0 = kk << lv.lg, e0 = (kk + mm - 1) << lv.lg;
+        for (int idx = lane; idx < g * g; idx += 32) {
+            const int i = i0 + (idx >> lv.lg), e = e0 + (idx & (g - 1));
+            const int w = e - i + 1;
+            if (w < 1 || w < lv.wlo || w > lv.whi || cx.t0 + e >= cx.n) continue;
+            const float S = cx.Z[3 + e + 1] - cx.Z[3 + i];
+            if (S + cx.slack >= __ldg(cx.Tp + (w - 1))) cx.sflag[(int)((cx.t0 + i) / cx.C - cx.c_first)] = 1;
+        }
+        if (g <= cx.C) {       // later covers of this cell: drop those whose blocks have just been marked
+            bool dead = false;
+            if (hits >> lane & 1u) {
+                const int b0 = cx.t0 + (k0 << lv.lg);
+                dead = cx.sflag[(int)(b0 / cx.C - cx.c_first)] && cx.sflag[(int)((b0 + g - 1) / cx.C - cx.c_first)];
+            }
+            __syncwarp();
+            hits &= ~__ballot_sync(0xffffffffu, dead);
         }
     }
 }
@@ -190,63 +313,95 @@ __device__ __forceinline__ void publish_flags(const unsigned char* sflag, int nb
     }
 }
 
+struct SweepCtl {
+    ScanSmem scan;
+    unsigned work[kWorkCap];
+    unsigned task_ctr, work_n;
+    uint64_t mbar;
+};
+
+// The sweep proper, on a tile whose PP region and decimated arrays are ready.  Marks sflag[]; the caller publishes.
+// counters[2] += work-list cells, counters[3] += tiles whose work list overflowed (all their blocks get marked).
+__device__ __forceinline__ void sweep_covers(const SweepParams& sp, const float* __restrict__ Z, const float* __restrict__ sG,
+                                             const float* __restrict__ sTau, SweepCtl& ctl, const SweepCtx& cx,
+                                             int nblk_tile, unsigned* __restrict__ counters) {
+    const int lane = threadIdx.x & 31;
+    // ---- cover sums: warps draw (level, 256 group starts) tasks, most expensive levels first
+    for (;;) {
+        unsigned q = 0;
+        if (lane == 0) q = atomicAdd(&ctl.task_ctr, 1u);
+        q = __shfl_sync(0xffffffffu, q, 0);
+        if (q >= (unsigned)sp.ntasks) break;
+        int L = 0;
+        while (L + 1 < sp.nlevels && (int)q >= sp.lv[L + 1].wt_off) ++L;
+        const SweepLevel& lv = sp.lv[L];
+        const int k0b = (((int)q - lv.wt_off) * 32 + lane) * kSweepR;
+        if (k0b < lv.nk) {
+            unsigned mask = sweep_task(sG + lv.pg_off, k0b, lv.m_start, lv.nsteps, sTau + lv.tau_off, cx.slack);
+            while (mask) {
+                const int s = __ffs(mask) - 1;
+                mask &= mask - 1;
+                const unsigned pos = atomicAdd(&ctl.work_n, 1u);
+                if (pos < (unsigned)kWorkCap) ctl.work[pos] = ((unsigned)L << 28) | ((unsigned)s << 20) | (unsigned)(k0b >> 3);
+            }
+        }
+    }
+    __syncthreads();
+    // ---- refinement of the flagged cells, one warp per cell
+    const unsigned nwork = ctl.work_n;
+    if (nwork > (unsigned)kWorkCap) {
+        for (int i = threadIdx.x; i < nblk_tile; i += kSweepThreads) cx.sflag[i] = 1;
+    } else {
+        for (unsigned e = threadIdx.x >> 5; e < nwork; e += kSweepThreads / 32) {
+            const unsigned w = ctl.work[e];
+            const SweepLevel& lv = sp.lv[w >> 28];
+            refine_cell(cx, lv, sG + lv.pg_off, sTau + lv.tau_off, (int)(w & 0xFFFFFu) << 3, (int)((w >> 20) & 0xFFu));
+        }
+    }
+    if (threadIdx.x == 0 && nwork) {
+        atomicAdd(counters + 2, nwork);
+        if (nwork > (unsigned)kWorkCap) atomicAdd(counters + 3, 1u);
+    }
+    __syncthreads();
+}
+
 // Pruned sweep.  Grid: tiles_per_row · batch CTAs of kSweepThreads; dynamic shared memory:
-//   [smem_floats group arrays][ntau τ][nblk_tile flag bytes][mbarrier].
+//   [z_floats PP region][decimated arrays][ntau τ][SweepCtl][nblk_tile flag bytes].
 __global__ void __launch_bounds__(kSweepThreads)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, int C, long long nblk, const float* __restrict__ tau_g,
                     const float* __restrict__ Tp_g, unsigned* __restrict__ bitmap, unsigned* __restrict__ flagged,
                     unsigned* __restrict__ counters) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float* sG = reinterpret_cast<float*>(smem_raw);
-    float* sTau = sG + sp.smem_floats;
-    uint64_t* mbar = reinterpret_cast<uint64_t*>(sTau + ((sp.ntau + 3) & ~3));
-    unsigned char* sflag = reinterpret_cast<unsigned char*>(mbar + 2);
+    float* Z = reinterpret_cast<float*>(smem_raw);
+    float* sG = Z + sp.z_floats;
+    float* sTau = Z + sp.smem_floats;
+    SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTau + ((sp.ntau + 3) & ~3));
+    unsigned char* sflag = reinterpret_cast<unsigned char*>(&ctl + 1);
 
     const int tid = threadIdx.x;
-    const long long row = blockIdx.x / tiles_per_row;
-    const long long t0 = (long long)(blockIdx.x % tiles_per_row) * sp.tile;
-    const long long c_first = t0 / C;
-    long long last_start = t0 + sp.tile - 1;
-    if (last_start > n - 1) last_start = n - 1;
-    const int nblk_tile = (int)(last_start / C - c_first) + 1;
+    const int row = (int)(blockIdx.x / (unsigned)tiles_per_row);
+    const int t0 = (int)(blockIdx.x - (unsigned)row * (unsigned)tiles_per_row) * sp.tile;   // n < 2^31
+    const int c_first = t0 / C;
+    const int last_start = (int)min((long long)t0 + sp.tile - 1, n - 1);
+    const int nblk_tile = last_start / C - c_first + 1;
 
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
     for (int i = tid; i < nblk_tile; i += kSweepThreads) sflag[i] = 0;
-    load_tile(sG, P + row * pitchP, t0, n, pitchP, sp.len, mbar); // ends with __syncthreads()
+    if (tid == 0) { ctl.task_ctr = 0; ctl.work_n = 0; }
+    load_tile(Z + 4, P + (long long)row * pitchP, t0, n, pitchP, sp.len, &ctl.mbar); // ends with __syncthreads()
 
-    // group arrays: G_lg[k] = G_{lg−1}[2k] + G_{lg−1}[2k+1], plus kSweepPad zeros after each array
-    for (int i = tid; i < kSweepPad; i += kSweepThreads) sG[sp.len + i] = 0.f;
-    for (int lg = 1; lg <= sp.lgmax; ++lg) {
-        const float* src = sG + sp.g_off[lg - 1];
-        float* dst = sG + sp.g_off[lg];
-        const int cnt = sp.len >> lg;
-        for (int k = tid; k < cnt; k += kSweepThreads) {
-            const float2 a = reinterpret_cast<const float2*>(src)[k];
-            dst[k] = a.x + a.y;
-        }
-        for (int i = tid; i < kSweepPad; i += kSweepThreads) dst[cnt + i] = 0.f;
-        __syncthreads();
-    }
-    if (sp.lgmax == 0) __syncthreads();
+    const float4* src = reinterpret_cast<const float4*>(Z + 4);
+    const float pp_max = scan_tile(sp, Z, sG, ctl.scan, [src](int i4) { return src[i4]; });
 
-    SweepCtx cx{sG, Tp_g, sflag, t0, n, sp.tile, C, c_first};
-    for (int task = tid; task < sp.ntasks; task += kSweepThreads) {
-        int L = 0;
-        while (L + 1 < sp.nlevels && task >= sp.lv[L + 1].task_off) ++L;
-        const SweepLevel& lv = sp.lv[L];
-        const int base = (task - lv.task_off) * kSweepR;
-        const float* G = sG + lv.g_off;
-        const float flag = sweep_task<kSweepR>(G, base, lv.m_hi, sTau + lv.tau_off);
-        if (flag >= 0.f) refine_task<kSweepR>(cx, lv, G, base, sTau + lv.tau_off);
-    }
-    __syncthreads();
+    SweepCtx cx{Z, Tp_g, sflag, t0, (int)n, sp.tile, C, c_first, kSlackUlps * 5.9604644775390625e-8f * pp_max};
+    sweep_covers(sp, Z, sG, sTau, ctl, cx, nblk_tile, counters);
     publish_flags(sflag, nblk_tile, c_first, nblk, row, bitmap, flagged, counters);
 }
 
 // Exhaustive sweep (cross-check mode): thread per start bin, the paper's recursion S(i,w) = S(i,w−1) + P[i+w−1]
 // over every width, compared with T'_w.  Same outputs as the pruned kernel.  Dynamic shared memory:
-//   [len floats][zmax T'][nblk_tile flag bytes][mbarrier].
+//   [len floats][zmax T'][mbarrier][nblk_tile flag bytes].
 __global__ void __launch_bounds__(kSweepThreads)
 boxcar_exhaustive_kernel(int tile, int len, int zmax, const float* __restrict__ P, long long pitchP, long long n,
                          int tiles_per_row, int C, long long nblk, const float* __restrict__ Tp_g,

@@ -64,7 +64,7 @@ struct pulscan_plan {
     int64_t pitch = 0;
     int32_t mode = 0;
     int32_t tile_user = 0;
-    double log10_p_flag = -5.0;
+    double log10_p_flag = -3.0;
     bool host_staging = false;
     // derived (host)
     bool dirty = true;         // derived tables need (re)building
@@ -134,72 +134,103 @@ int derive(pulscan_plan& p) {
     int tile = p.tile_user ? p.tile_user : (p.zmax <= 512 ? 4096 : 8192);
     // ---- group size per width: the largest g = 2^lg whose worst cover (w + 2g − 2 bins) of pure noise passes the
     //      width's threshold with probability ≤ p_flag; made non-decreasing in w by a suffix minimum.
-    const double ln_pflag = p.log10_p_flag * 2.302585092994046;
+    //      If the width range then needs more than kMaxLevels levels (very low σ thresholds), p_flag is relaxed
+    //      tenfold at a time: it affects speed only.
     const int lg_cap = 6;
     std::vector<int> lgw(p.zmax + 2, 0);
-    for (int w = 1; w <= p.zmax; ++w) {
-        int best = 0;
-        for (int lg = 1; lg <= lg_cap; ++lg) {
-            const int g = 1 << lg, Lc = w + 2 * g - 2;
-            if ((tile >> lg) % kSweepR != 0) break;
-            if (ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
+    std::vector<SweepLevel> lvls;
+    int lgmax = 0;
+    for (double l10 = p.log10_p_flag;; l10 += 1.0) {
+        const double ln_pflag = l10 * 2.302585092994046;
+        for (int w = 1; w <= p.zmax; ++w) {
+            int best = 0;
+            for (int lg = 1; lg <= lg_cap; ++lg) {
+                const int g = 1 << lg, Lc = w + 2 * g - 2;
+                if ((tile >> lg) % kSweepR != 0) break;
+                if (l10 >= 0.0 || ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
+            }
+            lgw[w] = best;
         }
-        lgw[w] = best;
+        for (int w = p.zmax - 1; w >= 1; --w) lgw[w] = std::min(lgw[w], lgw[w + 1]);
+        lvls.clear();
+        lgmax = 0;
+        bool fits = true;
+        for (int w = 1; w <= p.zmax && fits;) {
+            const int lg = lgw[w], g = 1 << lg;
+            auto m_range = [&](int w2, int& m_lo, int& m_hi) {
+                if (g == 1) { m_lo = w; m_hi = w2; }
+                else { m_lo = (w + g - 1) / g; m_hi = (w2 >= 2) ? (w2 - 2) / g + 2 : 1; }
+            };
+            int w2 = w, m_lo = 0, m_hi = 0;
+            while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lg) {   // extend the run while the m range fits 32 steps of 4
+                m_range(w2 + 1, m_lo, m_hi);
+                if (m_hi - m_lo + 1 > 128) break;
+                ++w2;
+            }
+            m_range(w2, m_lo, m_hi);
+            if ((int)lvls.size() >= kMaxLevels) { fits = false; break; }
+            SweepLevel lv{};
+            lv.lg = lg; lv.wlo = w; lv.whi = w2; lv.m_lo = m_lo; lv.m_hi = m_hi;
+            lv.m_start = m_lo & ~3;
+            lv.nsteps = (m_hi - lv.m_start + 4) / 4;
+            lv.nk = tile >> lg;
+            lv.nwt = (lv.nk + 32 * kSweepR - 1) / (32 * kSweepR);
+            lvls.push_back(lv);
+            lgmax = std::max(lgmax, lg);
+            w = w2 + 1;
+        }
+        if (fits) {   // shared memory of the PP region + one decimated array per distinct (group size, shift)
+            const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
+            size_t fl = (size_t)len + 8;
+            std::vector<int> seen;
+            for (const SweepLevel& lv : lvls)
+                if (std::find(seen.begin(), seen.end(), lv.lg) == seen.end()) {
+                    seen.push_back(lv.lg);
+                    fl += (size_t)(len >> lv.lg) + 1 + kPadG + 3;
+                }
+            if (fl * 4 + 16384 <= 227 * 1024) break;
+        }
+        if (l10 >= 0.0) return fail(PULSCAN_EINVAL, "zmax = %d with tile = %d does not fit the sweep's shared memory", p.zmax, tile);
     }
-    for (int w = p.zmax - 1; w >= 1; --w) lgw[w] = std::min(lgw[w], lgw[w + 1]);
-
     SweepParams& sp = p.sp;
     std::memset(&sp, 0, sizeof sp);
     p.tau.clear();
-    int nlev = 0, lgmax = 0;
-    for (int w = 1; w <= p.zmax;) {
-        int w2 = w;
-        while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lgw[w]) ++w2;
-        if (nlev >= kMaxLevels) return fail(PULSCAN_EINVAL, "internal: too many sweep levels");
-        SweepLevel& lv = sp.lv[nlev++];
-        lv.lg = lgw[w];
-        lv.wlo = w;
-        lv.whi = w2;
-        const int g = 1 << lv.lg;
-        if (g == 1) { lv.m_lo = w; lv.m_hi = w2; }
-        else {
-            lv.m_lo = (w + g - 1) / g;
-            lv.m_hi = (w2 >= 2) ? (w2 - 2) / g + 2 : 1;
+    std::stable_sort(lvls.begin(), lvls.end(), [](const SweepLevel& a, const SweepLevel& b) { return a.nsteps > b.nsteps; });
+    sp.nlevels = (int)lvls.size();
+    sp.tile = tile;
+    const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
+    sp.len = tile + halo;
+    sp.z_floats = (int)align_up((size_t)(4 + sp.len + 4), 4);
+    int off = 0, task = 0;
+    for (int l = 0; l < sp.nlevels; ++l) {
+        SweepLevel& lv = lvls[l];
+        int a = 0;
+        while (a < sp.narr && sp.arr_lg[a] != lv.lg) ++a;
+        if (a == sp.narr) {
+            sp.arr_lg[a] = lv.lg; sp.arr_off[a] = off;
+            off += (int)align_up((size_t)((sp.len >> lv.lg) + 1 + kPadG), 4);
+            ++sp.narr;
         }
+        lv.pg_off = sp.arr_off[a];
+        lv.wt_off = task;
+        task += lv.nwt;
         lv.tau_off = (int)p.tau.size();
-        for (int m = 1; m <= lv.m_hi; ++m) {
-            if (m < lv.m_lo) { p.tau.push_back(INFINITY); continue; }
+        const int g = 1 << lv.lg;
+        for (int m = lv.m_start; m < lv.m_start + 4 * lv.nsteps; ++m) {
+            if (m < lv.m_lo || m > lv.m_hi) { p.tau.push_back(INFINITY); continue; }
             const int wmin = (g == 1) ? m : (m == 1 ? 1 : (m - 2) * g + 2);
             const int wq = std::min(std::max(lv.wlo, wmin), lv.whi);
             p.tau.push_back(conservative_threshold(p.T[wq - 1], m * g));
         }
-        lgmax = std::max(lgmax, lv.lg);
-        w = w2 + 1;
-    }
-    sp.nlevels = nlev;
-    sp.lgmax = lgmax;
-    sp.tile = tile;
-    const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
-    sp.len = tile + halo;
-    int off = 0;
-    for (int lg = 0; lg <= lgmax; ++lg) {
-        sp.g_off[lg] = off;
-        off += (int)align_up((size_t)((sp.len >> lg) + kSweepPad), 4);
-    }
-    sp.smem_floats = off;
-    int task = 0;
-    for (int l = 0; l < nlev; ++l) {
-        SweepLevel& lv = sp.lv[l];
-        lv.g_off = sp.g_off[lv.lg];
-        lv.task_off = task;
-        lv.ntasks = ((tile >> lv.lg) + kSweepR - 1) / kSweepR;
-        task += lv.ntasks;
+        sp.lv[l] = lv;
     }
     sp.ntasks = task;
     sp.ntau = (int)p.tau.size();
+    sp.smem_floats = sp.z_floats + off;
     p.tiles_per_row = (int)((p.n + tile - 1) / tile);
     const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
-    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + 16 + flag_bytes;
+    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + sizeof(SweepCtl) + flag_bytes;
+    if (p.smem_sweep > 227 * 1024) return fail(PULSCAN_EINVAL, "sweep tile needs %zu bytes of shared memory", p.smem_sweep);
     p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
     p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
@@ -369,7 +400,7 @@ extern "C" {
 pulscan_plan* pulscan_plan_create(int64_t n_bins, int32_t batch, int32_t zmax, int32_t block_width,
                                   float sigma_threshold) {
     auto bad = [](const char* fmt, auto... a) -> pulscan_plan* { fail(PULSCAN_EINVAL, fmt, a...); return nullptr; };
-    if (n_bins < 2 || n_bins > 2147483647LL) return bad("n_bins = %lld out of range [2, 2^31)", (long long)n_bins);
+    if (n_bins < 2 || n_bins > 2147483647LL - 65536) return bad("n_bins = %lld out of range [2, 2^31 - 2^16)", (long long)n_bins);
     if (batch < 1) return bad("batch = %d < 1", batch);
     if (zmax < 1 || zmax > PULSCAN_MAX_ZMAX) return bad("zmax = %d out of range [1, %d]", zmax, PULSCAN_MAX_ZMAX);
     if ((int64_t)zmax >= n_bins) return bad("zmax = %d must be < n_bins = %lld", zmax, (long long)n_bins);
@@ -425,7 +456,7 @@ int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_
     if (log10_p_flag != 0.0 && !(log10_p_flag <= -2.0 && log10_p_flag >= -9.0))
         return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -2]");
     plan->tile_user = tile_bins;
-    plan->log10_p_flag = (log10_p_flag == 0.0) ? -5.0 : log10_p_flag;
+    plan->log10_p_flag = (log10_p_flag == 0.0) ? -3.0 : log10_p_flag;
     plan->dirty = true; release_device(*plan);
     return PULSCAN_OK;
 }
@@ -590,10 +621,11 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
     double evals = 0;
     for (int l = 0; l < p.sp.nlevels; ++l) {
         const SweepLevel& lv = p.sp.lv[l];
-        const double ev = (double)lv.m_hi / (double)(1 << lv.lg);
+        const double ev = 4.0 * lv.nsteps / (double)(1 << lv.lg);
         evals += ev;
-        snprintf(line, sizeof line, "sweep level %d: g=%d widths [%d,%d] covers m=[%d,%d] tasks/tile=%d  (%.3f cover sums per bin)\n", l,
-                 1 << lv.lg, lv.wlo, lv.whi, lv.m_lo, lv.m_hi, lv.ntasks, ev);
+        snprintf(line, sizeof line,
+                 "sweep level %d: g=%d widths [%d,%d] covers m=[%d,%d] steps=%d warp-tasks/tile=%d  (%.3f cover sums per bin)\n", l,
+                 1 << lv.lg, lv.wlo, lv.whi, lv.m_lo, lv.m_hi, lv.nsteps, lv.nwt, ev);
         s += line;
     }
     snprintf(line, sizeof line,
