@@ -195,7 +195,7 @@ class Plan:
         return out[:, : self.n_bins]
 
     def stats(self, stream: Optional[torch.cuda.Stream] = None) -> np.ndarray:
-        h = np.zeros(8, dtype=np.uint32)
+        h = np.zeros(16, dtype=np.uint32)
         _check(self.lib.pulscan_plan_get_stats(self.handle, h.ctypes.data, _stream_ptr(stream)))
         return h
 

@@ -200,14 +200,16 @@ __device__ __forceinline__ void block_median_pair(const float (&v)[EPT], int len
 }
 
 // One component of one block: v ← |v − median(v)| in place; returns 1/(√2·κ·MAD) (0 if κ·MAD is 0 or not finite,
-// R7), the √2 folding the ½ of P = (re'² + im'²)/2 into the scale.
+// R7), the √2 folding the ½ of P = (re'² + im'²)/2 into the scale, and the median as a + h (a = lower central value,
+// h = half the gap to the upper one).
 // The median (a + b)/2 is never rounded to float32: v − (a+b)/2 is formed as (v − a) − (b − a)/2, whose rounding
 // errors are relative to the deviation itself, so a spectrum riding on a large offset loses nothing.
 template <int EPT, int NT>
-__device__ __forceinline__ float normalise_component(float (&v)[EPT], int len, SelectSmem& sm) {
+__device__ __forceinline__ float normalise_component(float (&v)[EPT], int len, SelectSmem& sm, float& a_out, float& h_out) {
     float a, b;
     block_median_pair<EPT, NT>(v, len, sm, a, b);
     const float h = 0.5f * __fsub_rn(b, a);
+    a_out = a; h_out = h;
 #pragma unroll
     for (int r = 0; r < EPT; ++r) v[r] = fabsf(__fsub_rn(__fsub_rn(v[r], a), h));
     block_median_pair<EPT, NT>(v, len, sm, a, b);
@@ -215,7 +217,9 @@ __device__ __forceinline__ float normalise_component(float (&v)[EPT], int len, S
     return (s > 0.0 && isfinite(s)) ? (float)(0.70710678118654752440 / s) : 0.f;
 }
 
-// One normalisation block by the general path: len values at src → powers at dst.
+// One normalisation block by the general path: len values at src → powers at dst.  The normalised component
+// ((v − a) − h)·inv is evaluated as fma(v − a, inv, −h·inv) from the re-read input (the registers hold |v − m| by
+// then); norm_power_v2.cuh uses the same expression, so both paths produce identical bits.
 template <int EPT, int NT>
 __device__ __forceinline__ void norm_block_general(const float2* __restrict__ src, int len, float* __restrict__ dst,
                                                    SelectSmem& sm) {
@@ -229,14 +233,17 @@ __device__ __forceinline__ void norm_block_general(const float2* __restrict__ sr
         re[r] = z.x;
         im[r] = z.y;
     }
-    const float inv_re = normalise_component<EPT, NT>(re, len, sm);
-    const float inv_im = normalise_component<EPT, NT>(im, len, sm);
+    float a_re, h_re, a_im, h_im;
+    const float inv_re = normalise_component<EPT, NT>(re, len, sm, a_re, h_re);
+    const float inv_im = normalise_component<EPT, NT>(im, len, sm, a_im, h_im);
+    const float k_re = -h_re * inv_re, k_im = -h_im * inv_im;
 #pragma unroll
     for (int r = 0; r < EPT; ++r) {
         const int idx = tid + r * NT;
         if (idx < len) {
-            const float x = re[r] * inv_re, y = im[r] * inv_im;
-            dst[idx] = fmaf(x, x, y * y);
+            const float2 z = __ldg(src + idx);
+            const float x = __fmaf_rn(__fsub_rn(z.x, a_re), inv_re, k_re), y = __fmaf_rn(__fsub_rn(z.y, a_im), inv_im, k_im);
+            dst[idx] = __fmaf_rn(x, x, y * y);
         }
     }
 }

@@ -16,7 +16,7 @@
 #include "block_exact.cuh"
 #include "boxcar_sweep.cuh"
 #include "norm_power.cuh"
-#include "norm_power_fast.cuh"
+#include "norm_power_v2.cuh"
 #include "significance.cuh"
 
 using namespace pulscan;
@@ -82,7 +82,7 @@ struct pulscan_plan {
     // normalisation launch shapes
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
     bool has_tail = false;
-    bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_fast_kernel
+    bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_v2_kernel + redo list
     // workspace (device, caller-owned)
     void* ws = nullptr;
     size_t ws_bytes = 0;
@@ -249,7 +249,7 @@ int derive(pulscan_plan& p) {
         p.main_blocks_per_row = p.nb;
     }
 
-    p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.main_blocks_per_row > 0 &&
+    p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 &&
                  std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
 
     // ---- workspace layout
@@ -336,25 +336,34 @@ constexpr int kRedoGrid = 148;
 // Fast kernel for the full blocks + redo kernel (general path) for the blocks it declined.
 int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* spec, float* P, unsigned* redo,
                      unsigned* redo_count) {
-#define PULSCAN_FAST_CASE(E)                                                                                          \
-    case E:                                                                                                           \
-        norm_power_fast_kernel<E, 256><<<grid, 256, 0, st>>>(spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo,  \
-                                                             redo_count);                                             \
+    const char* lim_lo = reinterpret_cast<const char*>(spec);
+    const char* lim_hi = lim_lo + ((size_t)(p.batch - 1) * p.pitch + p.n) * 8;
+#define PULSCAN_V2_CASE(E)                                                                                            \
+    case E: {                                                                                                         \
+        static bool attr_set = false;                                                                                 \
+        if (!attr_set) {                                                                                              \
+            CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<E, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                                          (int)v2_smem_bytes<E, 256>()));                                             \
+            attr_set = true;                                                                                          \
+        }                                                                                                             \
+        norm_power_v2_kernel<E, 256><<<grid, 256, v2_smem_bytes<E, 256>(), st>>>(spec, p.pitch, p.main_blocks_per_row, \
+                                                                                 P, p.pitchP, redo, redo_count,       \
+                                                                                 lim_lo, lim_hi);                     \
         norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P,        \
                                                                   p.pitchP, redo, redo_count);                        \
-        break;
+        break;                                                                                                        \
+    }
     switch (p.ept_main) {
-        PULSCAN_FAST_CASE(1)
-        PULSCAN_FAST_CASE(2)
-        PULSCAN_FAST_CASE(4)
-        PULSCAN_FAST_CASE(8)
-        PULSCAN_FAST_CASE(16)
-        PULSCAN_FAST_CASE(32)
+        PULSCAN_V2_CASE(2)
+        PULSCAN_V2_CASE(4)
+        PULSCAN_V2_CASE(8)
+        PULSCAN_V2_CASE(16)
+        PULSCAN_V2_CASE(32)
         default: return fail(PULSCAN_EINVAL, "internal: unsupported elements-per-thread %d", p.ept_main);
     }
-#undef PULSCAN_FAST_CASE
+#undef PULSCAN_V2_CASE
     CUDA_TRY(cudaGetLastError());
-    return debug_sync("norm_power_fast_kernel + norm_power_redo_kernel");
+    return debug_sync("fast normalisation kernel + norm_power_redo_kernel");
 }
 
 // d_scratch: the redo list and its counter (inside the workspace for pulscan_search; a temporary for the stand-alone
@@ -614,7 +623,7 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
              "pulscan plan: n_bins=%lld batch=%d zmax=%d block_width=%d norm_block=%d sigma_threshold=%g n_trials=%g pitch=%lld mode=%s\n",
              (long long)p.n, p.batch, p.zmax, p.C, p.B, p.sigma_thr, p.n_trials, (long long)p.pitch, p.mode ? "exhaustive" : "pruned");
     s += line;
-    snprintf(line, sizeof line, "norm: %d blocks/row, main %s<EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.use_fast ? "fast" : "general",
+    snprintf(line, sizeof line, "norm: %d blocks/row, main %s<EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.use_fast ? "single-histogram" : "general",
              p.ept_main, p.nt_main, p.main_blocks_per_row, p.has_tail ? "" : " (no tail launch)");
     s += line;
     if (p.has_tail) { snprintf(line, sizeof line, "norm tail: <EPT=%d,NT=%d> x 1/row\n", p.ept_tail, p.nt_tail); s += line; }
@@ -648,7 +657,7 @@ int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_str
     if (rc) return rc;
     if (!h_stats) return fail(PULSCAN_EINVAL, "null pointer");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    CUDA_TRY(cudaMemcpyAsync(h_stats, static_cast<char*>(plan->ws) + plan->off_counters, 8 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(h_stats, static_cast<char*>(plan->ws) + plan->off_counters, 16 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     return PULSCAN_OK;
 }

@@ -33,7 +33,7 @@ def test_normalise_power_matches_oracle(orc, n, B):
     stats = plan.stats()
     plan.destroy()
     assert np.array_equal(P_general, P_fast)           # both paths select exactly, then share the arithmetic
-    assert stats[1] <= 1                               # fast-path blocks sent to the redo list
+    assert stats[1] <= 1                               # fast-path blocks sent to the redo list (h_stats[4..8] say why)
     for b in range(3):
         ref = orc.normalise_power(spec[b].cpu().numpy(), B)
         err = np.abs(P_fast[b] - ref)
