@@ -60,8 +60,9 @@ struct SweepParams {
     int narr;        // decimated arrays: one per distinct group size
     int arr_lg[kMaxLevels];
     int arr_off[kMaxLevels];
-    int z_floats;    // floats of the PP region (4 + len + pad)
-    int smem_floats; // PP region + decimated arrays
+    int npass;       // scan passes per tile = ceil(len / kScanPass)
+    int z_floats;    // floats of ONE tile buffer: 4 + npass·kScanPass + 4 (Z[3] = PP[0], raw powers / PP from Z[4])
+    int smem_floats; // two tile buffers + decimated arrays
     SweepLevel lv[kMaxLevels];
 };
 
@@ -111,36 +112,51 @@ __device__ __forceinline__ void load_tile(float* sP, const float* __restrict__ P
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Prefix scan.  Z is the PP region: Z[3] = PP[0] = 0 and Z[4+i] = Σ_{j≤i} P[j], i.e. PP[i] = Z[3+i] for i ∈ [0, len].
-// `fetch(i4)` returns the four powers P[4·i4 .. 4·i4+3] of the tile (zeros beyond the row's end); for the in-place
-// variant it reads Z+4 itself, which is safe because every read of a pass happens before the pass's barrier and every
-// write after it, and a pass only writes where it (or an earlier pass) has read.
-// The decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg], are written straight from the scan registers
-// (each thread owns 20 consecutive entries, so the multiples of g among them are known), followed by kPadG copies of
-// PP[len]: a cover that reaches past the staged bins gains nothing.
-// Returns PP[len] (the largest entry) in every thread.  Ends with a CTA barrier.
+// Prefix scan, in place.  Z is a tile buffer: on entry Z[4+i] = P[t0+i] for i < len and 0 for len ≤ i < len+kScanPer
+// (beyond that: don't care); on exit Z[3+i] = PP[i] = Σ_{j<i} P[t0+j] for i ∈ [0, len] (Z[3] = 0 is set once per
+// kernel).  In-place is safe because every read of a pass happens before the pass's barrier and every write after it,
+// and a thread writes exactly the entries it has read.
+// Each thread owns kScanPer = 20 consecutive entries (80-byte lane stride: conflict-free 16-byte accesses), so the
+// multiples of g among them follow a fixed pattern and the decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg],
+// are written straight from the scan registers with compile-time register indices.  Entries past len >> lg (written by
+// the thread that straddles len, ≤ 5 of them, inside the kPadG pad) equal PP[len] because of the zeros after len: a
+// cover that reaches past the staged bins gains nothing.  The remaining pad entries are filled by sweep_pads().
+// Ends with a CTA barrier.
 struct ScanSmem {
-    float wtot[kSweepThreads / 32];
+    alignas(16) float wtot[kSweepThreads / 32];
 };
 
-template <class Fetch>
-__device__ __forceinline__ float scan_tile(const SweepParams& sp, float* Z, float* sG, ScanSmem& ss, Fetch fetch) {
+__device__ __forceinline__ float scan_sel5(const float (&x)[kScanPer], int q) {
+    float v = x[19];
+    v = (q == 3) ? x[15] : v;
+    v = (q == 2) ? x[11] : v;
+    v = (q == 1) ? x[7] : v;
+    v = (q == 0) ? x[3] : v;
+    return v;
+}
+
+__device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float* sG, ScanSmem& ss) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int len = sp.len;
     float carry = 0.f;
-    if (tid == 0) Z[3] = 0.f;
     if (tid < sp.narr) sG[sp.arr_off[tid]] = 0.f;
-    for (int base = 0; base < len; base += kScanPass) {
-        const int i0 = base + kScanPer * tid;
+    for (int pass = 0; pass < sp.npass; ++pass) {
+        const int i0 = pass * kScanPass + kScanPer * tid;
+        const bool act = i0 < len;
+        float4* zq = reinterpret_cast<float4*>(Z + 4) + (i0 >> 2);
         float x[kScanPer];
+        if (act) {
 #pragma unroll
-        for (int q = 0; q < kScanPer / 4; ++q) {
-            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (i0 + 4 * q < len) v = fetch((i0 >> 2) + q);
-            x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+            for (int q = 0; q < kScanPer / 4; ++q) {
+                const float4 v = zq[q];
+                x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
+            }
+#pragma unroll
+            for (int j = 1; j < kScanPer; ++j) x[j] += x[j - 1];
+        } else {
+#pragma unroll
+            for (int j = 0; j < kScanPer; ++j) x[j] = 0.f;
         }
-#pragma unroll
-        for (int j = 1; j < kScanPer; ++j) x[j] += x[j - 1];
         float incl = x[kScanPer - 1];
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
@@ -151,52 +167,50 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, float* Z, floa
         if (lane == 0) excl = 0.f;
         if (lane == 31) ss.wtot[warp] = incl;
         __syncthreads();
+        const float4 wa = *reinterpret_cast<const float4*>(ss.wtot), wb = *reinterpret_cast<const float4*>(ss.wtot + 4);
+        const float wt[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
         float wbase = 0.f, total = 0.f;
 #pragma unroll
         for (int w = 0; w < kSweepThreads / 32; ++w) {
-            const float t = ss.wtot[w];
-            if (w < warp) wbase += t;
-            total += t;
+            if (w == warp) wbase = total;
+            total += wt[w];
         }
-        const float off = carry + (wbase + excl);
+        if (act) {
+            const float off = carry + (wbase + excl);
 #pragma unroll
-        for (int j = 0; j < kScanPer; ++j) x[j] += off;     // x[j] = PP[i0 + j + 1]
-        if (i0 < len) {
+            for (int j = 0; j < kScanPer; ++j) x[j] += off;     // x[j] = PP[i0 + j + 1]
 #pragma unroll
-            for (int q = 0; q < kScanPer / 4; ++q)
-                if (i0 + 4 * q < len)
-                    reinterpret_cast<float4*>(Z + 4)[(i0 >> 2) + q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
+            for (int q = 0; q < kScanPer / 4; ++q) zq[q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
+            const int u = (i0 >> 2) + 1;                        // candidates for lg ≥ 2: PP[4(u+q)] = x[4q+3], q = 0..4
             for (int a = 0; a < sp.narr; ++a) {
                 const int lg = sp.arr_lg[a];
                 float* dst = sG + sp.arr_off[a];
-                if (lg >= 2) {              // candidates: PP[i0 + 4q + 4]
-                    const int gm = (1 << lg) - 1;
+                if (lg == 2) {
 #pragma unroll
-                    for (int q = 0; q < kScanPer / 4; ++q) {
-                        const int pos = i0 + 4 * q + 4;
-                        if ((pos & gm) == 0 && pos <= len) dst[pos >> lg] = x[4 * q + 3];
-                    }
+                    for (int q = 0; q < 5; ++q) dst[u + q] = x[4 * q + 3];
+                } else if (lg == 3) {
+                    const bool odd = u & 1;                     // hits q = odd, odd+2 (and 4 when even)
+                    float* d = dst + ((u + 1) >> 1);
+                    d[0] = odd ? x[7] : x[3];
+                    d[1] = odd ? x[15] : x[11];
+                    if (!odd) d[2] = x[19];
+                } else if (lg >= 4) {
+                    const int sh = lg - 2, q0 = (-u) & ((1 << sh) - 1);
+                    if (q0 < 5) dst[(u + q0) >> sh] = scan_sel5(x, q0);
+                    if (lg == 4 && q0 == 0) dst[((u + 4) >> 2)] = x[19];
                 } else if (lg == 1) {
 #pragma unroll
-                    for (int q = 0; q < kScanPer / 2; ++q) {
-                        const int pos = i0 + 2 * q + 2;
-                        if (pos <= len) dst[pos >> 1] = x[2 * q + 1];
-                    }
+                    for (int q = 0; q < kScanPer / 2; ++q) dst[(i0 >> 1) + 1 + q] = x[2 * q + 1];
                 } else {
 #pragma unroll
                     for (int j = 0; j < kScanPer; ++j)
-                        if (i0 + j + 1 <= len) dst[i0 + j + 1] = x[j];
+                        if (i0 + j + 1 <= len + kPadG) dst[i0 + j + 1] = x[j];
                 }
             }
         }
         carry += total;
-        if (base + kScanPass >= len && tid < kPadG * sp.narr) {   // last pass: carry = PP[len]
-            const int a = tid / kPadG;
-            sG[sp.arr_off[a] + (len >> sp.arr_lg[a]) + 1 + (tid % kPadG)] = carry;
-        }
         __syncthreads();
     }
-    return carry;
 }
 
 // One 4-wide step over m for 8 group starts.  O is the rotation of the 12-entry window W (compile time, so that the
@@ -313,29 +327,35 @@ __device__ __forceinline__ void publish_flags(const unsigned char* sflag, int nb
     }
 }
 
+// What one tile needs to know; written by thread 0 when it issues the tile's TMA copy, read by everybody two barriers later.
+struct TileMeta {
+    int row, t0;
+    int c_first, nblk_tile;   // candidate blocks touched by the tile's start bins
+    int first_pad;            // valid bins staged (the rest of the buffer up to len + kScanPer must read as zero)
+    int pad_[3];
+};
+
 struct SweepCtl {
     ScanSmem scan;
     unsigned work[kWorkCap];
-    unsigned task_ctr, work_n;
-    uint64_t mbar;
+    unsigned work_n;
+    alignas(8) uint64_t mbar[2];
+    TileMeta meta[2];
 };
 
 // The sweep proper, on a tile whose PP region and decimated arrays are ready.  Marks sflag[]; the caller publishes.
 // counters[2] += work-list cells, counters[3] += tiles whose work list overflowed (all their blocks get marked).
-__device__ __forceinline__ void sweep_covers(const SweepParams& sp, const float* __restrict__ Z, const float* __restrict__ sG,
+// Ends with a CTA barrier after which nobody reads Z, sG or the work list any more.
+__device__ __forceinline__ void sweep_covers(const SweepParams& sp, const float* __restrict__ sG,
                                              const float* __restrict__ sTau, SweepCtl& ctl, const SweepCtx& cx,
                                              int nblk_tile, unsigned* __restrict__ counters) {
     const int lane = threadIdx.x & 31;
-    // ---- cover sums: warps draw (level, 256 group starts) tasks, most expensive levels first
-    for (;;) {
-        unsigned q = 0;
-        if (lane == 0) q = atomicAdd(&ctl.task_ctr, 1u);
-        q = __shfl_sync(0xffffffffu, q, 0);
-        if (q >= (unsigned)sp.ntasks) break;
+    // ---- cover sums: warp-tasks (level, 256 group starts) dealt round-robin, most expensive levels first
+    for (int q = threadIdx.x >> 5; q < sp.ntasks; q += kSweepThreads / 32) {
         int L = 0;
-        while (L + 1 < sp.nlevels && (int)q >= sp.lv[L + 1].wt_off) ++L;
+        while (L + 1 < sp.nlevels && q >= sp.lv[L + 1].wt_off) ++L;
         const SweepLevel& lv = sp.lv[L];
-        const int k0b = (((int)q - lv.wt_off) * 32 + lane) * kSweepR;
+        const int k0b = ((q - lv.wt_off) * 32 + lane) * kSweepR;
         if (k0b < lv.nk) {
             unsigned mask = sweep_task(sG + lv.pg_off, k0b, lv.m_start, lv.nsteps, sTau + lv.tau_off, cx.slack);
             while (mask) {
@@ -365,38 +385,105 @@ __device__ __forceinline__ void sweep_covers(const SweepParams& sp, const float*
     __syncthreads();
 }
 
-// Pruned sweep.  Grid: tiles_per_row · batch CTAs of kSweepThreads; dynamic shared memory:
-//   [z_floats PP region][decimated arrays][ntau τ][SweepCtl][nblk_tile flag bytes].
-__global__ void __launch_bounds__(kSweepThreads)
+// Thread 0: describe tile `item` (= row·tiles_per_row + tile index) in `m` and start its TMA copy into Zbuf + 4.
+// The copy is clipped to the row's allocation (pitchP), so it never touches the next spectrum (R11); P rows start
+// 16-byte aligned and pitchP, tile and len are multiples of 4, so the copy always satisfies TMA's alignment rules.
+__device__ __forceinline__ void sweep_issue_tile(const SweepParams& sp, long long item, const float* __restrict__ P,
+                                                 long long pitchP, long long n, int tiles_per_row, int C, float* Zbuf,
+                                                 uint64_t* mbar, TileMeta& m) {
+    const int row = (int)(item / tiles_per_row);
+    const int t0 = (int)(item - (long long)row * tiles_per_row) * sp.tile;          // n < 2^31
+    const long long avail = pitchP - t0;
+    const int ncopy = (int)(avail < (long long)sp.len ? avail : (long long)sp.len);
+    const long long nv = n - t0;
+    m.row = row; m.t0 = t0;
+    m.first_pad = (int)(nv < (long long)sp.len ? nv : (long long)sp.len);
+    m.c_first = t0 / C;
+    const int last_start = (int)min((long long)t0 + sp.tile - 1, n - 1);
+    m.nblk_tile = last_start / C - m.c_first + 1;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the buffer's earlier generic accesses precede the copy
+    const uint32_t bytes = (uint32_t)ncopy * 4u;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(Zbuf + 4)),
+                 "l"(P + (long long)row * pitchP + t0), "r"(bytes), "r"(smem_u32(mbar))
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(mbar)), "r"(parity)
+            : "memory");
+    }
+}
+
+// Pruned sweep, persistent: gridDim.x CTAs (a multiple of the SM count) stride over the n_items = tiles_per_row · batch
+// tiles; two tile buffers, so the TMA copy of a CTA's next tile is in flight while it scans and sweeps the current one.
+// Dynamic shared memory: [2 × z_floats tile buffers][decimated arrays][ntau τ][SweepCtl][flag bytes].
+__global__ void __launch_bounds__(kSweepThreads, 4)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
-                    int tiles_per_row, int C, long long nblk, const float* __restrict__ tau_g,
+                    int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
                     const float* __restrict__ Tp_g, unsigned* __restrict__ bitmap, unsigned* __restrict__ flagged,
                     unsigned* __restrict__ counters) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float* Z = reinterpret_cast<float*>(smem_raw);
-    float* sG = Z + sp.z_floats;
-    float* sTau = Z + sp.smem_floats;
+    float* Zb0 = reinterpret_cast<float*>(smem_raw);
+    float* sG = Zb0 + 2 * sp.z_floats;
+    float* sTau = Zb0 + sp.smem_floats;
     SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTau + ((sp.ntau + 3) & ~3));
     unsigned char* sflag = reinterpret_cast<unsigned char*>(&ctl + 1);
-
     const int tid = threadIdx.x;
-    const int row = (int)(blockIdx.x / (unsigned)tiles_per_row);
-    const int t0 = (int)(blockIdx.x - (unsigned)row * (unsigned)tiles_per_row) * sp.tile;   // n < 2^31
-    const int c_first = t0 / C;
-    const int last_start = (int)min((long long)t0 + sp.tile - 1, n - 1);
-    const int nblk_tile = last_start / C - c_first + 1;
+    const long long stride = gridDim.x;
 
+    // ---- once per CTA: τ table, constants of the buffers, the first two copies
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
-    for (int i = tid; i < nblk_tile; i += kSweepThreads) sflag[i] = 0;
-    if (tid == 0) { ctl.task_ctr = 0; ctl.work_n = 0; }
-    load_tile(Z + 4, P + (long long)row * pitchP, t0, n, pitchP, sp.len, &ctl.mbar); // ends with __syncthreads()
+    for (int i = tid; i < sp.smem_floats - 2 * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;   // incl. the arrays' pads
+    if (tid < 2) Zb0[tid * sp.z_floats + 3] = 0.f;                                             // PP[0]
+    if (tid < 2 * kScanPer) Zb0[(tid / kScanPer) * sp.z_floats + 4 + sp.len + tid % kScanPer] = 0.f;   // zeros after len
+    if (tid == 0) {
+        ctl.work_n = 0;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[0])));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[1])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const long long i0 = blockIdx.x;
+        if (i0 < n_items) sweep_issue_tile(sp, i0, P, pitchP, n, tiles_per_row, C, Zb0, &ctl.mbar[0], ctl.meta[0]);
+        if (i0 + stride < n_items)
+            sweep_issue_tile(sp, i0 + stride, P, pitchP, n, tiles_per_row, C, Zb0 + sp.z_floats, &ctl.mbar[1], ctl.meta[1]);
+    }
+    __syncthreads();
 
-    const float4* src = reinterpret_cast<const float4*>(Z + 4);
-    const float pp_max = scan_tile(sp, Z, sG, ctl.scan, [src](int i4) { return src[i4]; });
-
-    SweepCtx cx{Z, Tp_g, sflag, t0, (int)n, sp.tile, C, c_first, kSlackUlps * 5.9604644775390625e-8f * pp_max};
-    sweep_covers(sp, Z, sG, sTau, ctl, cx, nblk_tile, counters);
-    publish_flags(sflag, nblk_tile, c_first, nblk, row, bitmap, flagged, counters);
+    int it = 0;
+    for (long long item = blockIdx.x; item < n_items; item += stride, ++it) {
+        const int b = it & 1;
+        float* Z = Zb0 + b * sp.z_floats;
+        const TileMeta mt = ctl.meta[b];
+        mbar_wait(&ctl.mbar[b], (uint32_t)(it >> 1) & 1u);
+        if (mt.first_pad < sp.len) {                         // last tile of a row: nothing beyond the spectrum's end
+            for (int i = mt.first_pad + tid; i < sp.len; i += kSweepThreads) Z[4 + i] = 0.f;
+            __syncthreads();
+        }
+        scan_tile(sp, Z, sG, ctl.scan);                      // ends with a barrier: publish_flags of the previous tile is done
+        for (int i = tid; i < mt.nblk_tile; i += kSweepThreads) sflag[i] = 0;
+        const float pp_max = Z[3 + sp.len];
+        SweepCtx cx{Z, Tp_g, sflag, mt.t0, (int)n, sp.tile, C, mt.c_first, kSlackUlps * 5.9604644775390625e-8f * pp_max};
+        sweep_covers(sp, sG, sTau, ctl, cx, mt.nblk_tile, counters);   // its first barrier orders the sflag zeroing
+        if (tid == 0) {
+            ctl.work_n = 0;
+            const long long nxt = item + 2 * stride;
+            if (nxt < n_items) sweep_issue_tile(sp, nxt, P, pitchP, n, tiles_per_row, C, Z, &ctl.mbar[b], ctl.meta[b]);
+        } else if (tid >= 32 && tid < 32 + kScanPer) {
+            Z[4 + sp.len + (tid - 32)] = 0.f;                // the scan has written PP garbage over the zeros after len
+        }
+        publish_flags(sflag, mt.nblk_tile, mt.c_first, nblk, mt.row, bitmap, flagged, counters);
+    }
 }
 
 // Exhaustive sweep (cross-check mode): thread per start bin, the paper's recursion S(i,w) = S(i,w−1) + P[i+w−1]

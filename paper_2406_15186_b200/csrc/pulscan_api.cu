@@ -77,6 +77,7 @@ struct pulscan_plan {
     std::vector<float> tau;    // per-level cover thresholds
     SweepParams sp{};
     int tiles_per_row = 0;
+    int sweep_grid = 0;        // persistent CTAs of the pruned sweep: SM count × resident CTAs per SM
     size_t smem_sweep = 0, smem_exh = 0, smem_exact = 0;
     int exh_len = 0;
     // normalisation launch shapes
@@ -179,9 +180,9 @@ int derive(pulscan_plan& p) {
             lgmax = std::max(lgmax, lg);
             w = w2 + 1;
         }
-        if (fits) {   // shared memory of the PP region + one decimated array per distinct (group size, shift)
+        if (fits) {   // shared memory of the two tile buffers + one decimated array per distinct group size
             const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
-            size_t fl = (size_t)len + 8;
+            size_t fl = 2 * ((size_t)((len + kScanPass - 1) / kScanPass) * kScanPass + 8);
             std::vector<int> seen;
             for (const SweepLevel& lv : lvls)
                 if (std::find(seen.begin(), seen.end(), lv.lg) == seen.end()) {
@@ -200,7 +201,8 @@ int derive(pulscan_plan& p) {
     sp.tile = tile;
     const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
     sp.len = tile + halo;
-    sp.z_floats = (int)align_up((size_t)(4 + sp.len + 4), 4);
+    sp.npass = (sp.len + kScanPass - 1) / kScanPass;
+    sp.z_floats = 4 + sp.npass * kScanPass + 4;
     int off = 0, task = 0;
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = lvls[l];
@@ -226,7 +228,7 @@ int derive(pulscan_plan& p) {
     }
     sp.ntasks = task;
     sp.ntau = (int)p.tau.size();
-    sp.smem_floats = sp.z_floats + off;
+    sp.smem_floats = 2 * sp.z_floats + off;
     p.tiles_per_row = (int)((p.n + tile - 1) / tile);
     const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
     p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + sizeof(SweepCtl) + flag_bytes;
@@ -287,6 +289,10 @@ int ensure_device(pulscan_plan& p) {
     CUDA_TRY(cudaMemcpy(p.d_Tp, p.Tp.data(), p.Tp.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(p.d_tau, p.tau.data(), p.tau.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_sweep));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, boxcar_sweep_kernel, kSweepThreads, p.smem_sweep));
+    if (occ < 1) return fail(PULSCAN_ECUDA, "boxcar_sweep_kernel does not fit an SM with %zu bytes of shared memory", p.smem_sweep);
+    p.sweep_grid = (int)std::min<long long>((long long)p.tiles_per_row * p.batch, (long long)p.sm_count * occ);
     CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exh));
     CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exact));
     p.device_ready = true;
@@ -561,9 +567,9 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
     if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
     if (p.mode == 0) {
-        boxcar_sweep_kernel<<<(int)grid_b, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
-                                                                             p.nblk, p.d_tau, p.d_Tp, d_bitmap, d_flagged,
-                                                                             d_counters);
+        boxcar_sweep_kernel<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
+                                                                              p.C, p.nblk, p.d_tau, p.d_Tp, d_bitmap,
+                                                                              d_flagged, d_counters);
     } else {
         boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_P, p.pitchP,
                                                                                 p.n, p.tiles_per_row, p.C, p.nblk, p.d_Tp,
