@@ -224,7 +224,8 @@ def run_ours(args):
     ms_step = ms_total / steps
     value = total_bins / (ms_step * 1e-3)
     n_cand = int(plan.d_count.item())
-    flagged = int(plan.stats()[0])
+    stats = plan.stats()
+    flagged = int(stats[0])
 
     # per-kernel device times of the timed steps (CUDA events recorded by the library on the launching stream)
     prof = np.array([plan.profile(s) for s in range(warm, warm + steps)], dtype=np.float64).mean(axis=0)
@@ -277,7 +278,8 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic", "config": config_dict(wl, world), "bin_widths_per_sec": value * wl.zmax,
-            "candidates_per_step": n_cand, "blocks_flagged_by_sweep": flagged, "clocks": clk.summary(),
+            "candidates_per_step": n_cand, "blocks_flagged_by_sweep": flagged,
+            "sweep_cells_refined": int(stats[2]), "norm_blocks_redone": int(stats[1]), "clocks": clk.summary(),
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
         }
         print(json.dumps(out), flush=True)

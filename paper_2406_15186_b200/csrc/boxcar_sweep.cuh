@@ -34,6 +34,7 @@ constexpr int kSweepR = 8;                 // consecutive group starts per threa
 constexpr int kScanPer = 20;               // floats per thread per scan pass: 80-byte lane stride is bank-conflict-free
 constexpr int kScanPass = kScanPer * kSweepThreads;
 constexpr int kWorkCap = 384;              // flagged (8 group starts × 4 cover lengths) cells per tile before giving up
+constexpr int kMaxWarpTasks = 128;         // warp-tasks per tile (8 levels of at most tile/(256·g) each)
 constexpr int kPadG = 16;                  // replicated entries after each decimated prefix array (window over-read)
 constexpr float kSlackUlps = 96.f;         // ≥ 2·(19 + 5 + 7 + 3 + passes) + 1 roundings, see above
 
@@ -57,6 +58,7 @@ struct SweepParams {
     int len;         // tile + halo, multiple of 64; halo ≥ zmax + 2·g_max
     int ntasks;      // warp-tasks per tile (levels are ordered by decreasing cost)
     int ntau;
+    int zmax;
     int narr;        // decimated arrays: one per distinct group size
     int arr_lg[kMaxLevels];
     int arr_off[kMaxLevels];
@@ -120,8 +122,8 @@ __device__ __forceinline__ void load_tile(float* sP, const float* __restrict__ P
 // multiples of g among them follow a fixed pattern and the decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg],
 // are written straight from the scan registers with compile-time register indices.  Entries past len >> lg (written by
 // the thread that straddles len, ≤ 5 of them, inside the kPadG pad) equal PP[len] because of the zeros after len: a
-// cover that reaches past the staged bins gains nothing.  The remaining pad entries are filled by sweep_pads().
-// Ends with a CTA barrier.
+// cover that reaches past the staged bins gains nothing; the other pad entries only ever meet τ = +inf and are zeroed
+// once per kernel.  Also clears the tile's block flags (between its barriers).  Ends with a CTA barrier.
 struct ScanSmem {
     alignas(16) float wtot[kSweepThreads / 32];
 };
@@ -135,7 +137,8 @@ __device__ __forceinline__ float scan_sel5(const float (&x)[kScanPer], int q) {
     return v;
 }
 
-__device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float* sG, ScanSmem& ss) {
+__device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float* sG, ScanSmem& ss, unsigned char* sflag,
+                                          int nblk_tile) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int len = sp.len;
     float carry = 0.f;
@@ -151,8 +154,13 @@ __device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float
                 const float4 v = zq[q];
                 x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
             }
+            // prefix inside each quad (5 independent chains), then the chain over the quad totals
 #pragma unroll
-            for (int j = 1; j < kScanPer; ++j) x[j] += x[j - 1];
+            for (int q = 0; q < kScanPer / 4; ++q) {
+                x[4 * q + 1] += x[4 * q]; x[4 * q + 2] += x[4 * q + 1]; x[4 * q + 3] += x[4 * q + 2];
+            }
+#pragma unroll
+            for (int q = 1; q < kScanPer / 4; ++q) x[4 * q + 3] += x[4 * q - 1];
         } else {
 #pragma unroll
             for (int j = 0; j < kScanPer; ++j) x[j] = 0.f;
@@ -167,6 +175,10 @@ __device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float
         if (lane == 0) excl = 0.f;
         if (lane == 31) ss.wtot[warp] = incl;
         __syncthreads();
+        // every thread has left the previous tile's publish_flags: clear the block flags for this tile (ordered before
+        // the first refinement by the barrier that ends the pass)
+        if (pass == 0)
+            for (int i = tid; i < nblk_tile; i += kSweepThreads) sflag[i] = 0;
         const float4 wa = *reinterpret_cast<const float4*>(ss.wtot), wb = *reinterpret_cast<const float4*>(ss.wtot + 4);
         const float wt[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
         float wbase = 0.f, total = 0.f;
@@ -178,7 +190,11 @@ __device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float
         if (act) {
             const float off = carry + (wbase + excl);
 #pragma unroll
-            for (int j = 0; j < kScanPer; ++j) x[j] += off;     // x[j] = PP[i0 + j + 1]
+            for (int q = kScanPer / 4 - 1; q >= 0; --q) {       // x[j] = PP[i0 + j + 1]
+                const float oq = q ? off + x[4 * q - 1] : off;  // x[4q−1] is still the thread-local prefix here
+                x[4 * q] += oq; x[4 * q + 1] += oq; x[4 * q + 2] += oq;
+                x[4 * q + 3] += off;
+            }
 #pragma unroll
             for (int q = 0; q < kScanPer / 4; ++q) zq[q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
             const int u = (i0 >> 2) + 1;                        // candidates for lg ≥ 2: PP[4(u+q)] = x[4q+3], q = 0..4
@@ -265,15 +281,26 @@ __device__ __forceinline__ unsigned sweep_task(const float* __restrict__ PG, int
 
 struct SweepCtx {
     const float* Z;         // PP region (PP[i] = Z[3+i])
-    const float* Tp;        // global: T'_w, w = 1..zmax (conservative float thresholds)
+    const float* Tp;        // shared: T'_w, w = 1..zmax (conservative float thresholds)
     unsigned char* sflag;   // shared: one byte per candidate block touched by the tile
     int t0, n;              // n_bins < 2^31 (pulscan_plan_create)
-    int tile, C;
-    int c_first;            // first candidate block of the tile
+    int C;
+    int rem;                // t0 − c_first·C: offset of the tile's first bin inside its candidate block
+    float inv_C;
     float slack;
 };
 
-// One work-list cell (level L, group starts k0b..k0b+7, cover lengths m4..m4+3), one cover per lane: re-test it and sum
+// Candidate block (relative to the tile's first one) that owns start bin t0 + i.  i < 2^24, so the float quotient is
+// off by at most one and the two corrections make it exact.
+__device__ __forceinline__ int rel_block(const SweepCtx& cx, int i) {
+    const int x = cx.rem + i;
+    int q = __float2int_rz(__int2float_rn(x) * cx.inv_C);
+    q -= (q * cx.C > x);
+    q += ((q + 1) * cx.C <= x);
+    return q;
+}
+
+// One flagged cell (level L, group starts k0b..k0b+7, cover lengths m4..m4+3), one cover per lane: re-test it and sum
 // the windows of every cover that passes, all 32 lanes sharing the ≤ g² (start, end) pairs.
 __device__ __forceinline__ void refine_cell(const SweepCtx& cx, const SweepLevel& lv, const float* __restrict__ PG,
                                             const float* __restrict__ tau, int k0b, int step) {
@@ -284,8 +311,8 @@ __device__ __forceinline__ void refine_cell(const SweepCtx& cx, const SweepLevel
     const int g = 1 << lv.lg;
     bool live = U + cx.slack >= tau[4 * step + (lane >> 3)];
     if (live && g <= cx.C) {   // nothing left to find if the (one or two) blocks owning the cover's start bins are marked
-        const int b0 = cx.t0 + (k0 << lv.lg);
-        live = !(cx.sflag[(int)(b0 / cx.C - cx.c_first)] && cx.sflag[(int)((b0 + g - 1) / cx.C - cx.c_first)]);
+        const int b0 = k0 << lv.lg;
+        live = !(cx.sflag[rel_block(cx, b0)] && cx.sflag[rel_block(cx, b0 + g - 1)]);
     }
     unsigned hits = __ballot_sync(0xffffffffu, live);
     while (hits) {
@@ -298,13 +325,13 @@ __device__ __forceinline__ void refine_cell(const SweepCtx& cx, const SweepLevel
             const int w = e - i + 1;
             if (w < 1 || w < lv.wlo || w > lv.whi || cx.t0 + e >= cx.n) continue;
             const float S = cx.Z[3 + e + 1] - cx.Z[3 + i];
-            if (S + cx.slack >= __ldg(cx.Tp + (w - 1))) cx.sflag[(int)((cx.t0 + i) / cx.C - cx.c_first)] = 1;
+            if (S + cx.slack >= cx.Tp[w - 1]) cx.sflag[rel_block(cx, i)] = 1;
         }
         if (g <= cx.C) {       // later covers of this cell: drop those whose blocks have just been marked
             bool dead = false;
             if (hits >> lane & 1u) {
-                const int b0 = cx.t0 + (k0 << lv.lg);
-                dead = cx.sflag[(int)(b0 / cx.C - cx.c_first)] && cx.sflag[(int)((b0 + g - 1) / cx.C - cx.c_first)];
+                const int b0 = k0 << lv.lg;
+                dead = cx.sflag[rel_block(cx, b0)] && cx.sflag[rel_block(cx, b0 + g - 1)];
             }
             __syncwarp();
             hits &= ~__ballot_sync(0xffffffffu, dead);
@@ -335,47 +362,54 @@ struct TileMeta {
     int pad_[3];
 };
 
+// A warp-task: the covers of one level for 32 × 8 consecutive group starts.  The list is the same for every tile, so it
+// is built once per CTA; warp w runs tasks w, w + 8, … of every tile.
+struct alignas(16) WarpTask {
+    int pg_off, tau_off, m_start, nsteps;
+    int level, kbase, nk, pad_;
+};
+
 struct SweepCtl {
     ScanSmem scan;
-    unsigned work[kWorkCap];
-    unsigned work_n;
     alignas(8) uint64_t mbar[2];
     TileMeta meta[2];
+    unsigned work_n;
+    unsigned work[kWorkCap];
+    WarpTask task[kMaxWarpTasks];
 };
 
 // The sweep proper, on a tile whose PP region and decimated arrays are ready.  Marks sflag[]; the caller publishes.
+// Flagged cells go to a shared work list and are refined by all warps after a barrier (a warp refining its own cells
+// on the spot was measured slower: the few warps with hits then hold everybody at the final barrier).
 // counters[2] += work-list cells, counters[3] += tiles whose work list overflowed (all their blocks get marked).
 // Ends with a CTA barrier after which nobody reads Z, sG or the work list any more.
 __device__ __forceinline__ void sweep_covers(const SweepParams& sp, const float* __restrict__ sG,
                                              const float* __restrict__ sTau, SweepCtl& ctl, const SweepCtx& cx,
                                              int nblk_tile, unsigned* __restrict__ counters) {
     const int lane = threadIdx.x & 31;
-    // ---- cover sums: warp-tasks (level, 256 group starts) dealt round-robin, most expensive levels first
     for (int q = threadIdx.x >> 5; q < sp.ntasks; q += kSweepThreads / 32) {
-        int L = 0;
-        while (L + 1 < sp.nlevels && q >= sp.lv[L + 1].wt_off) ++L;
-        const SweepLevel& lv = sp.lv[L];
-        const int k0b = ((q - lv.wt_off) * 32 + lane) * kSweepR;
-        if (k0b < lv.nk) {
-            unsigned mask = sweep_task(sG + lv.pg_off, k0b, lv.m_start, lv.nsteps, sTau + lv.tau_off, cx.slack);
+        const int4 ta = *reinterpret_cast<const int4*>(&ctl.task[q]);            // pg_off, tau_off, m_start, nsteps
+        const int4 tb = *reinterpret_cast<const int4*>(&ctl.task[q].level);      // level, kbase, nk
+        const int k0b = tb.y + lane * kSweepR;
+        if (k0b < tb.z) {
+            unsigned mask = sweep_task(sG + ta.x, k0b, ta.z, ta.w, sTau + ta.y, cx.slack);
             while (mask) {
                 const int s = __ffs(mask) - 1;
                 mask &= mask - 1;
                 const unsigned pos = atomicAdd(&ctl.work_n, 1u);
-                if (pos < (unsigned)kWorkCap) ctl.work[pos] = ((unsigned)L << 28) | ((unsigned)s << 20) | (unsigned)(k0b >> 3);
+                if (pos < (unsigned)kWorkCap) ctl.work[pos] = ((unsigned)q << 24) | ((unsigned)s << 16) | (unsigned)(k0b >> 3);
             }
         }
     }
     __syncthreads();
-    // ---- refinement of the flagged cells, one warp per cell
     const unsigned nwork = ctl.work_n;
     if (nwork > (unsigned)kWorkCap) {
         for (int i = threadIdx.x; i < nblk_tile; i += kSweepThreads) cx.sflag[i] = 1;
     } else {
         for (unsigned e = threadIdx.x >> 5; e < nwork; e += kSweepThreads / 32) {
             const unsigned w = ctl.work[e];
-            const SweepLevel& lv = sp.lv[w >> 28];
-            refine_cell(cx, lv, sG + lv.pg_off, sTau + lv.tau_off, (int)(w & 0xFFFFFu) << 3, (int)((w >> 20) & 0xFFu));
+            const WarpTask& t = ctl.task[w >> 24];
+            refine_cell(cx, sp.lv[t.level], sG + t.pg_off, sTau + t.tau_off, (int)(w & 0xFFFFu) << 3, (int)((w >> 16) & 0xFFu));
         }
     }
     if (threadIdx.x == 0 && nwork) {
@@ -425,7 +459,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
 
 // Pruned sweep, persistent: gridDim.x CTAs (a multiple of the SM count) stride over the n_items = tiles_per_row · batch
 // tiles; two tile buffers, so the TMA copy of a CTA's next tile is in flight while it scans and sweeps the current one.
-// Dynamic shared memory: [2 × z_floats tile buffers][decimated arrays][ntau τ][SweepCtl][flag bytes].
+// Dynamic shared memory: [2 × z_floats tile buffers][decimated arrays][ntau τ][zmax T'][SweepCtl][flag bytes].
 __global__ void __launch_bounds__(kSweepThreads, 4)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
@@ -435,16 +469,25 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
     float* Zb0 = reinterpret_cast<float*>(smem_raw);
     float* sG = Zb0 + 2 * sp.z_floats;
     float* sTau = Zb0 + sp.smem_floats;
-    SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTau + ((sp.ntau + 3) & ~3));
+    float* sTp = sTau + ((sp.ntau + 3) & ~3);
+    SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTp + ((sp.zmax + 3) & ~3));
     unsigned char* sflag = reinterpret_cast<unsigned char*>(&ctl + 1);
     const int tid = threadIdx.x;
     const long long stride = gridDim.x;
+    const float inv_C = 1.0f / (float)C;
 
     // ---- once per CTA: τ table, constants of the buffers, the first two copies
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
+    for (int i = tid; i < sp.zmax; i += kSweepThreads) sTp[i] = Tp_g[i];
     for (int i = tid; i < sp.smem_floats - 2 * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;   // incl. the arrays' pads
     if (tid < 2) Zb0[tid * sp.z_floats + 3] = 0.f;                                             // PP[0]
     if (tid < 2 * kScanPer) Zb0[(tid / kScanPer) * sp.z_floats + 4 + sp.len + tid % kScanPer] = 0.f;   // zeros after len
+    for (int q = tid; q < sp.ntasks; q += kSweepThreads) {
+        int L = 0;
+        while (L + 1 < sp.nlevels && q >= sp.lv[L + 1].wt_off) ++L;
+        const SweepLevel& lv = sp.lv[L];
+        ctl.task[q] = WarpTask{lv.pg_off, lv.tau_off, lv.m_start, lv.nsteps, L, (q - lv.wt_off) * 32 * kSweepR, lv.nk, 0};
+    }
     if (tid == 0) {
         ctl.work_n = 0;
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[0])));
@@ -470,11 +513,10 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             for (int i = mt.first_pad + tid; i < sp.len; i += kSweepThreads) Z[4 + i] = 0.f;
             __syncthreads();
         }
-        scan_tile(sp, Z, sG, ctl.scan);                      // ends with a barrier: publish_flags of the previous tile is done
-        for (int i = tid; i < mt.nblk_tile; i += kSweepThreads) sflag[i] = 0;
+        scan_tile(sp, Z, sG, ctl.scan, sflag, mt.nblk_tile);
         const float pp_max = Z[3 + sp.len];
-        SweepCtx cx{Z, Tp_g, sflag, mt.t0, (int)n, sp.tile, C, mt.c_first, kSlackUlps * 5.9604644775390625e-8f * pp_max};
-        sweep_covers(sp, sG, sTau, ctl, cx, mt.nblk_tile, counters);   // its first barrier orders the sflag zeroing
+        SweepCtx cx{Z, sTp, sflag, mt.t0, (int)n, C, mt.t0 - mt.c_first * C, inv_C, kSlackUlps * 5.9604644775390625e-8f * pp_max};
+        sweep_covers(sp, sG, sTau, ctl, cx, mt.nblk_tile, counters);
         if (tid == 0) {
             ctl.work_n = 0;
             const long long nxt = item + 2 * stride;

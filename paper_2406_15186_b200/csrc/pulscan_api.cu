@@ -182,14 +182,14 @@ int derive(pulscan_plan& p) {
         }
         if (fits) {   // shared memory of the two tile buffers + one decimated array per distinct group size
             const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
-            size_t fl = 2 * ((size_t)((len + kScanPass - 1) / kScanPass) * kScanPass + 8);
+            size_t fl = 2 * ((size_t)len + kScanPer + 8);
             std::vector<int> seen;
             for (const SweepLevel& lv : lvls)
                 if (std::find(seen.begin(), seen.end(), lv.lg) == seen.end()) {
                     seen.push_back(lv.lg);
                     fl += (size_t)(len >> lv.lg) + 1 + kPadG + 3;
                 }
-            if (fl * 4 + 16384 <= 227 * 1024) break;
+            if (fl * 4 + (size_t)p.zmax * 4 + sizeof(SweepCtl) + 8192 <= 227 * 1024) break;
         }
         if (l10 >= 0.0) return fail(PULSCAN_EINVAL, "zmax = %d with tile = %d does not fit the sweep's shared memory", p.zmax, tile);
     }
@@ -202,7 +202,7 @@ int derive(pulscan_plan& p) {
     const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
     sp.len = tile + halo;
     sp.npass = (sp.len + kScanPass - 1) / kScanPass;
-    sp.z_floats = 4 + sp.npass * kScanPass + 4;
+    sp.z_floats = (int)align_up((size_t)(4 + sp.len + kScanPer), 4);
     int off = 0, task = 0;
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = lvls[l];
@@ -227,11 +227,13 @@ int derive(pulscan_plan& p) {
         sp.lv[l] = lv;
     }
     sp.ntasks = task;
+    if (task > kMaxWarpTasks) return fail(PULSCAN_EINVAL, "sweep tile of %d bins needs %d warp-tasks (limit %d)", tile, task, kMaxWarpTasks);
     sp.ntau = (int)p.tau.size();
     sp.smem_floats = 2 * sp.z_floats + off;
     p.tiles_per_row = (int)((p.n + tile - 1) / tile);
     const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
-    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + sizeof(SweepCtl) + flag_bytes;
+    sp.zmax = p.zmax;
+    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + align_up((size_t)p.zmax, 4) * 4 + sizeof(SweepCtl) + flag_bytes;
     if (p.smem_sweep > 227 * 1024) return fail(PULSCAN_EINVAL, "sweep tile needs %zu bytes of shared memory", p.smem_sweep);
     p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
