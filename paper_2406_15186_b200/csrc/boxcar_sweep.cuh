@@ -3,23 +3,30 @@
 // What must be found (§2.2.5; Alg. 4): for every start bin i and every width
 // w ≤ zmax the sum S(i,w) = Σ_{j<w} P[i+j], and per candidate block the maxima.  A window can only become a candidate
 // if S(i,w) ≥ T_w, the power at which width w reaches the σ threshold (L342-344: "compared with precomputed
-// threshold values").  In noise that happens for ~1e-9 of all (i,w), so this kernel is a FILTER: it marks the
+// threshold values").  In noise that happens for ~1e-9 of all (i,w), so this stage is a FILTER: it marks the
 // candidate blocks that contain at least one window with S ≥ T_w·(1−ε) and kernel (c) then evaluates exactly those
 // blocks in double precision.  Nothing a marked block could emit is lost and an unmarked block cannot emit.
 //
 // The paper's kernel (Alg. 4) does one shared-memory add per (bin, width) — issue-bound, ~2·zmax instructions per
-// bin.  Here the tile (+ zmax halo) is staged in shared memory by one TMA bulk copy, turned into its prefix sum
-// PP[i] = Σ_{j<i} P[j] once, and swept with COVER SUMS: P ≥ 0, so a window of width w is bounded above by the sum of
-// the aligned g-bin groups that cover it, U(k0,m) = PP[(k0+m)·g] − PP[k0·g].  For a level (g, [wlo, whi]) a thread
-// holds PP at 8 consecutive group starts in registers and slides over m: one FADD + half an FMNMX3 per cover sum,
-// (n/g)·(whi/g+2) cover sums instead of n·(whi−wlo+1) window sums.  g grows like √w (chosen on the host so that a
-// cover of pure noise passes with probability ≤ p_flag), which makes every level cost O(n).  Covers that pass go to a
-// shared-memory work list and are refined afterwards by whole warps: their ≤ g² windows are summed from PP and
-// compared with their own T'_w.
+// bin.  Here the work is split in two kernels:
 //
-// Float safety.  PP is a float32 scan; every PP[i] carries at most ~36 roundings of magnitude
-// ≤ 2⁻²⁴·PP[len], so a difference of two entries is off by < slack = kSlackUlps·2⁻²⁴·PP[len] from the exact sum of
-// the float32 powers.  Every comparison adds the slack on the side that keeps the cover / window.
+//  boxcar_sweep_kernel (streaming, every bin): persistent CTAs stride over tiles; a tile (+ zmax halo) lands in one of
+//    two shared-memory buffers by a TMA bulk copy issued a whole tile ahead.  Each thread sums its 5 quads of powers and
+//    a CTA scan turns the quad sums into PG4[k] = PP[4k] (PP[i] = Σ_{j<i} P[j]) and its decimations PG8, PG16, …
+//    COVER SUMS: P ≥ 0, so a window of width w is bounded above by the sum of the aligned g-bin groups that cover it,
+//    U(k0,m) = PG_g[k0+m] − PG_g[k0].  For a level (g, [wlo, whi]) a thread holds PG at 8 consecutive group starts in
+//    registers and slides over m: one FADD + half an FMNMX3 per cover sum, (n/g)·(whi/g+2) cover sums instead of
+//    n·(whi−wlo+1) window sums.  g ∈ {4, 8, 16, …} grows like √w (chosen on the host so that a cover of pure noise
+//    passes with probability ≤ p_flag), which makes every level cost O(n).  A cell (8 group starts × 4 cover lengths)
+//    with a passing cover is appended to a global list — ≈ 0.6 cells per 4096-bin tile in noise.
+//  sweep_refine_kernel (rare path, one warp per listed cell): re-reads the cell's span of P, builds its prefix sum in
+//    double, re-tests the 32 covers and sums the ≤ g² windows of each passing cover against their own T'_w; blocks
+//    with a window that reaches T'_w are marked (bitmap + list).
+//
+// Float safety of the streaming kernel.  Every PG entry carries at most ~25 roundings of magnitude ≤ 2⁻²⁴·PP[len], so
+// a difference of two entries is off by < slack = kSlackUlps·2⁻²⁴·PP[len] from the exact sum of the float32 powers;
+// the cover test adds the slack on the keeping side.  The refine kernel works in double and compares with T'_w, which
+// the host rounds down by 2w·2⁻²⁴ + 2·10⁻⁶ relative.
 //
 // Exhaustive mode (the cross-check) evaluates every (i, w) by the paper's recursion instead.
 #pragma once
@@ -33,10 +40,10 @@ constexpr int kSweepThreads = 256;
 constexpr int kSweepR = 8;                 // consecutive group starts per thread
 constexpr int kScanPer = 20;               // floats per thread per scan pass: 80-byte lane stride is bank-conflict-free
 constexpr int kScanPass = kScanPer * kSweepThreads;
-constexpr int kWorkCap = 384;              // flagged (8 group starts × 4 cover lengths) cells per tile before giving up
+constexpr int kRefineThreads = 128;        // sweep_refine_kernel: 4 warps, one listed cell per warp at a time
 constexpr int kMaxWarpTasks = 128;         // warp-tasks per tile (8 levels of at most tile/(256·g) each)
 constexpr int kPadG = 16;                  // replicated entries after each decimated prefix array (window over-read)
-constexpr float kSlackUlps = 96.f;         // ≥ 2·(19 + 5 + 7 + 3 + passes) + 1 roundings, see above
+constexpr float kSlackUlps = 96.f;         // ≥ 2·(2 + 4 + 5 + 7 + passes + 1) + 1 roundings, see above
 
 struct SweepLevel {
     int lg;        // log2 of the group size g
@@ -63,8 +70,9 @@ struct SweepParams {
     int arr_lg[kMaxLevels];
     int arr_off[kMaxLevels];
     int npass;       // scan passes per tile = ceil(len / kScanPass)
-    int z_floats;    // floats of ONE tile buffer: 4 + npass·kScanPass + 4 (Z[3] = PP[0], raw powers / PP from Z[4])
-    int smem_floats; // two tile buffers + decimated arrays
+    int z_floats;    // floats of ONE landing buffer: len + kScanPer zeros, rounded up to 4
+    int smem_floats; // two landing buffers + decimated arrays
+    int ref_span;    // longest span of bins a listed cell covers (sweep_refine_kernel's shared memory per warp)
     SweepLevel lv[kMaxLevels];
 };
 
@@ -114,58 +122,52 @@ __device__ __forceinline__ void load_tile(float* sP, const float* __restrict__ P
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Prefix scan, in place.  Z is a tile buffer: on entry Z[4+i] = P[t0+i] for i < len and 0 for len ≤ i < len+kScanPer
-// (beyond that: don't care); on exit Z[3+i] = PP[i] = Σ_{j<i} P[t0+j] for i ∈ [0, len] (Z[3] = 0 is set once per
-// kernel).  In-place is safe because every read of a pass happens before the pass's barrier and every write after it,
-// and a thread writes exactly the entries it has read.
-// Each thread owns kScanPer = 20 consecutive entries (80-byte lane stride: conflict-free 16-byte accesses), so the
-// multiples of g among them follow a fixed pattern and the decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg],
-// are written straight from the scan registers with compile-time register indices.  Entries past len >> lg (written by
-// the thread that straddles len, ≤ 5 of them, inside the kPadG pad) equal PP[len] because of the zeros after len: a
-// cover that reaches past the staged bins gains nothing; the other pad entries only ever meet τ = +inf and are zeroed
-// once per kernel.  Also clears the tile's block flags (between its barriers).  Ends with a CTA barrier.
+// Quad-sum scan.  raw[i] = P[t0+i] for i < len and 0 for len ≤ i < len + kScanPer.  Each thread owns kScanPer = 20
+// consecutive powers (80-byte lane stride: conflict-free 16-byte loads) = 5 quads, so PP at the multiples of 4 it owns,
+// PP[4(u+q)] with u = i0/4 + 1, q = 0..4, are its running quad sums plus the scanned offset, and the multiples of g
+// among them follow a fixed pattern: the decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg], lg ≥ 2, are
+// written straight from registers.  Entries past len >> lg (written by the thread that straddles len, inside the kPadG
+// pad) equal PP[len] because of the zeros after len; the other pad entries only ever meet τ = +inf and are zeroed once
+// per kernel.  After the first barrier of the last pass nobody reads `raw` any more (`after_loads` runs there: the next
+// TMA copy into this buffer).  Returns PP[len] in every thread.  Ends with a CTA barrier; the barrier inside a pass
+// also orders the previous tile's cover sums before this tile's writes to the arrays.
 struct ScanSmem {
     alignas(16) float wtot[kSweepThreads / 32];
 };
 
-__device__ __forceinline__ float scan_sel5(const float (&x)[kScanPer], int q) {
-    float v = x[19];
-    v = (q == 3) ? x[15] : v;
-    v = (q == 2) ? x[11] : v;
-    v = (q == 1) ? x[7] : v;
-    v = (q == 0) ? x[3] : v;
+__device__ __forceinline__ float scan_sel5(const float (&s)[5], int q) {
+    float v = s[4];
+    v = (q == 3) ? s[3] : v;
+    v = (q == 2) ? s[2] : v;
+    v = (q == 1) ? s[1] : v;
+    v = (q == 0) ? s[0] : v;
     return v;
 }
 
-__device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float* sG, ScanSmem& ss, unsigned char* sflag,
-                                          int nblk_tile) {
+template <class AfterLoads>
+__device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* raw, float* sG, ScanSmem& ss,
+                                           AfterLoads after_loads) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int len = sp.len;
     float carry = 0.f;
-    if (tid < sp.narr) sG[sp.arr_off[tid]] = 0.f;
     for (int pass = 0; pass < sp.npass; ++pass) {
         const int i0 = pass * kScanPass + kScanPer * tid;
         const bool act = i0 < len;
-        float4* zq = reinterpret_cast<float4*>(Z + 4) + (i0 >> 2);
-        float x[kScanPer];
+        float s[5];
         if (act) {
+            const float4* zq = reinterpret_cast<const float4*>(raw) + (i0 >> 2);
 #pragma unroll
-            for (int q = 0; q < kScanPer / 4; ++q) {
+            for (int q = 0; q < 5; ++q) {
                 const float4 v = zq[q];
-                x[4 * q] = v.x; x[4 * q + 1] = v.y; x[4 * q + 2] = v.z; x[4 * q + 3] = v.w;
-            }
-            // prefix inside each quad (5 independent chains), then the chain over the quad totals
-#pragma unroll
-            for (int q = 0; q < kScanPer / 4; ++q) {
-                x[4 * q + 1] += x[4 * q]; x[4 * q + 2] += x[4 * q + 1]; x[4 * q + 3] += x[4 * q + 2];
+                s[q] = (v.x + v.y) + (v.z + v.w);
             }
 #pragma unroll
-            for (int q = 1; q < kScanPer / 4; ++q) x[4 * q + 3] += x[4 * q - 1];
+            for (int q = 1; q < 5; ++q) s[q] += s[q - 1];
         } else {
 #pragma unroll
-            for (int j = 0; j < kScanPer; ++j) x[j] = 0.f;
+            for (int q = 0; q < 5; ++q) s[q] = 0.f;
         }
-        float incl = x[kScanPer - 1];
+        float incl = s[4];
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
             const float t = __shfl_up_sync(0xffffffffu, incl, off);
@@ -175,58 +177,46 @@ __device__ __forceinline__ void scan_tile(const SweepParams& sp, float* Z, float
         if (lane == 0) excl = 0.f;
         if (lane == 31) ss.wtot[warp] = incl;
         __syncthreads();
-        // every thread has left the previous tile's publish_flags: clear the block flags for this tile (ordered before
-        // the first refinement by the barrier that ends the pass)
-        if (pass == 0)
-            for (int i = tid; i < nblk_tile; i += kSweepThreads) sflag[i] = 0;
-        const float4 wa = *reinterpret_cast<const float4*>(ss.wtot), wb = *reinterpret_cast<const float4*>(ss.wtot + 4);
-        const float wt[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-        float wbase = 0.f, total = 0.f;
+        if (pass == sp.npass - 1) after_loads();
+        // exclusive prefix of the 8 warp totals: lane w < 8 holds total w, three shuffle steps, broadcast
+        float wt = (lane < kSweepThreads / 32) ? ss.wtot[lane] : 0.f;
+        const float mine = (lane < warp) ? wt : 0.f;
+        float wbase = mine, total = wt;
 #pragma unroll
-        for (int w = 0; w < kSweepThreads / 32; ++w) {
-            if (w == warp) wbase = total;
-            total += wt[w];
+        for (int off = 4; off > 0; off >>= 1) {
+            wbase += __shfl_xor_sync(0xffffffffu, wbase, off);
+            total += __shfl_xor_sync(0xffffffffu, total, off);
         }
+        wbase = __shfl_sync(0xffffffffu, wbase, 0);
+        total = __shfl_sync(0xffffffffu, total, 0);
         if (act) {
             const float off = carry + (wbase + excl);
 #pragma unroll
-            for (int q = kScanPer / 4 - 1; q >= 0; --q) {       // x[j] = PP[i0 + j + 1]
-                const float oq = q ? off + x[4 * q - 1] : off;  // x[4q−1] is still the thread-local prefix here
-                x[4 * q] += oq; x[4 * q + 1] += oq; x[4 * q + 2] += oq;
-                x[4 * q + 3] += off;
-            }
-#pragma unroll
-            for (int q = 0; q < kScanPer / 4; ++q) zq[q] = make_float4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3]);
-            const int u = (i0 >> 2) + 1;                        // candidates for lg ≥ 2: PP[4(u+q)] = x[4q+3], q = 0..4
+            for (int q = 0; q < 5; ++q) s[q] += off;            // s[q] = PP[4(u+q)]
+            const int u = (i0 >> 2) + 1;
             for (int a = 0; a < sp.narr; ++a) {
                 const int lg = sp.arr_lg[a];
                 float* dst = sG + sp.arr_off[a];
                 if (lg == 2) {
 #pragma unroll
-                    for (int q = 0; q < 5; ++q) dst[u + q] = x[4 * q + 3];
+                    for (int q = 0; q < 5; ++q) dst[u + q] = s[q];
                 } else if (lg == 3) {
                     const bool odd = u & 1;                     // hits q = odd, odd+2 (and 4 when even)
                     float* d = dst + ((u + 1) >> 1);
-                    d[0] = odd ? x[7] : x[3];
-                    d[1] = odd ? x[15] : x[11];
-                    if (!odd) d[2] = x[19];
-                } else if (lg >= 4) {
-                    const int sh = lg - 2, q0 = (-u) & ((1 << sh) - 1);
-                    if (q0 < 5) dst[(u + q0) >> sh] = scan_sel5(x, q0);
-                    if (lg == 4 && q0 == 0) dst[((u + 4) >> 2)] = x[19];
-                } else if (lg == 1) {
-#pragma unroll
-                    for (int q = 0; q < kScanPer / 2; ++q) dst[(i0 >> 1) + 1 + q] = x[2 * q + 1];
+                    d[0] = odd ? s[1] : s[0];
+                    d[1] = odd ? s[3] : s[2];
+                    if (!odd) d[2] = s[4];
                 } else {
-#pragma unroll
-                    for (int j = 0; j < kScanPer; ++j)
-                        if (i0 + j + 1 <= len + kPadG) dst[i0 + j + 1] = x[j];
+                    const int sh = lg - 2, q0 = (-u) & ((1 << sh) - 1);
+                    if (q0 < 5) dst[(u + q0) >> sh] = scan_sel5(s, q0);
+                    if (lg == 4 && q0 == 0) dst[(u + 4) >> 2] = s[4];
                 }
             }
         }
         carry += total;
         __syncthreads();
     }
+    return carry;
 }
 
 // One 4-wide step over m for 8 group starts.  O is the rotation of the 12-entry window W (compile time, so that the
@@ -279,66 +269,6 @@ __device__ __forceinline__ unsigned sweep_task(const float* __restrict__ PG, int
     return mask;
 }
 
-struct SweepCtx {
-    const float* Z;         // PP region (PP[i] = Z[3+i])
-    const float* Tp;        // shared: T'_w, w = 1..zmax (conservative float thresholds)
-    unsigned char* sflag;   // shared: one byte per candidate block touched by the tile
-    int t0, n;              // n_bins < 2^31 (pulscan_plan_create)
-    int C;
-    int rem;                // t0 − c_first·C: offset of the tile's first bin inside its candidate block
-    float inv_C;
-    float slack;
-};
-
-// Candidate block (relative to the tile's first one) that owns start bin t0 + i.  i < 2^24, so the float quotient is
-// off by at most one and the two corrections make it exact.
-__device__ __forceinline__ int rel_block(const SweepCtx& cx, int i) {
-    const int x = cx.rem + i;
-    int q = __float2int_rz(__int2float_rn(x) * cx.inv_C);
-    q -= (q * cx.C > x);
-    q += ((q + 1) * cx.C <= x);
-    return q;
-}
-
-// One flagged cell (level L, group starts k0b..k0b+7, cover lengths m4..m4+3), one cover per lane: re-test it and sum
-// the windows of every cover that passes, all 32 lanes sharing the ≤ g² (start, end) pairs.
-__device__ __forceinline__ void refine_cell(const SweepCtx& cx, const SweepLevel& lv, const float* __restrict__ PG,
-                                            const float* __restrict__ tau, int k0b, int step) {
-    const int lane = threadIdx.x & 31;
-    const int k0 = k0b + (lane & 7);
-    const int m = lv.m_start + 4 * step + (lane >> 3);
-    const float U = PG[k0 + m] - PG[k0];
-    const int g = 1 << lv.lg;
-    bool live = U + cx.slack >= tau[4 * step + (lane >> 3)];
-    if (live && g <= cx.C) {   // nothing left to find if the (one or two) blocks owning the cover's start bins are marked
-        const int b0 = k0 << lv.lg;
-        live = !(cx.sflag[rel_block(cx, b0)] && cx.sflag[rel_block(cx, b0 + g - 1)]);
-    }
-    unsigned hits = __ballot_sync(0xffffffffu, live);
-    while (hits) {
-        const int src = __ffs(hits) - 1;
-        hits &= hits - 1;
-        const int kk = k0b + (src & 7), mm = lv.m_start + 4 * step + (src >> 3);
-        const int i0 = kk << lv.lg, e0 = (kk + mm - 1) << lv.lg;
-        for (int idx = lane; idx < g * g; idx += 32) {
-            const int i = i0 + (idx >> lv.lg), e = e0 + (idx & (g - 1));
-            const int w = e - i + 1;
-            if (w < 1 || w < lv.wlo || w > lv.whi || cx.t0 + e >= cx.n) continue;
-            const float S = cx.Z[3 + e + 1] - cx.Z[3 + i];
-            if (S + cx.slack >= cx.Tp[w - 1]) cx.sflag[rel_block(cx, i)] = 1;
-        }
-        if (g <= cx.C) {       // later covers of this cell: drop those whose blocks have just been marked
-            bool dead = false;
-            if (hits >> lane & 1u) {
-                const int b0 = k0 << lv.lg;
-                dead = cx.sflag[rel_block(cx, b0)] && cx.sflag[rel_block(cx, b0 + g - 1)];
-            }
-            __syncwarp();
-            hits &= ~__ballot_sync(0xffffffffu, dead);
-        }
-    }
-}
-
 // Append the tile's marked candidate blocks to the global list, once each (bitmap test-and-set).
 __device__ __forceinline__ void publish_flags(const unsigned char* sflag, int nblk_tile, long long c_first, long long nblk,
                                               long long row, unsigned* __restrict__ bitmap,
@@ -354,14 +284,6 @@ __device__ __forceinline__ void publish_flags(const unsigned char* sflag, int nb
     }
 }
 
-// What one tile needs to know; written by thread 0 when it issues the tile's TMA copy, read by everybody two barriers later.
-struct TileMeta {
-    int row, t0;
-    int c_first, nblk_tile;   // candidate blocks touched by the tile's start bins
-    int first_pad;            // valid bins staged (the rest of the buffer up to len + kScanPer must read as zero)
-    int pad_[3];
-};
-
 // A warp-task: the covers of one level for 32 × 8 consecutive group starts.  The list is the same for every tile, so it
 // is built once per CTA; warp w runs tasks w, w + 8, … of every tile.
 struct alignas(16) WarpTask {
@@ -369,78 +291,41 @@ struct alignas(16) WarpTask {
     int level, kbase, nk, pad_;
 };
 
+// A flagged cell: tile `item` (= row·tiles_per_row + tile index), level, 4-wide step over m, first of 8 group starts.
+struct SweepCell {
+    unsigned item;
+    unsigned code;   // level << 28 | step << 20 | (k0b >> 3)
+};
+
 struct SweepCtl {
     ScanSmem scan;
     alignas(8) uint64_t mbar[2];
-    TileMeta meta[2];
-    unsigned work_n;
-    unsigned work[kWorkCap];
     WarpTask task[kMaxWarpTasks];
 };
 
-// The sweep proper, on a tile whose PP region and decimated arrays are ready.  Marks sflag[]; the caller publishes.
-// Flagged cells go to a shared work list and are refined by all warps after a barrier (a warp refining its own cells
-// on the spot was measured slower: the few warps with hits then hold everybody at the final barrier).
-// counters[2] += work-list cells, counters[3] += tiles whose work list overflowed (all their blocks get marked).
-// Ends with a CTA barrier after which nobody reads Z, sG or the work list any more.
-__device__ __forceinline__ void sweep_covers(const SweepParams& sp, const float* __restrict__ sG,
-                                             const float* __restrict__ sTau, SweepCtl& ctl, const SweepCtx& cx,
-                                             int nblk_tile, unsigned* __restrict__ counters) {
-    const int lane = threadIdx.x & 31;
-    for (int q = threadIdx.x >> 5; q < sp.ntasks; q += kSweepThreads / 32) {
-        const int4 ta = *reinterpret_cast<const int4*>(&ctl.task[q]);            // pg_off, tau_off, m_start, nsteps
-        const int4 tb = *reinterpret_cast<const int4*>(&ctl.task[q].level);      // level, kbase, nk
-        const int k0b = tb.y + lane * kSweepR;
-        if (k0b < tb.z) {
-            unsigned mask = sweep_task(sG + ta.x, k0b, ta.z, ta.w, sTau + ta.y, cx.slack);
-            while (mask) {
-                const int s = __ffs(mask) - 1;
-                mask &= mask - 1;
-                const unsigned pos = atomicAdd(&ctl.work_n, 1u);
-                if (pos < (unsigned)kWorkCap) ctl.work[pos] = ((unsigned)q << 24) | ((unsigned)s << 16) | (unsigned)(k0b >> 3);
-            }
-        }
-    }
-    __syncthreads();
-    const unsigned nwork = ctl.work_n;
-    if (nwork > (unsigned)kWorkCap) {
-        for (int i = threadIdx.x; i < nblk_tile; i += kSweepThreads) cx.sflag[i] = 1;
-    } else {
-        for (unsigned e = threadIdx.x >> 5; e < nwork; e += kSweepThreads / 32) {
-            const unsigned w = ctl.work[e];
-            const WarpTask& t = ctl.task[w >> 24];
-            refine_cell(cx, sp.lv[t.level], sG + t.pg_off, sTau + t.tau_off, (int)(w & 0xFFFFu) << 3, (int)((w >> 16) & 0xFFu));
-        }
-    }
-    if (threadIdx.x == 0 && nwork) {
-        atomicAdd(counters + 2, nwork);
-        if (nwork > (unsigned)kWorkCap) atomicAdd(counters + 3, 1u);
-    }
-    __syncthreads();
+// Mark candidate block gid = row·nblk + c once (bitmap test-and-set) and append it to the list kernel (c) works from.
+__device__ __forceinline__ void mark_block(unsigned long long gid, unsigned* __restrict__ bitmap,
+                                           unsigned* __restrict__ flagged, unsigned* __restrict__ counters) {
+    const unsigned bit = 1u << (gid & 31);
+    if (bitmap[gid >> 5] & bit) return;
+    const unsigned old = atomicOr(bitmap + (gid >> 5), bit);
+    if (!(old & bit)) flagged[atomicAdd(counters, 1u)] = (unsigned)gid;
 }
 
-// Thread 0: describe tile `item` (= row·tiles_per_row + tile index) in `m` and start its TMA copy into Zbuf + 4.
-// The copy is clipped to the row's allocation (pitchP), so it never touches the next spectrum (R11); P rows start
-// 16-byte aligned and pitchP, tile and len are multiples of 4, so the copy always satisfies TMA's alignment rules.
+// Thread 0: start the TMA copy of tile `item` into `dst`.  The copy is clipped to the row's allocation (pitchP), so it
+// never touches the next spectrum (R11); P rows start 16-byte aligned and pitchP, tile and len are multiples of 4, so the
+// copy always satisfies TMA's alignment rules.
 __device__ __forceinline__ void sweep_issue_tile(const SweepParams& sp, long long item, const float* __restrict__ P,
-                                                 long long pitchP, long long n, int tiles_per_row, int C, float* Zbuf,
-                                                 uint64_t* mbar, TileMeta& m) {
-    const int row = (int)(item / tiles_per_row);
-    const int t0 = (int)(item - (long long)row * tiles_per_row) * sp.tile;          // n < 2^31
+                                                 long long pitchP, int tiles_per_row, float* dst, uint64_t* mbar) {
+    const long long row = item / tiles_per_row;
+    const long long t0 = (item - row * tiles_per_row) * sp.tile;
     const long long avail = pitchP - t0;
-    const int ncopy = (int)(avail < (long long)sp.len ? avail : (long long)sp.len);
-    const long long nv = n - t0;
-    m.row = row; m.t0 = t0;
-    m.first_pad = (int)(nv < (long long)sp.len ? nv : (long long)sp.len);
-    m.c_first = t0 / C;
-    const int last_start = (int)min((long long)t0 + sp.tile - 1, n - 1);
-    m.nblk_tile = last_start / C - m.c_first + 1;
+    const uint32_t bytes = (uint32_t)(avail < (long long)sp.len ? avail : (long long)sp.len) * 4u;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the buffer's earlier generic accesses precede the copy
-    const uint32_t bytes = (uint32_t)ncopy * 4u;
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(bytes) : "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(Zbuf + 4)),
-                 "l"(P + (long long)row * pitchP + t0), "r"(bytes), "r"(smem_u32(mbar))
+                     smem_u32(dst)),
+                 "l"(P + row * pitchP + t0), "r"(bytes), "r"(smem_u32(mbar))
                  : "memory");
 }
 
@@ -457,31 +342,29 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
     }
 }
 
-// Pruned sweep, persistent: gridDim.x CTAs (a multiple of the SM count) stride over the n_items = tiles_per_row · batch
-// tiles; two tile buffers, so the TMA copy of a CTA's next tile is in flight while it scans and sweeps the current one.
-// Dynamic shared memory: [2 × z_floats tile buffers][decimated arrays][ntau τ][zmax T'][SweepCtl][flag bytes].
+// Streaming filter, persistent: gridDim.x CTAs (a multiple of the SM count) stride over the n_items = tiles_per_row ·
+// batch tiles.  Two landing buffers: a tile's copy is issued as soon as the previous user of its buffer has read its
+// powers into registers, i.e. a whole tile ahead.  Two CTA barriers per tile (both inside the scan).
+// counters[2] = cells appended (the refine kernel's work count), counters[3] = cells dropped because the list was full
+// (their tile's blocks are all marked instead, which is always allowed: kernel (c) decides).
+// Dynamic shared memory: [2 × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
 __global__ void __launch_bounds__(kSweepThreads, 4)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
-                    const float* __restrict__ Tp_g, unsigned* __restrict__ bitmap, unsigned* __restrict__ flagged,
-                    unsigned* __restrict__ counters) {
+                    SweepCell* __restrict__ cells, unsigned cell_cap, unsigned* __restrict__ bitmap,
+                    unsigned* __restrict__ flagged, unsigned* __restrict__ counters) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float* Zb0 = reinterpret_cast<float*>(smem_raw);
-    float* sG = Zb0 + 2 * sp.z_floats;
-    float* sTau = Zb0 + sp.smem_floats;
-    float* sTp = sTau + ((sp.ntau + 3) & ~3);
-    SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTp + ((sp.zmax + 3) & ~3));
-    unsigned char* sflag = reinterpret_cast<unsigned char*>(&ctl + 1);
-    const int tid = threadIdx.x;
+    float* raw0 = reinterpret_cast<float*>(smem_raw);
+    float* sG = raw0 + 2 * sp.z_floats;
+    float* sTau = raw0 + sp.smem_floats;
+    SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTau + ((sp.ntau + 3) & ~3));
+    const int tid = threadIdx.x, lane = tid & 31;
     const long long stride = gridDim.x;
-    const float inv_C = 1.0f / (float)C;
 
-    // ---- once per CTA: τ table, constants of the buffers, the first two copies
+    // ---- once per CTA: τ table, zeros after len and in the arrays (PG[0] = 0, pads), task list, the first two copies
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
-    for (int i = tid; i < sp.zmax; i += kSweepThreads) sTp[i] = Tp_g[i];
-    for (int i = tid; i < sp.smem_floats - 2 * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;   // incl. the arrays' pads
-    if (tid < 2) Zb0[tid * sp.z_floats + 3] = 0.f;                                             // PP[0]
-    if (tid < 2 * kScanPer) Zb0[(tid / kScanPer) * sp.z_floats + 4 + sp.len + tid % kScanPer] = 0.f;   // zeros after len
+    for (int i = tid; i < sp.smem_floats - 2 * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;
+    if (tid < 2 * kScanPer) raw0[(tid / kScanPer) * sp.z_floats + sp.len + tid % kScanPer] = 0.f;
     for (int q = tid; q < sp.ntasks; q += kSweepThreads) {
         int L = 0;
         while (L + 1 < sp.nlevels && q >= sp.lv[L + 1].wt_off) ++L;
@@ -489,7 +372,6 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
         ctl.task[q] = WarpTask{lv.pg_off, lv.tau_off, lv.m_start, lv.nsteps, L, (q - lv.wt_off) * 32 * kSweepR, lv.nk, 0};
     }
     if (tid == 0) {
-        ctl.work_n = 0;
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[0])));
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[1])));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -497,34 +379,119 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
     __syncthreads();
     if (tid == 0) {
         const long long i0 = blockIdx.x;
-        if (i0 < n_items) sweep_issue_tile(sp, i0, P, pitchP, n, tiles_per_row, C, Zb0, &ctl.mbar[0], ctl.meta[0]);
-        if (i0 + stride < n_items)
-            sweep_issue_tile(sp, i0 + stride, P, pitchP, n, tiles_per_row, C, Zb0 + sp.z_floats, &ctl.mbar[1], ctl.meta[1]);
+        if (i0 < n_items) sweep_issue_tile(sp, i0, P, pitchP, tiles_per_row, raw0, &ctl.mbar[0]);
+        if (i0 + stride < n_items) sweep_issue_tile(sp, i0 + stride, P, pitchP, tiles_per_row, raw0 + sp.z_floats, &ctl.mbar[1]);
     }
-    __syncthreads();
+
+    // (row, tile index) of the current item, advanced without divisions
+    long long row = blockIdx.x / tiles_per_row;
+    int tix = (int)(blockIdx.x - row * tiles_per_row);
+    const long long drow = stride / tiles_per_row;
+    const int dtix = (int)(stride - drow * tiles_per_row);
 
     int it = 0;
     for (long long item = blockIdx.x; item < n_items; item += stride, ++it) {
         const int b = it & 1;
-        float* Z = Zb0 + b * sp.z_floats;
-        const TileMeta mt = ctl.meta[b];
+        float* raw = raw0 + b * sp.z_floats;
         mbar_wait(&ctl.mbar[b], (uint32_t)(it >> 1) & 1u);
-        if (mt.first_pad < sp.len) {                         // last tile of a row: nothing beyond the spectrum's end
-            for (int i = mt.first_pad + tid; i < sp.len; i += kSweepThreads) Z[4 + i] = 0.f;
+        const long long nv = n - (long long)tix * sp.tile;      // valid bins from the tile's first one
+        if (nv < (long long)sp.len) {                            // last tile of a row: nothing beyond the spectrum's end
+            for (int i = (int)nv + tid; i < sp.len; i += kSweepThreads) raw[i] = 0.f;
             __syncthreads();
         }
-        scan_tile(sp, Z, sG, ctl.scan, sflag, mt.nblk_tile);
-        const float pp_max = Z[3 + sp.len];
-        SweepCtx cx{Z, sTp, sflag, mt.t0, (int)n, C, mt.t0 - mt.c_first * C, inv_C, kSlackUlps * 5.9604644775390625e-8f * pp_max};
-        sweep_covers(sp, sG, sTau, ctl, cx, mt.nblk_tile, counters);
-        if (tid == 0) {
-            ctl.work_n = 0;
+        const float pp_max = scan_tile(sp, raw, sG, ctl.scan, [&] {
             const long long nxt = item + 2 * stride;
-            if (nxt < n_items) sweep_issue_tile(sp, nxt, P, pitchP, n, tiles_per_row, C, Z, &ctl.mbar[b], ctl.meta[b]);
-        } else if (tid >= 32 && tid < 32 + kScanPer) {
-            Z[4 + sp.len + (tid - 32)] = 0.f;                // the scan has written PP garbage over the zeros after len
+            if (tid == 0 && nxt < n_items) sweep_issue_tile(sp, nxt, P, pitchP, tiles_per_row, raw, &ctl.mbar[b]);
+        });
+        const float slack = kSlackUlps * 5.9604644775390625e-8f * pp_max;
+
+        // ---- cover sums: warp-tasks dealt round-robin, most expensive levels first
+        for (int q = tid >> 5; q < sp.ntasks; q += kSweepThreads / 32) {
+            const int4 ta = *reinterpret_cast<const int4*>(&ctl.task[q]);            // pg_off, tau_off, m_start, nsteps
+            const int4 tb = *reinterpret_cast<const int4*>(&ctl.task[q].level);      // level, kbase, nk
+            const int k0b = tb.y + lane * kSweepR;
+            if (k0b < tb.z) {
+                unsigned mask = sweep_task(sG + ta.x, k0b, ta.z, ta.w, sTau + ta.y, slack);
+                while (mask) {
+                    const int st = __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    const unsigned pos = atomicAdd(counters + 2, 1u);
+                    if (pos < cell_cap) {
+                        cells[pos] = SweepCell{(unsigned)item, ((unsigned)tb.x << 28) | ((unsigned)st << 20) | (unsigned)(k0b >> 3)};
+                    } else {                                     // list full: mark every block the tile's start bins touch
+                        atomicAdd(counters + 3, 1u);
+                        const long long t0 = (long long)tix * sp.tile;
+                        const long long last = min(t0 + sp.tile - 1, n - 1);
+                        for (long long c = t0 / C; c <= last / C; ++c) mark_block((unsigned long long)(row * nblk + c), bitmap, flagged, counters);
+                    }
+                }
+            }
         }
-        publish_flags(sflag, mt.nblk_tile, mt.c_first, nblk, mt.row, bitmap, flagged, counters);
+        row += drow; tix += dtix;
+        if (tix >= tiles_per_row) { tix -= tiles_per_row; ++row; }
+    }
+}
+
+// Rare path: one warp per listed cell.  The cell covers group starts k0b..k0b+7 and cover lengths m4..m4+3 of its
+// level, i.e. the bins [k0b·g, (k0b + m4 + 10)·g) of its tile; their prefix sum is rebuilt in double from P, the 32
+// covers are re-tested against τ and the windows inside each passing cover (start in its first group, end in its last)
+// are summed and compared with T'_w.  A window that passes marks the candidate block of its start bin.
+// Dynamic shared memory: (kRefineThreads/32) × (ref_span + 1) doubles.
+__global__ void __launch_bounds__(kRefineThreads)
+sweep_refine_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
+                    int tiles_per_row, int C, long long nblk, const float* __restrict__ tau_g,
+                    const float* __restrict__ Tp_g, const SweepCell* __restrict__ cells, unsigned cell_cap,
+                    unsigned* __restrict__ bitmap, unsigned* __restrict__ flagged, unsigned* __restrict__ counters) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* pp = reinterpret_cast<double*>(smem_raw) + (size_t)warp * (sp.ref_span + 1);
+    const unsigned ncell = min(counters[2], cell_cap);
+    const unsigned nwarps = gridDim.x * (kRefineThreads / 32);
+    for (unsigned e = blockIdx.x * (kRefineThreads / 32) + warp; e < ncell; e += nwarps) {
+        const SweepCell cell = cells[e];
+        const SweepLevel& lv = sp.lv[cell.code >> 28];
+        const int step = (int)((cell.code >> 20) & 0xFFu), k0b = (int)(cell.code & 0xFFFFFu) << 3;
+        const int lg = lv.lg, g = 1 << lg, m4 = lv.m_start + 4 * step;
+        const long long row = cell.item / (unsigned)tiles_per_row;
+        const long long base = (long long)(cell.item - (unsigned)(row * tiles_per_row)) * sp.tile + ((long long)k0b << lg);
+        const int span = (m4 + 10) << lg;                        // ≤ ref_span
+        const long long room = n - base;
+        const int valid = (int)(room < (long long)span ? (room < 0 ? 0 : room) : (long long)span);
+        const float* src = P + row * pitchP + base;
+        // ---- prefix sum in double, 32 bins per step
+        double carry = 0.0;
+        if (lane == 0) pp[0] = 0.0;
+        for (int j0 = 0; j0 < span; j0 += 32) {
+            const int j = j0 + lane;
+            double x = (j < valid) ? (double)__ldg(src + j) : 0.0;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const double t = __shfl_up_sync(0xffffffffu, x, off);
+                if (lane >= off) x += t;
+            }
+            x += carry;
+            if (j < span) pp[j + 1] = x;
+            carry = __shfl_sync(0xffffffffu, x, 31);
+        }
+        __syncwarp();
+        // ---- re-test the 32 covers (lane = 8·(m − m4) + (k0 − k0b)), then the windows of those that pass
+        const int r = lane & 7, m = m4 + (lane >> 3);
+        const bool live = pp[(r + m) << lg] - pp[r << lg] >= (double)__ldg(tau_g + lv.tau_off + 4 * step + (lane >> 3)) * (1.0 - 1e-6);
+        unsigned hits = __ballot_sync(0xffffffffu, live);
+        while (hits) {
+            const int srcl = __ffs(hits) - 1;
+            hits &= hits - 1;
+            const int rr = srcl & 7, mm = m4 + (srcl >> 3);
+            const int i0 = rr << lg, e0 = (rr + mm - 1) << lg;
+            for (int idx = lane; idx < g * g; idx += 32) {
+                const int i = i0 + (idx >> lg), ee = e0 + (idx & (g - 1));
+                const int w = ee - i + 1;
+                if (w < 1 || w < lv.wlo || w > lv.whi || ee >= valid) continue;
+                if (pp[ee + 1] - pp[i] >= (double)__ldg(Tp_g + (w - 1)))
+                    mark_block((unsigned long long)(row * nblk + (base + i) / C), bitmap, flagged, counters);
+            }
+        }
+        __syncwarp();
     }
 }
 

@@ -78,7 +78,8 @@ struct pulscan_plan {
     SweepParams sp{};
     int tiles_per_row = 0;
     int sweep_grid = 0;        // persistent CTAs of the pruned sweep: SM count × resident CTAs per SM
-    size_t smem_sweep = 0, smem_exh = 0, smem_exact = 0;
+    size_t smem_sweep = 0, smem_refine = 0, smem_exh = 0, smem_exact = 0;
+    unsigned cell_cap = 0;     // capacity of the flagged-cell list between the sweep and its refine kernel
     int exh_len = 0;
     // normalisation launch shapes
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
@@ -87,7 +88,7 @@ struct pulscan_plan {
     // workspace (device, caller-owned)
     void* ws = nullptr;
     size_t ws_bytes = 0;
-    size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_redo = 0, off_stage_in = 0, off_stage_cand = 0,
+    size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_redo = 0, off_cells = 0, off_stage_in = 0, off_stage_cand = 0,
            off_stage_count = 0, bitmap_bytes = 0, need_bytes = 0;
     // device tables (plan-owned, small)
     double* d_T = nullptr;
@@ -135,7 +136,8 @@ int derive(pulscan_plan& p) {
     int tile = p.tile_user ? p.tile_user : (p.zmax <= 512 ? 4096 : 8192);
     // ---- group size per width: the largest g = 2^lg whose worst cover (w + 2g − 2 bins) of pure noise passes the
     //      width's threshold with probability ≤ p_flag; made non-decreasing in w by a suffix minimum.
-    //      If the width range then needs more than kMaxLevels levels (very low σ thresholds), p_flag is relaxed
+    //      g = 4 is always allowed (at very low σ thresholds its covers simply pass often and the refine kernel and
+    //      kernel (c) do the work).  If the width range then needs more than kMaxLevels levels, p_flag is relaxed
     //      tenfold at a time: it affects speed only.
     const int lg_cap = 6;
     std::vector<int> lgw(p.zmax + 2, 0);
@@ -144,8 +146,8 @@ int derive(pulscan_plan& p) {
     for (double l10 = p.log10_p_flag;; l10 += 1.0) {
         const double ln_pflag = l10 * 2.302585092994046;
         for (int w = 1; w <= p.zmax; ++w) {
-            int best = 0;
-            for (int lg = 1; lg <= lg_cap; ++lg) {
+            int best = 2;                 // the scan produces PP at multiples of 4 only: the finest group is 4 bins
+            for (int lg = 3; lg <= lg_cap; ++lg) {
                 const int g = 1 << lg, Lc = w + 2 * g - 2;
                 if ((tile >> lg) % kSweepR != 0) break;
                 if (l10 >= 0.0 || ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
@@ -182,14 +184,14 @@ int derive(pulscan_plan& p) {
         }
         if (fits) {   // shared memory of the two tile buffers + one decimated array per distinct group size
             const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
-            size_t fl = 2 * ((size_t)len + kScanPer + 8);
+            size_t fl = 2 * ((size_t)len + kScanPer + 4);
             std::vector<int> seen;
             for (const SweepLevel& lv : lvls)
                 if (std::find(seen.begin(), seen.end(), lv.lg) == seen.end()) {
                     seen.push_back(lv.lg);
                     fl += (size_t)(len >> lv.lg) + 1 + kPadG + 3;
                 }
-            if (fl * 4 + (size_t)p.zmax * 4 + sizeof(SweepCtl) + 8192 <= 227 * 1024) break;
+            if (fl * 4 + sizeof(SweepCtl) + 2048 <= 227 * 1024) break;
         }
         if (l10 >= 0.0) return fail(PULSCAN_EINVAL, "zmax = %d with tile = %d does not fit the sweep's shared memory", p.zmax, tile);
     }
@@ -202,7 +204,7 @@ int derive(pulscan_plan& p) {
     const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
     sp.len = tile + halo;
     sp.npass = (sp.len + kScanPass - 1) / kScanPass;
-    sp.z_floats = (int)align_up((size_t)(4 + sp.len + kScanPer), 4);
+    sp.z_floats = (int)align_up((size_t)(sp.len + kScanPer), 4);
     int off = 0, task = 0;
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = lvls[l];
@@ -233,7 +235,12 @@ int derive(pulscan_plan& p) {
     p.tiles_per_row = (int)((p.n + tile - 1) / tile);
     const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
     sp.zmax = p.zmax;
-    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + align_up((size_t)p.zmax, 4) * 4 + sizeof(SweepCtl) + flag_bytes;
+    sp.ref_span = 0;
+    for (int l = 0; l < sp.nlevels; ++l)
+        sp.ref_span = std::max(sp.ref_span, (sp.lv[l].m_start + 4 * sp.lv[l].nsteps + 6) << sp.lv[l].lg);
+    p.smem_sweep = (size_t)sp.smem_floats * 4 + align_up((size_t)sp.ntau, 4) * 4 + sizeof(SweepCtl);
+    p.smem_refine = (size_t)(kRefineThreads / 32) * (sp.ref_span + 1) * sizeof(double);
+    if (p.smem_refine > 227 * 1024) return fail(PULSCAN_EINVAL, "refine span of %d bins does not fit shared memory", sp.ref_span);
     if (p.smem_sweep > 227 * 1024) return fail(PULSCAN_EINVAL, "sweep tile needs %zu bytes of shared memory", p.smem_sweep);
     p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
@@ -264,6 +271,10 @@ int derive(pulscan_plan& p) {
     p.off_flagged = o; o += align_up((size_t)p.batch * p.nblk * 4, 256);
     p.off_counters = o; o += 256;
     p.off_redo = o; o += align_up((size_t)p.batch * p.nb * 4, 256);
+    // noise flags ≈ 0.6 cells per 4096 bins at the default p_flag; room for 16 per 4096 bins (then tiles fall back to
+    // marking all their blocks)
+    p.cell_cap = (unsigned)std::min<unsigned long long>(1ull << 28, std::max<unsigned long long>(65536, (unsigned long long)p.batch * p.n / 256));
+    p.off_cells = o; o += align_up((size_t)p.cell_cap * sizeof(SweepCell), 256);
     if (p.host_staging) {
         p.off_stage_in = o; o += align_up((size_t)p.batch * p.pitch * 8, 256);
         p.off_stage_cand = o; o += align_up((size_t)p.batch * p.nblk * sizeof(pulscan_candidate), 256);
@@ -291,6 +302,7 @@ int ensure_device(pulscan_plan& p) {
     CUDA_TRY(cudaMemcpy(p.d_Tp, p.Tp.data(), p.Tp.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(p.d_tau, p.tau.data(), p.tau.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_sweep));
+    CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_refine));
     int occ = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, boxcar_sweep_kernel, kSweepThreads, p.smem_sweep));
     if (occ < 1) return fail(PULSCAN_ECUDA, "boxcar_sweep_kernel does not fit an SM with %zu bytes of shared memory", p.smem_sweep);
@@ -569,16 +581,22 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
     if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
     if (p.mode == 0) {
+        SweepCell* d_cells = reinterpret_cast<SweepCell*>(ws + p.off_cells);
         boxcar_sweep_kernel<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
-                                                                              p.C, p.nblk, p.d_tau, p.d_Tp, d_bitmap,
-                                                                              d_flagged, d_counters);
+                                                                              p.C, p.nblk, p.d_tau, d_cells, p.cell_cap,
+                                                                              d_bitmap, d_flagged, d_counters);
+        CUDA_TRY(cudaGetLastError());
+        if ((rc = debug_sync("boxcar_sweep_kernel"))) return rc;
+        sweep_refine_kernel<<<p.sm_count * 4, kRefineThreads, p.smem_refine, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
+                                                                                  p.nblk, p.d_tau, p.d_Tp, d_cells, p.cell_cap,
+                                                                                  d_bitmap, d_flagged, d_counters);
     } else {
         boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_P, p.pitchP,
                                                                                 p.n, p.tiles_per_row, p.C, p.nblk, p.d_Tp,
                                                                                 d_bitmap, d_flagged, d_counters);
     }
     CUDA_TRY(cudaGetLastError());
-    if ((rc = debug_sync(p.mode ? "boxcar_exhaustive_kernel" : "boxcar_sweep_kernel"))) return rc;
+    if ((rc = debug_sync(p.mode ? "boxcar_exhaustive_kernel" : "sweep_refine_kernel"))) return rc;
     if (ev) CUDA_TRY(cudaEventRecord(ev[3], st));
 
     const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
@@ -673,7 +691,7 @@ int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_str
 int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan) {
     if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
     if (derive(*const_cast<pulscan_plan*>(plan))) return -1;
-    return (plan->main_blocks_per_row > 0 ? (plan->use_fast ? 2 : 1) : 0) + (plan->has_tail ? 1 : 0) + 2;
+    return (plan->main_blocks_per_row > 0 ? (plan->use_fast ? 2 : 1) : 0) + (plan->has_tail ? 1 : 0) + (plan->mode == 0 ? 3 : 2);
 }
 
 int pulscan_plan_set_profiling(pulscan_plan* plan, int32_t n_slots) {

@@ -92,8 +92,8 @@ def test_sizes(binding):
     assert 256 * 4194308 * 4 <= ws <= 256 * 4194308 * 4 + 64e6
     ph = binding.Plan(4194305, 256, 200, 200, 6.0, norm_block=4096, host_staging=True)
     assert ph.workspace_bytes >= ws + 256 * 4194305 * 8
-    assert p.launches_per_search == 5      # (a) fast + (a) redo + (a) last blocks + (b) + (c)
-    assert binding.Plan(4096 * 8, 2, 16, 64, 6.0, norm_block=4096).launches_per_search == 4   # no ragged last block
+    assert p.launches_per_search == 6      # (a) single-histogram + (a) redo + (a) last blocks + (b) sweep + (b) refine + (c)
+    assert binding.Plan(4096 * 8, 2, 16, 64, 6.0, norm_block=4096).launches_per_search == 5   # no ragged last block
 
 
 def test_thresholds_match_survival_function(binding):
