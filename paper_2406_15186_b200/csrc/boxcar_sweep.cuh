@@ -458,21 +458,23 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const float* __restr
         const long long room = n - base;
         const int valid = (int)(room < (long long)span ? (room < 0 ? 0 : room) : (long long)span);
         const float* src = P + row * pitchP + base;
-        // ---- prefix sum in double, 32 bins per step
-        double carry = 0.0;
+        // ---- prefix sum in double: stage the span (coalesced loads, several in flight), then each lane scans its own
+        //      chunk of L consecutive bins and the chunk totals are scanned across the warp
+        for (int j = lane; j < span; j += 32) pp[j + 1] = (j < valid) ? (double)__ldg(src + j) : 0.0;
         if (lane == 0) pp[0] = 0.0;
-        for (int j0 = 0; j0 < span; j0 += 32) {
-            const int j = j0 + lane;
-            double x = (j < valid) ? (double)__ldg(src + j) : 0.0;
+        __syncwarp();
+        const int L = (span + 31) >> 5;
+        const int c0 = min(lane * L, span), c1 = min(c0 + L, span);
+        double run = 0.0;
+        for (int j = c0; j < c1; ++j) { run += pp[j + 1]; pp[j + 1] = run; }
+        double incl = run;
 #pragma unroll
-            for (int off = 1; off < 32; off <<= 1) {
-                const double t = __shfl_up_sync(0xffffffffu, x, off);
-                if (lane >= off) x += t;
-            }
-            x += carry;
-            if (j < span) pp[j + 1] = x;
-            carry = __shfl_sync(0xffffffffu, x, 31);
+        for (int off = 1; off < 32; off <<= 1) {
+            const double t = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += t;
         }
+        const double excl = incl - run;
+        for (int j = c0; j < c1; ++j) pp[j + 1] += excl;
         __syncwarp();
         // ---- re-test the 32 covers (lane = 8·(m − m4) + (k0 − k0b)), then the windows of those that pass
         const int r = lane & 7, m = m4 + (lane >> 3);
@@ -483,6 +485,12 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             hits &= hits - 1;
             const int rr = srcl & 7, mm = m4 + (srcl >> 3);
             const int i0 = rr << lg, e0 = (rr + mm - 1) << lg;
+            if (g <= C) {   // nothing left to find if the (one or two) blocks owning the cover's start bins are already marked
+                const unsigned long long ga = (unsigned long long)(row * nblk + (base + i0) / C);
+                const unsigned long long gb = (unsigned long long)(row * nblk + min(base + i0 + g - 1, n - 1) / C);
+                const unsigned wa = __ldcg(bitmap + (ga >> 5)), wb = __ldcg(bitmap + (gb >> 5));
+                if ((wa >> (ga & 31) & 1u) && (wb >> (gb & 31) & 1u)) continue;
+            }
             for (int idx = lane; idx < g * g; idx += 32) {
                 const int i = i0 + (idx >> lg), ee = e0 + (idx & (g - 1));
                 const int w = ee - i + 1;

@@ -77,6 +77,7 @@ struct pulscan_plan {
     std::vector<float> tau;    // per-level cover thresholds
     SweepParams sp{};
     int tiles_per_row = 0;
+    int refine_grid = 0;
     int sweep_grid = 0;        // persistent CTAs of the pruned sweep: SM count × resident CTAs per SM
     size_t smem_sweep = 0, smem_refine = 0, smem_exh = 0, smem_exact = 0;
     unsigned cell_cap = 0;     // capacity of the flagged-cell list between the sweep and its refine kernel
@@ -307,6 +308,9 @@ int ensure_device(pulscan_plan& p) {
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, boxcar_sweep_kernel, kSweepThreads, p.smem_sweep));
     if (occ < 1) return fail(PULSCAN_ECUDA, "boxcar_sweep_kernel does not fit an SM with %zu bytes of shared memory", p.smem_sweep);
     p.sweep_grid = (int)std::min<long long>((long long)p.tiles_per_row * p.batch, (long long)p.sm_count * occ);
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_refine_kernel, kRefineThreads, p.smem_refine));
+    if (occ < 1) return fail(PULSCAN_ECUDA, "sweep_refine_kernel does not fit an SM with %zu bytes of shared memory", p.smem_refine);
+    p.refine_grid = p.sm_count * std::min(occ, 16);
     CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exh));
     CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exact));
     p.device_ready = true;
@@ -587,7 +591,7 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
                                                                               d_bitmap, d_flagged, d_counters);
         CUDA_TRY(cudaGetLastError());
         if ((rc = debug_sync("boxcar_sweep_kernel"))) return rc;
-        sweep_refine_kernel<<<p.sm_count * 4, kRefineThreads, p.smem_refine, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
+        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
                                                                                   p.nblk, p.d_tau, p.d_Tp, d_cells, p.cell_cap,
                                                                                   d_bitmap, d_flagged, d_counters);
     } else {
