@@ -21,7 +21,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
     tmp = LIB.with_suffix(f".{os.getpid()}.tmp")
-    cmd = [nvcc, *NVCC_FLAGS] + (["-Xptxas", "-v"] if verbose else []) + ["-o", str(tmp)] + [str(s) for s in SOURCES]
+    extra = os.environ.get("PULSCAN_NVCC_EXTRA", "").split()
+    cmd = [nvcc, *NVCC_FLAGS, *extra] + (["-Xptxas", "-v"] if verbose else []) + ["-o", str(tmp)] + [str(s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

@@ -40,6 +40,13 @@ constexpr int kSweepThreads = 256;
 constexpr int kSweepR = 8;                 // consecutive group starts per thread
 constexpr int kScanPer = 20;               // floats per thread per scan pass: 80-byte lane stride is bank-conflict-free
 constexpr int kScanPass = kScanPer * kSweepThreads;
+#ifndef PULSCAN_SWEEP_BUFS
+#define PULSCAN_SWEEP_BUFS 2
+#endif
+#ifndef PULSCAN_SWEEP_OCC
+#define PULSCAN_SWEEP_OCC 4
+#endif
+constexpr int kSweepBufs = PULSCAN_SWEEP_BUFS;   // landing buffers per CTA (copies in flight ahead of the scan)
 constexpr int kRefineThreads = 128;        // sweep_refine_kernel: 4 warps, one listed cell per warp at a time
 constexpr int kMaxWarpTasks = 128;         // warp-tasks per tile (8 levels of at most tile/(256·g) each)
 constexpr int kPadG = 16;                  // replicated entries after each decimated prefix array (window over-read)
@@ -299,7 +306,7 @@ struct SweepCell {
 
 struct SweepCtl {
     ScanSmem scan;
-    alignas(8) uint64_t mbar[2];
+    alignas(8) uint64_t mbar[kSweepBufs];
     WarpTask task[kMaxWarpTasks];
 };
 
@@ -347,15 +354,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
 // powers into registers, i.e. a whole tile ahead.  Two CTA barriers per tile (both inside the scan).
 // counters[2] = cells appended (the refine kernel's work count), counters[3] = cells dropped because the list was full
 // (their tile's blocks are all marked instead, which is always allowed: kernel (c) decides).
-// Dynamic shared memory: [2 × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
-__global__ void __launch_bounds__(kSweepThreads, 4)
+// Dynamic shared memory: [kSweepBufs × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
+__global__ void __launch_bounds__(kSweepThreads, PULSCAN_SWEEP_OCC)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
                     SweepCell* __restrict__ cells, unsigned cell_cap, unsigned* __restrict__ bitmap,
                     unsigned* __restrict__ flagged, unsigned* __restrict__ counters) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* raw0 = reinterpret_cast<float*>(smem_raw);
-    float* sG = raw0 + 2 * sp.z_floats;
+    float* sG = raw0 + kSweepBufs * sp.z_floats;
     float* sTau = raw0 + sp.smem_floats;
     SweepCtl& ctl = *reinterpret_cast<SweepCtl*>(sTau + ((sp.ntau + 3) & ~3));
     const int tid = threadIdx.x, lane = tid & 31;
@@ -363,8 +370,8 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
 
     // ---- once per CTA: τ table, zeros after len and in the arrays (PG[0] = 0, pads), task list, the first two copies
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
-    for (int i = tid; i < sp.smem_floats - 2 * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;
-    if (tid < 2 * kScanPer) raw0[(tid / kScanPer) * sp.z_floats + sp.len + tid % kScanPer] = 0.f;
+    for (int i = tid; i < sp.smem_floats - kSweepBufs * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;
+    if (tid < kSweepBufs * kScanPer) raw0[(tid / kScanPer) * sp.z_floats + sp.len + tid % kScanPer] = 0.f;
     for (int q = tid; q < sp.ntasks; q += kSweepThreads) {
         int L = 0;
         while (L + 1 < sp.nlevels && q >= sp.lv[L + 1].wt_off) ++L;
@@ -372,15 +379,15 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
         ctl.task[q] = WarpTask{lv.pg_off, lv.tau_off, lv.m_start, lv.nsteps, L, (q - lv.wt_off) * 32 * kSweepR, lv.nk, 0};
     }
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[0])));
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[1])));
+        for (int b = 0; b < kSweepBufs; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&ctl.mbar[b])));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     if (tid == 0) {
         const long long i0 = blockIdx.x;
-        if (i0 < n_items) sweep_issue_tile(sp, i0, P, pitchP, tiles_per_row, raw0, &ctl.mbar[0]);
-        if (i0 + stride < n_items) sweep_issue_tile(sp, i0 + stride, P, pitchP, tiles_per_row, raw0 + sp.z_floats, &ctl.mbar[1]);
+        for (int b = 0; b < kSweepBufs; ++b)
+            if (i0 + b * stride < n_items)
+                sweep_issue_tile(sp, i0 + b * stride, P, pitchP, tiles_per_row, raw0 + b * sp.z_floats, &ctl.mbar[b]);
     }
 
     // (row, tile index) of the current item, advanced without divisions
@@ -391,16 +398,16 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
 
     int it = 0;
     for (long long item = blockIdx.x; item < n_items; item += stride, ++it) {
-        const int b = it & 1;
+        const int b = it % kSweepBufs;
         float* raw = raw0 + b * sp.z_floats;
-        mbar_wait(&ctl.mbar[b], (uint32_t)(it >> 1) & 1u);
+        mbar_wait(&ctl.mbar[b], (uint32_t)(it / kSweepBufs) & 1u);
         const long long nv = n - (long long)tix * sp.tile;      // valid bins from the tile's first one
         if (nv < (long long)sp.len) {                            // last tile of a row: nothing beyond the spectrum's end
             for (int i = (int)nv + tid; i < sp.len; i += kSweepThreads) raw[i] = 0.f;
             __syncthreads();
         }
         const float pp_max = scan_tile(sp, raw, sG, ctl.scan, [&] {
-            const long long nxt = item + 2 * stride;
+            const long long nxt = item + kSweepBufs * stride;
             if (tid == 0 && nxt < n_items) sweep_issue_tile(sp, nxt, P, pitchP, tiles_per_row, raw, &ctl.mbar[b]);
         });
         const float slack = kSlackUlps * 5.9604644775390625e-8f * pp_max;

@@ -367,16 +367,19 @@ __device__ __forceinline__ void v2_mbar_wait(unsigned long long* mbar, unsigned 
 }
 
 // Dynamic shared memory of norm_power_v2_kernel<EPT, NT>: [stage: 8·B + 16 bytes][hist: 2·NB·4][V2Ctl].
-template <int EPT, int NT>
+template <int EPT, int NT, bool STAGED>
 constexpr size_t v2_smem_bytes() {
-    return (size_t)EPT * NT * 8 + 16 + (size_t)2 * kV2NB * 4 + sizeof(V2Ctl);
+    return (STAGED ? (size_t)EPT * NT * 8 + 16 : 0) + (size_t)2 * kV2NB * 4 + sizeof(V2Ctl);
 }
 
 // Grid: blocks_per_row · batch CTAs; CTA x handles block (x mod blocks_per_row) of spectrum x / blocks_per_row, bins
 // [j·B, (j+1)·B).  `lim_lo`/`lim_hi` bound the input allocation: the TMA copy is 16-byte granular and is only used when
 // its rounded range stays inside; otherwise the CTA stages the block with ordinary loads.
-template <int EPT, int NT>
-__global__ void __launch_bounds__(NT, (EPT * NT <= 4096) ? 4 : 2)
+// STAGED = false: nothing is staged; the histogram pass, the (rare) gather hits and the output pass read the block from
+// global memory (the second and third time out of L1/L2, where a block read microseconds earlier still is), which
+// leaves 19 KB of shared memory per CTA so that more blocks are in flight per SM to cover the warp-serial phases.
+template <int EPT, int NT, bool STAGED>
+__global__ void __launch_bounds__(NT, STAGED ? ((EPT * NT <= 4096) ? 4 : 2) : ((EPT * NT <= 4096) ? 6 : 4))
 norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int blocks_per_row, float* __restrict__ P,
                      long long pitchP, unsigned* __restrict__ redo, unsigned* __restrict__ redo_count,
                      const char* __restrict__ lim_lo, const char* __restrict__ lim_hi) {
@@ -385,7 +388,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     constexpr int B = EPT * NT;
     extern __shared__ __align__(128) unsigned char v2_raw[];
     unsigned char* stage = v2_raw;
-    unsigned* hist = reinterpret_cast<unsigned*>(v2_raw + (size_t)B * 8 + 16);
+    unsigned* hist = reinterpret_cast<unsigned*>(v2_raw + (STAGED ? (size_t)B * 8 + 16 : 0));
     V2Ctl& ctl = *reinterpret_cast<V2Ctl*>(hist + 2 * kV2NB);
     const int tid = threadIdx.x, warp = tid >> 5;
     const unsigned row = blockIdx.x / (unsigned)blocks_per_row;
@@ -397,8 +400,8 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     const unsigned shift = (unsigned)(reinterpret_cast<uintptr_t>(src) & 15);          // 0 or 8
     const char* csrc = reinterpret_cast<const char*>(src) - shift;
     const unsigned nbytes = (unsigned)B * 8u + (shift ? 16u : 0u);
-    const bool use_tma = csrc >= lim_lo && csrc + nbytes <= lim_hi;
-    const float2* sdat = reinterpret_cast<const float2*>(stage + shift);
+    const bool use_tma = STAGED && csrc >= lim_lo && csrc + nbytes <= lim_hi;
+    const float2* sdat = STAGED ? reinterpret_cast<const float2*>(stage + shift) : src;
     if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(v2_smem(&ctl.mbar)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -410,7 +413,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
 #pragma unroll
         for (int i = tid; i < 2 * kV2NB / 4; i += NT) hz[i] = make_uint4(0, 0, 0, 0);
     }
-    if (!use_tma) {
+    if (STAGED && !use_tma) {
         float2* sw = reinterpret_cast<float2*>(stage + shift);
 #pragma unroll 4
         for (int r = 0; r < EPT; ++r) sw[tid + r * NT] = __ldg(src + tid + r * NT);

@@ -85,6 +85,7 @@ struct pulscan_plan {
     // normalisation launch shapes
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
     bool has_tail = false;
+    bool norm_staged = false;  // single-histogram kernel variant: block staged in shared memory by TMA, or read from global
     bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_v2_kernel + redo list
     // workspace (device, caller-owned)
     void* ws = nullptr;
@@ -185,7 +186,7 @@ int derive(pulscan_plan& p) {
         }
         if (fits) {   // shared memory of the two tile buffers + one decimated array per distinct group size
             const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
-            size_t fl = 2 * ((size_t)len + kScanPer + 4);
+            size_t fl = kSweepBufs * ((size_t)len + kScanPer + 4);
             std::vector<int> seen;
             for (const SweepLevel& lv : lvls)
                 if (std::find(seen.begin(), seen.end(), lv.lg) == seen.end()) {
@@ -232,7 +233,7 @@ int derive(pulscan_plan& p) {
     sp.ntasks = task;
     if (task > kMaxWarpTasks) return fail(PULSCAN_EINVAL, "sweep tile of %d bins needs %d warp-tasks (limit %d)", tile, task, kMaxWarpTasks);
     sp.ntau = (int)p.tau.size();
-    sp.smem_floats = 2 * sp.z_floats + off;
+    sp.smem_floats = kSweepBufs * sp.z_floats + off;
     p.tiles_per_row = (int)((p.n + tile - 1) / tile);
     const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
     sp.zmax = p.zmax;
@@ -261,6 +262,7 @@ int derive(pulscan_plan& p) {
         p.main_blocks_per_row = p.nb;
     }
 
+    p.norm_staged = std::getenv("PULSCAN_NORM_STAGED") != nullptr;
     p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 &&
                  std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
 
@@ -362,17 +364,20 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
                      unsigned* redo_count) {
     const char* lim_lo = reinterpret_cast<const char*>(spec);
     const char* lim_hi = lim_lo + ((size_t)(p.batch - 1) * p.pitch + p.n) * 8;
-#define PULSCAN_V2_CASE(E)                                                                                            \
-    case E: {                                                                                                         \
+#define PULSCAN_V2_LAUNCH(E, ST)                                                                                      \
+    {                                                                                                                 \
         static bool attr_set = false;                                                                                 \
         if (!attr_set) {                                                                                              \
-            CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<E, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
-                                          (int)v2_smem_bytes<E, 256>()));                                             \
+            CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<E, 256, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                          (int)v2_smem_bytes<E, 256, ST>()));                                         \
             attr_set = true;                                                                                          \
         }                                                                                                             \
-        norm_power_v2_kernel<E, 256><<<grid, 256, v2_smem_bytes<E, 256>(), st>>>(spec, p.pitch, p.main_blocks_per_row, \
-                                                                                 P, p.pitchP, redo, redo_count,       \
-                                                                                 lim_lo, lim_hi);                     \
+        norm_power_v2_kernel<E, 256, ST><<<grid, 256, v2_smem_bytes<E, 256, ST>(), st>>>(                              \
+            spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo, redo_count, lim_lo, lim_hi);                     \
+    }
+#define PULSCAN_V2_CASE(E)                                                                                            \
+    case E: {                                                                                                         \
+        if (p.norm_staged) PULSCAN_V2_LAUNCH(E, true) else PULSCAN_V2_LAUNCH(E, false)                                \
         norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P,        \
                                                                   p.pitchP, redo, redo_count);                        \
         break;                                                                                                        \
@@ -385,6 +390,7 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
         PULSCAN_V2_CASE(32)
         default: return fail(PULSCAN_EINVAL, "internal: unsupported elements-per-thread %d", p.ept_main);
     }
+#undef PULSCAN_V2_LAUNCH
 #undef PULSCAN_V2_CASE
     CUDA_TRY(cudaGetLastError());
     return debug_sync("fast normalisation kernel + norm_power_redo_kernel");
