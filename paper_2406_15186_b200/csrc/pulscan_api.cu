@@ -85,6 +85,7 @@ struct pulscan_plan {
     // normalisation launch shapes
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
     bool has_tail = false;
+    int norm_nt = 256;         // threads per CTA of the single-histogram kernel
     bool norm_staged = false;  // single-histogram kernel variant: block staged in shared memory by TMA, or read from global
     bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_v2_kernel + redo list
     // workspace (device, caller-owned)
@@ -263,6 +264,9 @@ int derive(pulscan_plan& p) {
     }
 
     p.norm_staged = std::getenv("PULSCAN_NORM_STAGED") != nullptr;
+    // 128-thread CTAs (two of four warps busy in the warp-serial phases, 8 CTAs/SM) measured 8 % faster than 256-thread
+    // ones at cfg 3; B = 8192 needs 256 threads (at most 32 values per thread)
+    p.norm_nt = (std::getenv("PULSCAN_NORM_NT256") == nullptr && p.ept_main <= 16) ? 128 : 256;
     p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 &&
                  std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
 
@@ -364,20 +368,22 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
                      unsigned* redo_count) {
     const char* lim_lo = reinterpret_cast<const char*>(spec);
     const char* lim_hi = lim_lo + ((size_t)(p.batch - 1) * p.pitch + p.n) * 8;
-#define PULSCAN_V2_LAUNCH(E, ST)                                                                                      \
+#define PULSCAN_V2_LAUNCH(E, NT_, ST)                                                                                 \
     {                                                                                                                 \
         static bool attr_set = false;                                                                                 \
         if (!attr_set) {                                                                                              \
-            CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<E, 256, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                          (int)v2_smem_bytes<E, 256, ST>()));                                         \
+            CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<E, NT_, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                          (int)v2_smem_bytes<E, NT_, ST>()));                                         \
             attr_set = true;                                                                                          \
         }                                                                                                             \
-        norm_power_v2_kernel<E, 256, ST><<<grid, 256, v2_smem_bytes<E, 256, ST>(), st>>>(                              \
+        norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                              \
             spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo, redo_count, lim_lo, lim_hi);                     \
     }
 #define PULSCAN_V2_CASE(E)                                                                                            \
     case E: {                                                                                                         \
-        if (p.norm_staged) PULSCAN_V2_LAUNCH(E, true) else PULSCAN_V2_LAUNCH(E, false)                                \
+        if (p.norm_staged) PULSCAN_V2_LAUNCH(E, 256, true)                                                            \
+        else if (p.norm_nt == 128) PULSCAN_V2_LAUNCH(2 * E, 128, false)                                               \
+        else PULSCAN_V2_LAUNCH(E, 256, false)                                                                         \
         norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P,        \
                                                                   p.pitchP, redo, redo_count);                        \
         break;                                                                                                        \
@@ -387,7 +393,12 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
         PULSCAN_V2_CASE(4)
         PULSCAN_V2_CASE(8)
         PULSCAN_V2_CASE(16)
-        PULSCAN_V2_CASE(32)
+        case 32: {
+            if (p.norm_staged) PULSCAN_V2_LAUNCH(32, 256, true) else PULSCAN_V2_LAUNCH(32, 256, false)
+            norm_power_redo_kernel<32, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P, p.pitchP, redo,
+                                                                      redo_count);
+            break;
+        }
         default: return fail(PULSCAN_EINVAL, "internal: unsupported elements-per-thread %d", p.ept_main);
     }
 #undef PULSCAN_V2_LAUNCH
