@@ -81,6 +81,12 @@ int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode);
  * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);
 
+/* Capacity (in cells, 8 bytes each) of the list that carries flagged cover cells from the sweep to its refine kernel;
+ * 0 = default (max(65536, batch·n_bins/256): ≈ 25× what noise flags at the default p_flag).  When the list is full the
+ * sweep marks every candidate block of the affected tile instead, so the setting affects speed only, never results.
+ * Changes pulscan_plan_workspace_bytes(). */
+int pulscan_plan_set_cell_capacity(pulscan_plan* plan, int64_t cells);
+
 /* Capacity the caller must give d_candidates: batch · ceil(n_bins / block_width) records. */
 int64_t pulscan_plan_max_candidates(const pulscan_plan* plan);
 

@@ -80,6 +80,7 @@ struct pulscan_plan {
     int refine_grid = 0;
     int sweep_grid = 0;        // persistent CTAs of the pruned sweep: SM count × resident CTAs per SM
     size_t smem_sweep = 0, smem_refine = 0, smem_exh = 0, smem_exact = 0;
+    unsigned cell_cap_user = 0;
     unsigned cell_cap = 0;     // capacity of the flagged-cell list between the sweep and its refine kernel
     int exh_len = 0;
     // normalisation launch shapes
@@ -281,6 +282,7 @@ int derive(pulscan_plan& p) {
     // noise flags ≈ 0.6 cells per 4096 bins at the default p_flag; room for 16 per 4096 bins (then tiles fall back to
     // marking all their blocks)
     p.cell_cap = (unsigned)std::min<unsigned long long>(1ull << 28, std::max<unsigned long long>(65536, (unsigned long long)p.batch * p.n / 256));
+    if (p.cell_cap_user) p.cell_cap = p.cell_cap_user;
     p.off_cells = o; o += align_up((size_t)p.cell_cap * sizeof(SweepCell), 256);
     if (p.host_staging) {
         p.off_stage_in = o; o += align_up((size_t)p.batch * p.pitch * 8, 256);
@@ -508,6 +510,13 @@ int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_
     plan->tile_user = tile_bins;
     plan->log10_p_flag = (log10_p_flag == 0.0) ? -3.0 : log10_p_flag;
     plan->dirty = true; release_device(*plan);
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_cell_capacity(pulscan_plan* plan, int64_t cells) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (cells < 0 || cells > (1ll << 28)) return fail(PULSCAN_EINVAL, "cell capacity out of range [0, 2^28]");
+    plan->cell_cap_user = (unsigned)cells; plan->dirty = true;
     return PULSCAN_OK;
 }
 

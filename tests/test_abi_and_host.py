@@ -67,6 +67,11 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_mode(p.handle, 7) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 1000, 0.0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 2048, -1.0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_cell_capacity(p.handle, -1) == binding.PULSCAN_EINVAL
+    ws0 = p.workspace_bytes
+    assert lib.pulscan_plan_set_cell_capacity(p.handle, 1 << 20) == binding.PULSCAN_OK
+    assert p.workspace_bytes == ws0 + ((1 << 20) - 65536) * 8          # 8-byte cells; the default here is 65536
+    assert lib.pulscan_plan_set_cell_capacity(p.handle, 0) == binding.PULSCAN_OK
     assert lib.pulscan_plan_set_workspace(p.handle, None, 1 << 30) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_workspace(p.handle, 4096 + 8, 1 << 30) == binding.PULSCAN_EINVAL      # misaligned
     assert lib.pulscan_plan_set_workspace(p.handle, 4096, 16) == binding.PULSCAN_ENOWORKSPACE

@@ -121,6 +121,15 @@ def test_tuning_never_changes_results(orc, tile, lpf):
     assert np.array_equal(ref, got)
 
 
+def test_full_cell_list_falls_back_to_marking_tiles(orc):
+    spec = noise_spectra(2, 50001, seed=99)
+    ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)
+    got, st = gpu_search(spec, 64, 2048, 128, 3.0, cell_capacity=16)
+    assert st_ref[3] == 0 and st_ref[2] > 16           # the default list holds every flagged cell of this input
+    assert st[3] > 0 and st[0] >= st_ref[0]            # cells were dropped, so whole tiles were marked instead
+    assert np.array_equal(ref, got)
+
+
 def test_pitch_and_trials(orc):
     spec = noise_spectra(3, 6000, seed=321)
     bump(spec, 1, 1000, 12, 3.5)
