@@ -265,9 +265,10 @@ int derive(pulscan_plan& p) {
     }
 
     p.norm_staged = std::getenv("PULSCAN_NORM_STAGED") != nullptr;
-    // 128-thread CTAs (two of four warps busy in the warp-serial phases, 8 CTAs/SM) measured 8 % faster than 256-thread
-    // ones at cfg 3; B = 8192 needs 256 threads (at most 32 values per thread)
-    p.norm_nt = (std::getenv("PULSCAN_NORM_NT256") == nullptr && p.ept_main <= 16) ? 128 : 256;
+    // Fewer warps per CTA: the warp-serial phases keep two warps busy and idle the rest.  Measured: cfg 3 (B = 4096)
+    // 256 threads 3.71 ms, 128 threads 3.41 ms; cfg 5 (B = 2048) 128 threads 9.06 ms, 64 threads 10.5 ms.
+    // PULSCAN_NORM_NT256 / PULSCAN_NORM_STAGED select the earlier variants for comparison.
+    p.norm_nt = (std::getenv("PULSCAN_NORM_NT256") == nullptr && !p.norm_staged && p.B >= 512 && p.B <= 4096) ? 128 : 256;
     p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 &&
                  std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
 
@@ -381,30 +382,32 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
         norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                              \
             spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo, redo_count, lim_lo, lim_hi);                     \
     }
-#define PULSCAN_V2_CASE(E)                                                                                            \
-    case E: {                                                                                                         \
-        if (p.norm_staged) PULSCAN_V2_LAUNCH(E, 256, true)                                                            \
-        else if (p.norm_nt == 128) PULSCAN_V2_LAUNCH(2 * E, 128, false)                                               \
-        else PULSCAN_V2_LAUNCH(E, 256, false)                                                                         \
-        norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P,        \
-                                                                  p.pitchP, redo, redo_count);                        \
-        break;                                                                                                        \
+#define PULSCAN_V2_REDO(E)                                                                                            \
+    norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P, p.pitchP, redo, \
+                                                              redo_count);
+    // key = threads per CTA · 64 + values per thread of the single-histogram kernel (B = their product)
+    switch (p.norm_nt * 64 + p.B / p.norm_nt) {
+        case 256 * 64 + 2: PULSCAN_V2_LAUNCH(2, 256, false) break;
+        case 256 * 64 + 4: PULSCAN_V2_LAUNCH(4, 256, false) break;
+        case 256 * 64 + 8: PULSCAN_V2_LAUNCH(8, 256, false) break;
+        case 256 * 64 + 16: if (p.norm_staged) PULSCAN_V2_LAUNCH(16, 256, true) else PULSCAN_V2_LAUNCH(16, 256, false) break;
+        case 256 * 64 + 32: if (p.norm_staged) PULSCAN_V2_LAUNCH(32, 256, true) else PULSCAN_V2_LAUNCH(32, 256, false) break;
+        case 128 * 64 + 32: PULSCAN_V2_LAUNCH(32, 128, false) break;
+        case 128 * 64 + 16: PULSCAN_V2_LAUNCH(16, 128, false) break;
+        case 128 * 64 + 8: PULSCAN_V2_LAUNCH(8, 128, false) break;
+        case 128 * 64 + 4: PULSCAN_V2_LAUNCH(4, 128, false) break;
+        default: return fail(PULSCAN_EINVAL, "internal: no single-histogram kernel for %d threads x %d values", p.norm_nt, p.B / p.norm_nt);
     }
     switch (p.ept_main) {
-        PULSCAN_V2_CASE(2)
-        PULSCAN_V2_CASE(4)
-        PULSCAN_V2_CASE(8)
-        PULSCAN_V2_CASE(16)
-        case 32: {
-            if (p.norm_staged) PULSCAN_V2_LAUNCH(32, 256, true) else PULSCAN_V2_LAUNCH(32, 256, false)
-            norm_power_redo_kernel<32, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P, p.pitchP, redo,
-                                                                      redo_count);
-            break;
-        }
+        case 2: PULSCAN_V2_REDO(2) break;
+        case 4: PULSCAN_V2_REDO(4) break;
+        case 8: PULSCAN_V2_REDO(8) break;
+        case 16: PULSCAN_V2_REDO(16) break;
+        case 32: PULSCAN_V2_REDO(32) break;
         default: return fail(PULSCAN_EINVAL, "internal: unsupported elements-per-thread %d", p.ept_main);
     }
+#undef PULSCAN_V2_REDO
 #undef PULSCAN_V2_LAUNCH
-#undef PULSCAN_V2_CASE
     CUDA_TRY(cudaGetLastError());
     return debug_sync("fast normalisation kernel + norm_power_redo_kernel");
 }
@@ -680,7 +683,8 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
              (long long)p.n, p.batch, p.zmax, p.C, p.B, p.sigma_thr, p.n_trials, (long long)p.pitch, p.mode ? "exhaustive" : "pruned");
     s += line;
     snprintf(line, sizeof line, "norm: %d blocks/row, main %s<EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.use_fast ? "single-histogram" : "general",
-             p.ept_main, p.nt_main, p.main_blocks_per_row, p.has_tail ? "" : " (no tail launch)");
+             p.use_fast ? p.B / p.norm_nt : p.ept_main, p.use_fast ? p.norm_nt : p.nt_main, p.main_blocks_per_row,
+             p.has_tail ? "" : " (no tail launch)");
     s += line;
     if (p.has_tail) { snprintf(line, sizeof line, "norm tail: <EPT=%d,NT=%d> x 1/row\n", p.ept_tail, p.nt_tail); s += line; }
     double evals = 0;
