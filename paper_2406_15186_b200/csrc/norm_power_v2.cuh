@@ -72,7 +72,7 @@ __device__ __forceinline__ unsigned v2_bucket_bits(float v, float scale, float o
     return __float_as_uint(__fmaf_rn(t, kV2IdxScale, 2.0f));
 }
 
-// One warp: location and spread of the block from 128 of its bins (4 per lane, spread over the block) → the bucket
+// One warp: location and spread of the block from 128 of its bins (four runs of 32 consecutive bins) → the bucket
 // map (scale, off) of both components in ctl; ctl.fail = 5 if the sample is degenerate.
 template <int B>
 __device__ __forceinline__ void v2_estimate(const float2* __restrict__ sdat, V2Ctl& ctl) {
@@ -81,7 +81,7 @@ __device__ __forceinline__ void v2_estimate(const float2* __restrict__ sdat, V2C
     float q[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const float2 s = sdat[lane * (B / 32) + k * (B / 128)];
+        const float2 s = sdat[k * (B / 4) + lane];
         const float r = s.x - pv.x, i = s.y - pv.y;
         q[0] += r; q[1] = __fmaf_rn(r, r, q[1]); q[2] += i; q[3] = __fmaf_rn(i, i, q[3]);
     }
