@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--log10-p-flag", type=float, default=0.0)
+    ap.add_argument("--z-step", type=int, default=1, help="search every z_step-th drift only (PAPER.md:L152; not the headline)")
+    ap.add_argument("--log-sampling", action="store_true", help="search z = 0, 1, 2, 4, ... only (PAPER.md:L411; not the headline)")
     return ap.parse_args()
 
 
@@ -57,8 +59,14 @@ def workload(args):
     return wl
 
 
-def config_dict(wl, n_gpus):
+def config_dict(wl, n_gpus, args=None):
+    sampling = "every width 1..zmax"
+    if args is not None and args.log_sampling:
+        sampling = "drifts z = 0, 1, 2, 4, ... (PAPER.md:L411)"
+    elif args is not None and args.z_step != 1:
+        sampling = f"every {args.z_step}-th drift (PAPER.md:L152)"
     return {
+        "widths_searched": sampling,
         "workload": f"BASELINE.json configs[{int(wl.name[3]) - 1}] ({wl.name}): {wl.batch} spectra x {wl.n_bins} complex64 bins "
                     f"per GPU, zmax={wl.zmax}, norm_block={wl.norm_block}, block_width={wl.block_width}, "
                     f"sigma_threshold={wl.sigma_threshold}",
@@ -135,19 +143,20 @@ def recorded_traffic(kernel: str, cfg: int):
         return None
 
 
-def cpu_baseline(wl, X_host_rows, budget_s=15.0):
+def cpu_baseline(wl, X_host_rows, budget_s=15.0, z_step=1, log_sampling=False):
     """The oracle, as it stands, on a bounded sample of the same spectra (host rows already in memory)."""
     import oracle
     import numpy as np
     oracle.build()
     t0 = time.perf_counter()
-    oracle.search(X_host_rows[0], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+    oracle.search(X_host_rows[0], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold, z_step=z_step, log_sampling=log_sampling)
     t1 = time.perf_counter() - t0
     extra = int(max(0, min(len(X_host_rows) - 1, round(budget_s / max(t1, 1e-3)) - 1)))
     t_all, n_sp = t1, 1
     if extra:
         t0 = time.perf_counter()
-        oracle.search(np.ascontiguousarray(X_host_rows[1:1 + extra]), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+        oracle.search(np.ascontiguousarray(X_host_rows[1:1 + extra]), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold,
+                      z_step=z_step, log_sampling=log_sampling)
         t_all += time.perf_counter() - t0
         n_sp += extra
     return {"value": n_sp * wl.n_bins / t_all, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
@@ -168,17 +177,18 @@ def run_reference(args):
     rows = X.numpy()
     per_step = 1
     for _ in range(args.warmup):
-        oracle.search(rows[0], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+        oracle.search(rows[0], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold, z_step=args.z_step, log_sampling=args.log_sampling)
     t0 = time.perf_counter()
     for i in range(args.steps):
-        oracle.search(rows[i % len(rows)], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+        oracle.search(rows[i % len(rows)], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold, z_step=args.z_step,
+                      log_sampling=args.log_sampling)
     dt = time.perf_counter() - t0
     value = args.steps * per_step * wl.n_bins / dt
     sample = f"{per_step} spectrum of the workload per step ({wl.n_bins} bins x {wl.zmax} widths)"
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(wl, args.gpus),
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(wl, args.gpus, args),
         "bin_widths_per_sec": value * wl.zmax,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -205,7 +215,7 @@ def run_ours(args):
     steps, warm = args.steps, max(args.warmup, 3)
 
     plan = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
-                        tile=args.tile, log10_p_flag=args.log10_p_flag)
+                        tile=args.tile, log10_p_flag=args.log10_p_flag, z_step=args.z_step, log_sampling=args.log_sampling)
     plan.attach(dev)
     plan.set_profiling(warm + steps)
     stream = torch.cuda.current_stream()
@@ -253,7 +263,8 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         plan_h = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
-                              tile=args.tile, log10_p_flag=args.log10_p_flag, host_staging=True)
+                              tile=args.tile, log10_p_flag=args.log10_p_flag, host_staging=True, z_step=args.z_step,
+                              log_sampling=args.log_sampling)
         plan_h.attach(dev)
         Xh = torch.empty(X.shape, dtype=X.dtype, pin_memory=True)
         Xh.copy_(X)
@@ -272,13 +283,13 @@ def run_ours(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(wl, X[: min(wl.batch, 96)].cpu().numpy())
+        cpu = cpu_baseline(wl, X[: min(wl.batch, 96)].cpu().numpy(), z_step=args.z_step, log_sampling=args.log_sampling)
 
     if rank == 0:
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic", "config": config_dict(wl, world), "bin_widths_per_sec": value * wl.zmax,
+            "data": "synthetic", "config": config_dict(wl, world, args), "bin_widths_per_sec": value * wl.zmax,
             "candidates_per_step": n_cand, "blocks_flagged_by_sweep": flagged,
             "sweep_cells_refined": int(stats[2]), "norm_blocks_redone": int(stats[1]), "clocks": clk.summary(),
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,

@@ -77,6 +77,14 @@ int pulscan_plan_set_pitch(pulscan_plan* plan, int64_t pitch_bins);
  * their width's power threshold), 1 = exhaustive sweep (every (bin, width) evaluated; the cross-check). */
 int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode);
 
+/* Which boxcar widths are SEARCHED for candidates; all widths are still summed (L152 "the user can select the step size to
+ * determine which boxcar filtered spectra are searched").  With drift z = width − 1 (R9): z_step ≥ 1 searches z = 0,
+ * z_step, 2·z_step, … (Alg. 4: remainder(z / z_step) = 0); logarithmic ≠ 0 searches z = 0, 1, 2, 4, 8, … instead
+ * (L411 "z = 1, 2, 4, 8, ... z-max", the paper's GPU default; z = 0, the unfiltered spectrum, is kept: reading R28) and
+ * ignores z_step.  Default: z_step = 1, every width (north_star).  The reduction over widths (step 6) then runs over the
+ * searched widths only; pulscan_plan_get_thresholds() reports +inf for the others. */
+int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t logarithmic);
+
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
  * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);

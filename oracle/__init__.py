@@ -62,6 +62,12 @@ def _load():
         lib.orc_sigma_from_lnp.argtypes = [ctypes.c_double]
         lib.orc_power_threshold.restype = ctypes.c_double
         lib.orc_power_threshold.argtypes = [ctypes.c_int32, ctypes.c_double]
+        lib.orc_width_searched.restype = ctypes.c_int32
+        lib.orc_width_searched.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32]
+        lib.orc_search_sampled.restype = ctypes.c_int64
+        lib.orc_search_sampled.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                           ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
+                                           ctypes.c_void_p, ctypes.c_int64]
         lib.orc_search.restype = ctypes.c_int64
         lib.orc_search.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                    ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64]
@@ -155,9 +161,15 @@ def power_threshold(w: int, sigma_threshold: float, n_trials: float = 1.0) -> fl
     return float(_load().orc_power_threshold(int(w), ln_sf(sigma_threshold) - float(np.log(n_trials))))
 
 
+def width_searched(w: int, z_step: int = 1, log_sampling: bool = False) -> bool:
+    """Is width w (drift z = w − 1) searched for candidates?  PAPER.md:L152, L411, Alg. 4; reading R28."""
+    return bool(_load().orc_width_searched(int(w), int(z_step), int(bool(log_sampling))))
+
+
 def search(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshold: float, n_trials: float = 1.0,
-           n_bins: int | None = None) -> np.ndarray:
+           n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False) -> np.ndarray:
     """The whole path.  spectra: complex64 [batch, pitch] (or 1-D); n_bins defaults to the row length.
+    z_step / log_sampling restrict the widths that are searched; default: every width.
 
     Returns a structured array (CANDIDATE_DTYPE) sorted by (spectrum, bin): at most one record per candidate block.
     """
@@ -170,7 +182,7 @@ def search(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshol
     cap = batch * ((n + C - 1) // C)
     out = np.zeros(cap, dtype=CANDIDATE_DTYPE)
     f = s.view(np.float32)
-    found = _load().orc_search(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
-                               int(norm_block), C, float(sigma_threshold), float(n_trials),
-                               out.ctypes.data_as(ctypes.c_void_p), cap)
+    found = _load().orc_search_sampled(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
+                                       int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
+                                       int(bool(log_sampling)), out.ctypes.data_as(ctypes.c_void_p), cap)
     return out[: int(found)].copy()

@@ -190,8 +190,31 @@ double orc_power_threshold(int32_t w, double lnp_target) {
  *        the smallest such w on exact ties                                                            (R13)
  *   emit (b, I(c,w*), w*, M(c,w*), σ) iff ln p_adj <= ln sf(sigma_threshold)  (σ >= threshold)          (R17)
  */
+int64_t orc_search_sampled(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                           int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                           orc_candidate* out, int64_t cap);
+
 int64_t orc_search(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                    int64_t C, double sigma_threshold, double n_trials, orc_candidate* out, int64_t cap) {
+    return orc_search_sampled(spectra, batch, n, pitch, zmax, B, C, sigma_threshold, n_trials, 1, 0, out, cap);
+}
+
+/* Which boxcar widths are SEARCHED for candidates (all are computed): "the user can select the step size
+ * to determine which boxcar filtered spectra are searched"; Alg. 4 L693-695 searches drift z (from 0) when
+ * remainder(z / z_step) = 0, "this condition on z can be replaced with a check for if the current z is a power of 2
+ * for logarithmic sampling"; L411 "only search logarithmically spaced (i.e. z = 1, 2, 4, 8, ... z-max) boxcar filter
+ * widths".  The width is w = z + 1 (R9).  Reading R28: z = 0 (the unfiltered spectrum) is searched in both modes, as
+ * Alg. 4's loop starts at z = 0 and remainder(0 / z_step) = 0. */
+int32_t orc_width_searched(int32_t w, int32_t z_step, int32_t log_sampling) {
+    int32_t z = w - 1;
+    if (log_sampling) return z == 0 || (z & (z - 1)) == 0;
+    return z % z_step == 0;
+}
+
+/* orc_search restricted to the searched widths: the reduction over widths (R13) runs over those only. */
+int64_t orc_search_sampled(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                           int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                           orc_candidate* out, int64_t cap) {
     int64_t nblk = (n + C - 1) / C;
     double ln_trials = log(n_trials);
     double lnp_thr = orc_ln_sf(sigma_threshold);
@@ -212,6 +235,7 @@ int64_t orc_search(const float* spectra, int64_t batch, int64_t n, int64_t pitch
                 int32_t best_w = 0;
                 for (int32_t w = 1; w <= zmax; ++w) {
                     if (I[w - 1] < 0) continue; /* no window of this width starts in the block */
+                    if (!orc_width_searched(w, z_step, log_sampling)) continue;
                     double lnp = orc_ln_q(w, M[w - 1]) + ln_trials;
                     if (lnp > 0.0) lnp = 0.0;
                     if (lnp < best_lnp) { best_lnp = lnp; best_w = w; } /* strict: smallest w on ties */

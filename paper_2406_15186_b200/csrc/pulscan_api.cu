@@ -63,6 +63,7 @@ struct pulscan_plan {
     double sigma_thr = 0, n_trials = 1.0;
     int64_t pitch = 0;
     int32_t mode = 0;
+    int32_t z_step = 1, log_sampling = 0;   // which widths are searched (all are summed): Alg. 4
     int32_t tile_user = 0;
     double log10_p_flag = -3.0;
     bool host_staging = false;
@@ -131,9 +132,15 @@ int derive(pulscan_plan& p) {
     const double lnp_target = p.lnp_thr - p.ln_trials; // ln p_adj ≤ lnp_thr ⇔ ln p ≤ lnp_thr − ln N  (R15, R17)
     p.T.resize(p.zmax);
     p.Tp.resize(p.zmax);
+    // A width that is not searched gets an infinite threshold: no cover, window or block maximum of it can pass, so every
+    // later stage skips it without knowing about the sampling.
+    auto searched = [&](int w) {
+        const int z = w - 1;
+        return p.log_sampling ? (z == 0 || (z & (z - 1)) == 0) : (z % p.z_step == 0);
+    };
     for (int w = 1; w <= p.zmax; ++w) {
-        p.T[w - 1] = power_threshold(w, lnp_target);
-        p.Tp[w - 1] = conservative_threshold(p.T[w - 1], w);
+        p.T[w - 1] = searched(w) ? power_threshold(w, lnp_target) : INFINITY;
+        p.Tp[w - 1] = searched(w) ? conservative_threshold(p.T[w - 1], w) : INFINITY;
     }
 
     // ---- sweep tile
@@ -154,7 +161,8 @@ int derive(pulscan_plan& p) {
             for (int lg = 3; lg <= lg_cap; ++lg) {
                 const int g = 1 << lg, Lc = w + 2 * g - 2;
                 if ((tile >> lg) % kSweepR != 0) break;
-                if (l10 >= 0.0 || ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
+                if (l10 >= 0.0 || !std::isfinite(p.T[w - 1]) ||
+                    ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
             }
             lgw[w] = best;
         }
@@ -227,8 +235,10 @@ int derive(pulscan_plan& p) {
         for (int m = lv.m_start; m < lv.m_start + 4 * lv.nsteps; ++m) {
             if (m < lv.m_lo || m > lv.m_hi) { p.tau.push_back(INFINITY); continue; }
             const int wmin = (g == 1) ? m : (m == 1 ? 1 : (m - 2) * g + 2);
-            const int wq = std::min(std::max(lv.wlo, wmin), lv.whi);
-            p.tau.push_back(conservative_threshold(p.T[wq - 1], m * g));
+            // the lowest threshold among the level's searched widths this cover can hold (T_w grows with w)
+            int wq = std::min(std::max(lv.wlo, wmin), lv.whi);
+            while (wq <= lv.whi && !std::isfinite(p.T[wq - 1])) ++wq;
+            p.tau.push_back(wq <= lv.whi ? conservative_threshold(p.T[wq - 1], m * g) : INFINITY);
         }
         sp.lv[l] = lv;
     }
@@ -501,6 +511,14 @@ int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (mode != 0 && mode != 1) return fail(PULSCAN_EINVAL, "mode must be 0 (pruned) or 1 (exhaustive)");
     plan->mode = mode;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t logarithmic) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (z_step < 1) return fail(PULSCAN_EINVAL, "z_step = %d < 1", z_step);
+    plan->z_step = z_step; plan->log_sampling = logarithmic != 0;
+    plan->dirty = true; release_device(*plan);
     return PULSCAN_OK;
 }
 

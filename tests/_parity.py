@@ -23,8 +23,10 @@ def gpu_search(spectra: torch.Tensor, zmax, norm_block, block_width, thr, n_bins
     return rec, stats
 
 
-def oracle_search(orc, spectra: torch.Tensor, zmax, norm_block, block_width, thr, n_bins=None, n_trials=1.0):
-    return orc.search(spectra.cpu().numpy(), zmax, norm_block, block_width, thr, n_trials=n_trials, n_bins=n_bins)
+def oracle_search(orc, spectra: torch.Tensor, zmax, norm_block, block_width, thr, n_bins=None, n_trials=1.0, z_step=1,
+                  log_sampling=False):
+    return orc.search(spectra.cpu().numpy(), zmax, norm_block, block_width, thr, n_trials=n_trials, n_bins=n_bins,
+                      z_step=z_step, log_sampling=log_sampling)
 
 
 def assert_same_candidates(gpu, ora, context=""):

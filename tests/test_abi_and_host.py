@@ -67,6 +67,7 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_mode(p.handle, 7) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 1000, 0.0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 2048, -1.0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_width_sampling(p.handle, 0, 0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_cell_capacity(p.handle, -1) == binding.PULSCAN_EINVAL
     ws0 = p.workspace_bytes
     assert lib.pulscan_plan_set_cell_capacity(p.handle, 1 << 20) == binding.PULSCAN_OK
@@ -149,3 +150,15 @@ def test_pruning_bound_is_an_upper_bound_property():
             k0, k1 = i // g, (i + w - 1) // g
             lo, hi = k0 * g, min((k1 + 1) * g, 4096)
             assert pre[hi] - pre[lo] >= pre[i + w] - pre[i] - 1e-9
+
+
+def test_width_sampling_masks_thresholds(binding):
+    full = binding.Plan(50000, 1, 40, 100, 6.0).thresholds()
+    assert np.all(np.isfinite(full))
+    log = binding.Plan(50000, 1, 40, 100, 6.0, log_sampling=True).thresholds()
+    kept = [1, 2, 3, 5, 9, 17, 33]                          # z = width − 1 ∈ {0, 1, 2, 4, 8, 16, 32} (R28)
+    for w in range(1, 41):
+        assert (log[w - 1] == full[w - 1]) if w in kept else np.isinf(log[w - 1])
+    step = binding.Plan(50000, 1, 40, 100, 6.0, z_step=5).thresholds()
+    assert [w for w in range(1, 41) if np.isfinite(step[w - 1])] == [1, 6, 11, 16, 21, 26, 31, 36]   # Alg. 4
+    assert "sweep level" in binding.Plan(50000, 1, 40, 100, 6.0, log_sampling=True).describe()

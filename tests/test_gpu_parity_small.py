@@ -121,6 +121,21 @@ def test_tuning_never_changes_results(orc, tile, lpf):
     assert np.array_equal(ref, got)
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("z_step,log_sampling", [(4, False), (13, False), (1, True)])
+@pytest.mark.parametrize("n,batch,zmax,B,C,thr", [(20001, 2, 40, 2048, 100, 4.0), (9000, 2, 200, 4096, 200, 4.0),
+                                                  (30011, 1, 300, 8192, 1200, 4.0)])
+def test_width_sampling_matches_oracle(orc, n, batch, zmax, B, C, thr, z_step, log_sampling, mode):
+    spec = noise_spectra(batch, n, seed=n + zmax)
+    bump(spec, 0, n // 3, 6, 3.0)
+    bump(spec, batch - 1, n // 2, min(zmax, 60), 1.8)
+    gpu, _ = gpu_search(spec, zmax, B, C, thr, mode=mode, z_step=z_step, log_sampling=log_sampling)
+    ora = oracle_search(orc, spec, zmax, B, C, thr, z_step=z_step, log_sampling=log_sampling)
+    assert len(ora) > 0
+    assert all(orc.width_searched(int(w), z_step, log_sampling) for w in gpu["width"])
+    assert_same_candidates(gpu, ora, f"n={n} zmax={zmax} z_step={z_step} log={log_sampling} mode={mode}")
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)

@@ -6,7 +6,7 @@ from scipy import special, stats
 from paper_2406_15186_b200 import synth
 
 
-def library_route(spec, zmax, B, C, thr, n_trials=1.0):
+def library_route(spec, zmax, B, C, thr, n_trials=1.0, widths=None):
     """The same path through library routines only (numpy.median, scipy MAD, cumsum differences, chi2.logsf,
     norm.isf) — slow, tiny inputs."""
     n = spec.size
@@ -24,7 +24,7 @@ def library_route(spec, zmax, B, C, thr, n_trials=1.0):
     for c in range((n + C - 1) // C):
         lo, hi = c * C, min((c + 1) * C, n)
         best = None
-        for w in range(1, zmax + 1):
+        for w in (range(1, zmax + 1) if widths is None else widths):
             i = np.arange(lo, min(hi, n - w + 1))
             if i.size == 0:
                 continue
@@ -53,6 +53,38 @@ def test_search_matches_library_route(orc, seed, n, zmax, B, C, thr):
         assert g["sigma"] == pytest.approx(r[3], abs=1e-7)
     # sorted by bin, at most one per block, bin inside its block
     assert np.all(np.diff(got["bin"] // C) > 0)
+
+
+def test_searched_width_sets_follow_the_paper(orc):
+    # L411: "only search logarithmically spaced (i.e. z = 1, 2, 4, 8, ... z-max)"; width = z + 1 (R9); z = 0 kept (R28)
+    assert [w for w in range(1, 41) if orc.width_searched(w, log_sampling=True)] == [1, 2, 3, 5, 9, 17, 33]
+    # Alg. 4: z from 0, searched when remainder(z / z_step) = 0
+    assert [w for w in range(1, 15) if orc.width_searched(w, z_step=4)] == [1, 5, 9, 13]
+    assert all(orc.width_searched(w) for w in range(1, 100))                       # default: every width (north_star)
+    assert [w for w in range(1, 12) if orc.width_searched(w, z_step=3, log_sampling=True)] == [1, 2, 3, 5, 9]  # log wins
+
+
+@pytest.mark.parametrize("z_step,log_sampling", [(1, False), (3, False), (7, False), (1, True)])
+def test_sampled_search_matches_library_route(orc, z_step, log_sampling):
+    n, zmax, B, C, thr = 769, 24, 256, 32, 2.0
+    rng = np.random.default_rng(11)
+    spec = (rng.normal(0, 30, n) + 1j * rng.normal(0, 30, n)).astype(np.complex64)
+    spec[200:212] *= 2.5
+    spec[500:503] *= 4.0
+    if log_sampling:
+        widths = [w for w in range(1, zmax + 1) if w == 1 or (w - 1) & (w - 2) == 0]     # z = w − 1 ∈ {0} ∪ powers of two
+    else:
+        widths = [w for w in range(1, zmax + 1) if (w - 1) % z_step == 0]
+    got = orc.search(spec, zmax, B, C, thr, z_step=z_step, log_sampling=log_sampling)
+    ref = library_route(spec, zmax, B, C, thr, widths=widths)
+    assert len(got) == len(ref) > 0
+    assert set(got["width"].tolist()) <= set(widths)
+    for g, r in zip(got, ref):
+        assert (g["bin"], g["width"]) == (r[0], r[1])
+        assert g["power"] == pytest.approx(r[2], rel=1e-11)
+        assert g["sigma"] == pytest.approx(r[3], abs=1e-7)
+    if z_step == 1 and not log_sampling:
+        assert np.array_equal(got, orc.search(spec, zmax, B, C, thr))
 
 
 def test_bonferroni_trials_shift(orc):
