@@ -164,7 +164,7 @@ int derive(pulscan_plan& p) {
                 if (l10 >= 0.0 || !std::isfinite(p.T[w - 1]) ||
                     ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
             }
-            lgw[w] = best;
+            lgw[w] = (w > 1 && !std::isfinite(p.T[w - 1])) ? lgw[w - 1] : best;   // a width that is not searched follows its neighbour
         }
         for (int w = p.zmax - 1; w >= 1; --w) lgw[w] = std::min(lgw[w], lgw[w + 1]);
         lvls.clear();
@@ -228,18 +228,33 @@ int derive(pulscan_plan& p) {
             ++sp.narr;
         }
         lv.pg_off = sp.arr_off[a];
-        lv.wt_off = task;
-        task += lv.nwt;
         lv.tau_off = (int)p.tau.size();
         const int g = 1 << lv.lg;
         for (int m = lv.m_start; m < lv.m_start + 4 * lv.nsteps; ++m) {
             if (m < lv.m_lo || m > lv.m_hi) { p.tau.push_back(INFINITY); continue; }
             const int wmin = (g == 1) ? m : (m == 1 ? 1 : (m - 2) * g + 2);
-            // the lowest threshold among the level's searched widths this cover can hold (T_w grows with w)
+            // the lowest threshold among the level's searched widths whose windows have a cover of exactly m groups
+            // (widths wmin … m·g; T_w grows with w); +inf if there is none
+            const int wtop = std::min(lv.whi, m * g);
             int wq = std::min(std::max(lv.wlo, wmin), lv.whi);
-            while (wq <= lv.whi && !std::isfinite(p.T[wq - 1])) ++wq;
-            p.tau.push_back(wq <= lv.whi ? conservative_threshold(p.T[wq - 1], m * g) : INFINITY);
+            while (wq <= wtop && !std::isfinite(p.T[wq - 1])) ++wq;
+            p.tau.push_back(wq <= wtop ? conservative_threshold(p.T[wq - 1], m * g) : INFINITY);
         }
+        // with sparse width sampling whole 4-wide steps can be dead (τ = +inf): trim them off both ends
+        {
+            auto dead = [&](int st) {
+                for (int q = 0; q < 4; ++q)
+                    if (std::isfinite(p.tau[lv.tau_off + 4 * st + q])) return false;
+                return true;
+            };
+            int first = 0, last = lv.nsteps - 1;
+            while (first <= last && dead(first)) ++first;
+            while (last >= first && dead(last)) --last;
+            lv.m_start += 4 * first; lv.tau_off += 4 * first; lv.nsteps = last - first + 1;
+            if (lv.nsteps == 0) lv.nwt = 0;
+        }
+        lv.wt_off = task;
+        task += lv.nwt;
         sp.lv[l] = lv;
     }
     sp.ntasks = task;
