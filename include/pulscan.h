@@ -85,6 +85,11 @@ int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode);
  * searched widths only; pulscan_plan_get_thresholds() reports +inf for the others. */
 int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t logarithmic);
 
+/* "Pulscan R-Block" (L222-226 §2.4): save only the block index of a candidate, "an approximate frequency location".
+ * enable ≠ 0: a record's `bin` is the first bin of its candidate block, block index × block_width (Table 3:
+ * 360448 = 11 × 32768); width, power and sigma are unchanged.  Default 0: the exact first bin of the window. */
+int pulscan_plan_set_r_block(pulscan_plan* plan, int32_t enable);
+
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
  * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);

@@ -68,6 +68,10 @@ def _load():
         lib.orc_search_sampled.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                            ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
                                            ctypes.c_void_p, ctypes.c_int64]
+        lib.orc_search_ex.restype = ctypes.c_int64
+        lib.orc_search_ex.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                      ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
+                                      ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64]
         lib.orc_search.restype = ctypes.c_int64
         lib.orc_search.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                    ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64]
@@ -167,9 +171,10 @@ def width_searched(w: int, z_step: int = 1, log_sampling: bool = False) -> bool:
 
 
 def search(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshold: float, n_trials: float = 1.0,
-           n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False) -> np.ndarray:
+           n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False, r_block: bool = False) -> np.ndarray:
     """The whole path.  spectra: complex64 [batch, pitch] (or 1-D); n_bins defaults to the row length.
     z_step / log_sampling restrict the widths that are searched; default: every width.
+    r_block: report the candidate block's first bin instead of the exact bin ("Pulscan R-Block").
 
     Returns a structured array (CANDIDATE_DTYPE) sorted by (spectrum, bin): at most one record per candidate block.
     """
@@ -182,7 +187,7 @@ def search(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshol
     cap = batch * ((n + C - 1) // C)
     out = np.zeros(cap, dtype=CANDIDATE_DTYPE)
     f = s.view(np.float32)
-    found = _load().orc_search_sampled(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
-                                       int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
-                                       int(bool(log_sampling)), out.ctypes.data_as(ctypes.c_void_p), cap)
+    found = _load().orc_search_ex(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
+                                  int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
+                                  int(bool(log_sampling)), int(bool(r_block)), out.ctypes.data_as(ctypes.c_void_p), cap)
     return out[: int(found)].copy()

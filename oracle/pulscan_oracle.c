@@ -193,6 +193,9 @@ double orc_power_threshold(int32_t w, double lnp_target) {
 int64_t orc_search_sampled(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                            int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
                            orc_candidate* out, int64_t cap);
+int64_t orc_search_ex(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B, int64_t C,
+                      double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling, int32_t r_block,
+                      orc_candidate* out, int64_t cap);
 
 int64_t orc_search(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                    int64_t C, double sigma_threshold, double n_trials, orc_candidate* out, int64_t cap) {
@@ -215,6 +218,16 @@ int32_t orc_width_searched(int32_t w, int32_t z_step, int32_t log_sampling) {
 int64_t orc_search_sampled(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                            int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
                            orc_candidate* out, int64_t cap) {
+    return orc_search_ex(spectra, batch, n, pitch, zmax, B, C, sigma_threshold, n_trials, z_step, log_sampling, 0, out, cap);
+}
+
+/* ... and, with r_block != 0, "Pulscan R-Block" (§2.4): "simply saving the block index (an approximate
+ * frequency location) of candidates rather than the exact r-bin they came from".  The record's bin is then the first bin
+ * of the candidate block, block index × block width (Table 3: R-Block r = 360448 = 11 × 32768 against the exact
+ * 364318); width, power and significance are unchanged. */
+int64_t orc_search_ex(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B, int64_t C,
+                      double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling, int32_t r_block,
+                      orc_candidate* out, int64_t cap) {
     int64_t nblk = (n + C - 1) / C;
     double ln_trials = log(n_trials);
     double lnp_thr = orc_ln_sf(sigma_threshold);
@@ -245,7 +258,7 @@ int64_t orc_search_sampled(const float* spectra, int64_t batch, int64_t n, int64
                 r.spectrum = -1;
                 if (best_w > 0 && best_lnp <= lnp_thr) {
                     r.spectrum = (int32_t)b;
-                    r.bin = (int32_t)I[best_w - 1];
+                    r.bin = r_block ? (int32_t)(c * C) : (int32_t)I[best_w - 1];
                     r.width = best_w;
                     r.power = M[best_w - 1];
                     r.lnp = best_lnp;

@@ -33,7 +33,7 @@ struct ExactSmemHdr {
 
 __global__ void __launch_bounds__(kExactThreads)
 block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, int zmax, int C, long long nblk,
-                   const double* __restrict__ T_g, double ln_trials, double lnp_thr,
+                   const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block,
                    const unsigned* __restrict__ flagged, const unsigned* __restrict__ counters,
                    pulscan_candidate* __restrict__ out, unsigned* __restrict__ out_count) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -128,7 +128,7 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
             if (my_w > 0 && my_lnp <= lnp_thr) {
                 pulscan_candidate r;
                 r.spectrum = (int32_t)row;
-                r.bin = (int32_t)(lo + my_i);
+                r.bin = r_block ? (int32_t)lo : (int32_t)(lo + my_i);   // R-Block: the block index × block width (L222-226)
                 r.width = my_w;
                 r.power = (float)my_s;
                 r.sigma = (float)sigma_from_lnp(my_lnp);

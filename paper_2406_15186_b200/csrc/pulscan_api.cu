@@ -63,6 +63,7 @@ struct pulscan_plan {
     double sigma_thr = 0, n_trials = 1.0;
     int64_t pitch = 0;
     int32_t mode = 0;
+    int32_t r_block = 0;                     // report the candidate block's first bin instead of the exact bin (L222-226)
     int32_t z_step = 1, log_sampling = 0;   // which widths are searched (all are summed): Alg. 4
     int32_t tile_user = 0;
     double log10_p_flag = -3.0;
@@ -537,6 +538,12 @@ int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t 
     return PULSCAN_OK;
 }
 
+int pulscan_plan_set_r_block(pulscan_plan* plan, int32_t enable) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    plan->r_block = enable != 0;
+    return PULSCAN_OK;
+}
+
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (tile_bins != 0 && (tile_bins < 1024 || tile_bins > 16384 || tile_bins % 512 != 0))
@@ -668,7 +675,7 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
     const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
     block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
-                                                                   p.lnp_thr, d_flagged, d_counters, d_candidates, d_count);
+                                                                   p.lnp_thr, p.r_block, d_flagged, d_counters, d_candidates, d_count);
     CUDA_TRY(cudaGetLastError());
     if (ev) CUDA_TRY(cudaEventRecord(ev[4], st));
     return debug_sync("block_exact_kernel");

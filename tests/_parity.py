@@ -24,9 +24,9 @@ def gpu_search(spectra: torch.Tensor, zmax, norm_block, block_width, thr, n_bins
 
 
 def oracle_search(orc, spectra: torch.Tensor, zmax, norm_block, block_width, thr, n_bins=None, n_trials=1.0, z_step=1,
-                  log_sampling=False):
+                  log_sampling=False, r_block=False):
     return orc.search(spectra.cpu().numpy(), zmax, norm_block, block_width, thr, n_trials=n_trials, n_bins=n_bins,
-                      z_step=z_step, log_sampling=log_sampling)
+                      z_step=z_step, log_sampling=log_sampling, r_block=r_block)
 
 
 def assert_same_candidates(gpu, ora, context=""):

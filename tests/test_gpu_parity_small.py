@@ -136,6 +136,17 @@ def test_width_sampling_matches_oracle(orc, n, batch, zmax, B, C, thr, z_step, l
     assert_same_candidates(gpu, ora, f"n={n} zmax={zmax} z_step={z_step} log={log_sampling} mode={mode}")
 
 
+def test_r_block_matches_oracle(orc):
+    spec = noise_spectra(2, 20001, seed=4242)
+    bump(spec, 1, 7777, 20, 2.5)
+    gpu, _ = gpu_search(spec, 48, 2048, 100, 4.0, r_block=True, log_sampling=True)
+    ora = oracle_search(orc, spec, 48, 2048, 100, 4.0, r_block=True, log_sampling=True)
+    assert len(ora) > 0 and np.all(ora["bin"] % 100 == 0)
+    assert_same_candidates(gpu, ora, "R-Block + log sampling")
+    exact, _ = gpu_search(spec, 48, 2048, 100, 4.0, log_sampling=True)
+    assert np.array_equal(gpu["bin"], exact["bin"] // 100 * 100) and np.array_equal(gpu["sigma"], exact["sigma"])
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)

@@ -87,6 +87,21 @@ def test_sampled_search_matches_library_route(orc, z_step, log_sampling):
         assert np.array_equal(got, orc.search(spec, zmax, B, C, thr))
 
 
+def test_r_block_reports_block_index_times_width(orc):
+    # L222-226: "simply saving the block index"; Table 3: R-Block r = 360448 = 11 x 32768 for the exact r = 364318
+    assert 364318 // 32768 * 32768 == 360448
+    n, zmax, B, C, thr = 2049, 16, 512, 100, 2.5
+    rng = np.random.default_rng(5)
+    spec = (rng.normal(0, 30, n) + 1j * rng.normal(0, 30, n)).astype(np.complex64)
+    spec[700:706] *= 4.0
+    exact = orc.search(spec, zmax, B, C, thr)
+    approx = orc.search(spec, zmax, B, C, thr, r_block=True)
+    assert len(exact) == len(approx) > 0
+    assert np.array_equal(approx["bin"], exact["bin"] // C * C)
+    for f in ("spectrum", "width", "power", "sigma"):
+        assert np.array_equal(approx[f], exact[f])
+
+
 def test_bonferroni_trials_shift(orc):
     rng = np.random.default_rng(4)
     spec = (rng.normal(0, 1, 600) + 1j * rng.normal(0, 1, 600)).astype(np.complex64)
