@@ -19,7 +19,7 @@ _SRC = _HERE / "pulscan_oracle.c"
 _LIB = _HERE / "liboracle.so"
 
 CANDIDATE_DTYPE = np.dtype(
-    [("spectrum", "<i4"), ("bin", "<i4"), ("width", "<i4"), ("pad_", "<i4"), ("power", "<f8"), ("sigma", "<f8"),
+    [("spectrum", "<i4"), ("bin", "<i4"), ("width", "<i4"), ("numharm", "<i4"), ("power", "<f8"), ("sigma", "<f8"),
      ("lnp", "<f8")]
 )
 
@@ -72,6 +72,12 @@ def _load():
         lib.orc_search_ex.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                       ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
                                       ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64]
+        lib.orc_harmonic_sum.restype = ctypes.c_int64
+        lib.orc_harmonic_sum.argtypes = [c_dp, ctypes.c_int64, ctypes.c_int32, c_dp]
+        lib.orc_search_harmonics.restype = ctypes.c_int64
+        lib.orc_search_harmonics.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                             ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
+                                             ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64]
         lib.orc_search.restype = ctypes.c_int64
         lib.orc_search.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                    ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64]
@@ -190,4 +196,34 @@ def search(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshol
     found = _load().orc_search_ex(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
                                   int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
                                   int(bool(log_sampling)), int(bool(r_block)), out.ctypes.data_as(ctypes.c_void_p), cap)
+    return out[: int(found)].copy()
+
+
+def harmonic_sum(P, H: int) -> np.ndarray:
+    """Y_H(r) = sum over h = 1..H of the h adjacent powers starting at h·r (§2.3); floor(n/H) bins (R29)."""
+    P = np.ascontiguousarray(P, dtype=np.float64)
+    Y = np.empty(P.size // int(H), dtype=np.float64)
+    nH = _load().orc_harmonic_sum(_dp(P), P.size, int(H), _dp(Y))
+    assert nH == Y.size
+    return Y
+
+
+def search_harmonics(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshold: float, numharm: int,
+                     n_trials: float = 1.0, n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False,
+                     r_block: bool = False) -> np.ndarray:
+    """The search on every harmonic-summed spectrum Y_1 … Y_numharm (§2.3): records carry `numharm`; ordered by
+    (numharm, spectrum, bin); at most one per candidate block of each summed spectrum."""
+    s = np.ascontiguousarray(spectra, dtype=np.complex64)
+    if s.ndim == 1:
+        s = s[None, :]
+    batch, pitch = s.shape
+    n = pitch if n_bins is None else int(n_bins)
+    C = int(block_width)
+    cap = sum(batch * ((n // H + C - 1) // C) for H in range(1, int(numharm) + 1))
+    out = np.zeros(cap, dtype=CANDIDATE_DTYPE)
+    f = s.view(np.float32)
+    found = _load().orc_search_harmonics(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
+                                         int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
+                                         int(bool(log_sampling)), int(bool(r_block)), int(numharm),
+                                         out.ctypes.data_as(ctypes.c_void_p), cap)
     return out[: int(found)].copy()

@@ -29,7 +29,7 @@ typedef struct {
     int32_t spectrum; /* index in the batch                                   */
     int32_t bin;      /* first bin of the window (R10)                        */
     int32_t width;    /* boxcar width w in [1, zmax] (R9)                     */
-    int32_t pad_;
+    int32_t numharm;  /* harmonics summed, H (1 for the plain search); §2.3       */
     double power;     /* S(bin, width), mean-1 units (R2)                     */
     double sigma;     /* Gaussian-equivalent significance (R16)               */
     double lnp;       /* ln of the (Bonferroni-adjusted) p-value              */
@@ -260,6 +260,7 @@ int64_t orc_search_ex(const float* spectra, int64_t batch, int64_t n, int64_t pi
                     r.spectrum = (int32_t)b;
                     r.bin = r_block ? (int32_t)(c * C) : (int32_t)I[best_w - 1];
                     r.width = best_w;
+                    r.numharm = 1;
                     r.power = M[best_w - 1];
                     r.lnp = best_lnp;
                     r.sigma = orc_sigma_from_lnp(best_lnp);
@@ -275,6 +276,89 @@ int64_t orc_search_ex(const float* spectra, int64_t batch, int64_t n, int64_t pi
         }
     }
     free(P); free(blockbest);
+    return found;
+}
+
+/* Harmonic sum by decimation (§2.3).  "Summing adjacent non-overlapping pairs, triples, quartets,
+ * etc. of frequency magnitudes to produce a magnitude spectra decimated by factors of 2, 3, 4": D_h(r) = Σ_{j<h} P[h·r + j].
+ * "We then sum the overlapping sections of each decimated spectra (aligned so the 0th bin of each spectrum is summed) and
+ * discard the non-overlapping parts": Y_H(r) = Σ_{h=1}^{H} D_h(r) for r in [0, floor(n/H)), which in noise is χ² with
+ * Σ 2h = H(H+1) degrees of freedom (L214-216) — in the mean-1 units used here (R2) a Gamma variate of shape H(H+1)/2.
+ * Reading R29: only complete groups count, so Y_H has floor(n/H) bins.  Returns that length; Y must hold it. */
+int64_t orc_harmonic_sum(const double* P, int64_t n, int32_t H, double* Y) {
+    int64_t nH = n / H;
+    for (int64_t r = 0; r < nH; ++r) {
+        double y = 0.0;
+        for (int32_t h = 1; h <= H; ++h)
+            for (int32_t j = 0; j < h; ++j) y += P[(int64_t)h * r + j];
+        Y[r] = y;
+    }
+    return nH;
+}
+
+/* The search with harmonic summing: for H = 1..numharm the summed spectrum Y_H is boxcar-filtered "as previously
+ * described", the output being χ² with H(H+1)(z+1) degrees of freedom (L220): ln p = ln Q(w·H(H+1)/2, S) in mean-1
+ * units.  Candidate blocks, widths (zmax, sampling), the reduction over widths (R13), the threshold and R-Block are as in
+ * orc_search_ex, applied to each Y_H on its own (bins are those of Y_H, i.e. of the fundamental); a width needs
+ * w < floor(n/H) to exist.  Records carry numharm = H and come out ordered by (H, spectrum, bin).  Normalisation happens
+ * once, on the full-resolution spectrum, before the decimation (Table 4's kernel order L571-578). */
+int64_t orc_search_harmonics(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                             int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                             int32_t r_block, int32_t numharm, orc_candidate* out, int64_t cap) {
+    double ln_trials = log(n_trials);
+    double lnp_thr = orc_ln_sf(sigma_threshold);
+    double* P = (double*)malloc((size_t)n * sizeof(double));
+    double* Y = (double*)malloc((size_t)n * sizeof(double));
+    int64_t found = 0;
+    for (int32_t H = 1; H <= numharm; ++H) {
+        int32_t kappa = H * (H + 1) / 2;
+        for (int64_t b = 0; b < batch; ++b) {
+            orc_normalise_power(spectra + 2 * b * pitch, n, B, P);
+            int64_t nH = orc_harmonic_sum(P, n, H, Y);
+            int64_t nblk = (nH + C - 1) / C;
+            orc_candidate* blockbest = (orc_candidate*)malloc((size_t)nblk * sizeof(orc_candidate));
+#pragma omp parallel
+            {
+                double* sums = (double*)malloc((size_t)C * sizeof(double));
+                double* M = (double*)malloc((size_t)zmax * sizeof(double));
+                int64_t* I = (int64_t*)malloc((size_t)zmax * sizeof(int64_t));
+#pragma omp for schedule(dynamic, 16)
+                for (int64_t c = 0; c < nblk; ++c) {
+                    orc_block_maxima(Y, nH, zmax, C, c, sums, M, I);
+                    double best_lnp = INFINITY;
+                    int32_t best_w = 0;
+                    for (int32_t w = 1; w <= zmax; ++w) {
+                        if (I[w - 1] < 0) continue;
+                        if (!orc_width_searched(w, z_step, log_sampling)) continue;
+                        double lnp = orc_ln_q(w * kappa, M[w - 1]) + ln_trials;
+                        if (lnp > 0.0) lnp = 0.0;
+                        if (lnp < best_lnp) { best_lnp = lnp; best_w = w; }
+                    }
+                    orc_candidate r;
+                    memset(&r, 0, sizeof r);
+                    r.spectrum = -1;
+                    if (best_w > 0 && best_lnp <= lnp_thr) {
+                        r.spectrum = (int32_t)b;
+                        r.bin = r_block ? (int32_t)(c * C) : (int32_t)I[best_w - 1];
+                        r.width = best_w;
+                        r.numharm = H;
+                        r.power = M[best_w - 1];
+                        r.lnp = best_lnp;
+                        r.sigma = orc_sigma_from_lnp(best_lnp);
+                    }
+                    blockbest[c] = r;
+                }
+                free(sums); free(M); free(I);
+            }
+            for (int64_t c = 0; c < nblk; ++c) {
+                if (blockbest[c].spectrum < 0) continue;
+                if (found < cap) out[found] = blockbest[c];
+                ++found;
+            }
+            free(blockbest);
+        }
+    }
+    free(P); free(Y);
     return found;
 }
 
