@@ -55,6 +55,19 @@ typedef struct {
     float sigma;
 } pulscan_candidate;
 
+/* One candidate of the harmonic-summed search (pulscan_search_harmonics): 24 bytes, no padding.  `numharm` = H, the number
+ * of harmonics summed into the spectrum Y_H the candidate was found in (1 = the plain power spectrum); `bin` is a bin of
+ * Y_H, i.e. of the fundamental (L218 "aligned so the 0th bin of each spectrum is summed"); `power` = the boxcar sum of Y_H
+ * in mean-1 units (mean H(H+1)/2 per bin in noise). */
+typedef struct {
+    int32_t spectrum;
+    int32_t bin;
+    int32_t width;
+    int32_t numharm;
+    float power;
+    float sigma;
+} pulscan_hcandidate;
+
 /* Create a plan for `batch` spectra of `n_bins` complex64 bins each, boxcar widths 1..zmax, candidate blocks of
  * `block_width` start bins (Alg. 4's chunk_size; L224 "block width is a user defined parameter") and a
  * Gaussian-σ threshold (L361).  Host-only: touches no CUDA device.  Defaults: norm_block = next power of two
@@ -89,6 +102,18 @@ int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t 
  * enable ≠ 0: a record's `bin` is the first bin of its candidate block, block index × block_width (Table 3:
  * 360448 = 11 × 32768); width, power and sigma are unchanged.  Default 0: the exact first bin of the window. */
 int pulscan_plan_set_r_block(pulscan_plan* plan, int32_t enable);
+
+/* Harmonic sum (L201-220 §2.3; `-numharm`): numharm ∈ [1, 4].  pulscan_search_harmonics() then also searches the summed
+ * spectra Y_H(r) = Σ_{h≤H} Σ_{j<h} P[h·r + j], r < floor(n_bins/H) (R29), H = 2..numharm, each "boxcar filtered as
+ * previously described" with χ² of H(H+1)·width degrees of freedom (L220).  Needs zmax < floor(n_bins/numharm).  Changes
+ * pulscan_plan_workspace_bytes().  Default 1.  pulscan_search() is not affected. */
+int pulscan_plan_set_harmonics(pulscan_plan* plan, int32_t numharm);
+/* Capacity the caller must give d_hcandidates: Σ_{H ≤ numharm} batch · ceil(floor(n_bins/H) / block_width) records. */
+int64_t pulscan_plan_max_hcandidates(const pulscan_plan* plan);
+/* pulscan_search on Y_1 (the power spectrum) … Y_numharm: same contract as pulscan_search (device pointers, asynchronous, no
+ * allocation); at most one record per candidate block of each Y_H; *d_count is zeroed first and ends as the total. */
+int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_hcandidate* d_hcandidates, uint32_t* d_count,
+                             void* cuda_stream);
 
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
  * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */

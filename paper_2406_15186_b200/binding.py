@@ -19,6 +19,9 @@ PULSCAN_OK, PULSCAN_EINVAL, PULSCAN_ENOWORKSPACE, PULSCAN_ECUDA, PULSCAN_EARCH =
 
 CANDIDATE_DTYPE = np.dtype([("spectrum", "<i4"), ("bin", "<i4"), ("width", "<i4"), ("power", "<f4"), ("sigma", "<f4")])
 assert CANDIDATE_DTYPE.itemsize == 20
+HCANDIDATE_DTYPE = np.dtype([("spectrum", "<i4"), ("bin", "<i4"), ("width", "<i4"), ("numharm", "<i4"), ("power", "<f4"),
+                             ("sigma", "<f4")])
+assert HCANDIDATE_DTYPE.itemsize == 24
 
 # name → (restype, argtypes); the single source for the loader and for the exported-symbol test
 _P = ctypes.c_void_p
@@ -30,6 +33,9 @@ SIGNATURES = {
     "pulscan_plan_set_mode": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_width_sampling": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int32]),
     "pulscan_plan_set_r_block": (ctypes.c_int, [_P, ctypes.c_int32]),
+    "pulscan_plan_set_harmonics": (ctypes.c_int, [_P, ctypes.c_int32]),
+    "pulscan_plan_max_hcandidates": (ctypes.c_int64, [_P]),
+    "pulscan_search_harmonics": (ctypes.c_int, [_P, _P, _P, _P, _P]),
     "pulscan_plan_set_tuning": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_double]),
     "pulscan_plan_set_cell_capacity": (ctypes.c_int, [_P, ctypes.c_int64]),
     "pulscan_plan_max_candidates": (ctypes.c_int64, [_P]),
@@ -96,7 +102,7 @@ class Plan:
     def __init__(self, n_bins: int, batch: int, zmax: int, block_width: int, sigma_threshold: float,
                  norm_block: Optional[int] = None, n_trials: Optional[float] = None, pitch: Optional[int] = None,
                  mode: int = 0, tile: int = 0, log10_p_flag: float = 0.0, host_staging: bool = False,
-                 cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False):
+                 cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False, numharm: int = 1):
         self.lib = load_library()
         self.n_bins, self.batch, self.zmax, self.block_width = int(n_bins), int(batch), int(zmax), int(block_width)
         self.handle = self.lib.pulscan_plan_create(n_bins, batch, zmax, block_width, sigma_threshold)
@@ -118,6 +124,10 @@ class Plan:
             _check(self.lib.pulscan_plan_set_width_sampling(self.handle, z_step, int(bool(log_sampling))))
         if r_block:
             _check(self.lib.pulscan_plan_set_r_block(self.handle, 1))
+        if numharm != 1:
+            _check(self.lib.pulscan_plan_set_harmonics(self.handle, numharm))
+        self.numharm = int(numharm)
+        self.d_hcandidates = None
         if cell_capacity:
             _check(self.lib.pulscan_plan_set_cell_capacity(self.handle, cell_capacity))
         self.pitch = int(pitch) if pitch is not None else self.n_bins
@@ -176,6 +186,29 @@ class Plan:
         assert d_spectra.numel() >= (self.batch - 1) * self.pitch + self.n_bins
         _check(self.lib.pulscan_search(self.handle, d_spectra.data_ptr(), self.d_candidates.data_ptr(),
                                        self.d_count.data_ptr(), _stream_ptr(stream)))
+
+    @property
+    def max_hcandidates(self) -> int:
+        return int(self.lib.pulscan_plan_max_hcandidates(self.handle))
+
+    def search_harmonics(self, d_spectra: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> None:
+        """pulscan_search_harmonics on the current (or given) stream; asynchronous.  Results stay in d_hcandidates / d_count."""
+        if self.workspace is None:
+            self.attach(d_spectra.device)
+        if self.d_hcandidates is None:
+            self.d_hcandidates = torch.empty(self.max_hcandidates * HCANDIDATE_DTYPE.itemsize, dtype=torch.uint8,
+                                             device=d_spectra.device)
+        assert d_spectra.is_cuda and d_spectra.dtype == torch.complex64 and d_spectra.is_contiguous()
+        assert d_spectra.numel() >= (self.batch - 1) * self.pitch + self.n_bins
+        _check(self.lib.pulscan_search_harmonics(self.handle, d_spectra.data_ptr(), self.d_hcandidates.data_ptr(),
+                                                 self.d_count.data_ptr(), _stream_ptr(stream)))
+
+    def hcandidates(self) -> np.ndarray:
+        """Synchronise and return the records of the last search_harmonics, sorted by (numharm, spectrum, bin)."""
+        n = int(self.d_count.item())
+        raw = self.d_hcandidates[: n * HCANDIDATE_DTYPE.itemsize].cpu().numpy()
+        rec = raw.view(HCANDIDATE_DTYPE).copy()
+        return rec[np.lexsort((rec["bin"], rec["spectrum"], rec["numharm"]))]
 
     def candidates(self) -> np.ndarray:
         """Synchronise and return the records of the last search, sorted by (spectrum, bin)."""

@@ -33,7 +33,8 @@ struct ExactSmemHdr {
 
 __global__ void __launch_bounds__(kExactThreads)
 block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, int zmax, int C, long long nblk,
-                   const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block,
+                   const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int numharm,
+                   pulscan_hcandidate* __restrict__ out_h,
                    const unsigned* __restrict__ flagged, const unsigned* __restrict__ counters,
                    pulscan_candidate* __restrict__ out, unsigned* __restrict__ out_count) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -99,7 +100,7 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
                 if (v > best) { best = v; arg = i; }
             }
             if (arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
-                double lnp = ln_q(w, best) + ln_trials;
+                double lnp = ln_q(w * shape_mult, best) + ln_trials;   // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220)
                 if (lnp > 0.0) lnp = 0.0;
                 if (lnp < my_lnp) { my_lnp = lnp; my_w = w; my_i = arg; my_s = best; } // ascending w: ties keep the smaller
             }
@@ -126,13 +127,20 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
                 }
             }
             if (my_w > 0 && my_lnp <= lnp_thr) {
-                pulscan_candidate r;
-                r.spectrum = (int32_t)row;
-                r.bin = r_block ? (int32_t)lo : (int32_t)(lo + my_i);   // R-Block: the block index × block width (L222-226)
-                r.width = my_w;
-                r.power = (float)my_s;
-                r.sigma = (float)sigma_from_lnp(my_lnp);
-                out[atomicAdd(out_count, 1u)] = r;
+                const int32_t bin = r_block ? (int32_t)lo : (int32_t)(lo + my_i);   // R-Block: block index × block width (L222-226)
+                const float sigma = (float)sigma_from_lnp(my_lnp);
+                const unsigned slot = atomicAdd(out_count, 1u);
+                if (out_h) {
+                    pulscan_hcandidate r;
+                    r.spectrum = (int32_t)row; r.bin = bin; r.width = my_w; r.numharm = numharm;
+                    r.power = (float)my_s; r.sigma = sigma;
+                    out_h[slot] = r;
+                } else {
+                    pulscan_candidate r;
+                    r.spectrum = (int32_t)row; r.bin = bin; r.width = my_w;
+                    r.power = (float)my_s; r.sigma = sigma;
+                    out[slot] = r;
+                }
             }
         }
         __syncthreads();

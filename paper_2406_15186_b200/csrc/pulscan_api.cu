@@ -15,6 +15,7 @@
 #include "../../include/pulscan.h"
 #include "block_exact.cuh"
 #include "boxcar_sweep.cuh"
+#include "harmonic_sum.cuh"
 #include "norm_power.cuh"
 #include "norm_power_v2.cuh"
 #include "significance.cuh"
@@ -63,6 +64,12 @@ struct pulscan_plan {
     double sigma_thr = 0, n_trials = 1.0;
     int64_t pitch = 0;
     int32_t mode = 0;
+    int32_t numharm = 1;                     // harmonic-summed spectra searched by pulscan_search_harmonics (L201-220)
+    int32_t shape_mult = 1;                  // H(H+1)/2 of the spectrum this plan searches: a width-w sum is Gamma(w·shape_mult)
+    int32_t numharm_tag = 1;                 // the H written into pulscan_hcandidate records by this plan
+    bool is_child = false;                   // a plan for one Y_H, owned by the plan the user created; it never normalises
+    std::vector<pulscan_plan*> harm;         // children for H = 2..numharm
+    size_t off_child = 0, child_ws_bytes = 0;
     int32_t r_block = 0;                     // report the candidate block's first bin instead of the exact bin (L222-226)
     int32_t z_step = 1, log_sampling = 0;   // which widths are searched (all are summed): Alg. 4
     int32_t tile_user = 0;
@@ -107,6 +114,9 @@ struct pulscan_plan {
     std::vector<cudaEvent_t> prof_events;
 };
 
+extern "C" pulscan_plan* pulscan_plan_create(int64_t, int32_t, int32_t, int32_t, float);
+extern "C" int pulscan_plan_destroy(pulscan_plan*);
+
 namespace {
 
 // ---------------------------------------------------------------- host-side plan derivation
@@ -140,7 +150,7 @@ int derive(pulscan_plan& p) {
         return p.log_sampling ? (z == 0 || (z & (z - 1)) == 0) : (z % p.z_step == 0);
     };
     for (int w = 1; w <= p.zmax; ++w) {
-        p.T[w - 1] = searched(w) ? power_threshold(w, lnp_target) : INFINITY;
+        p.T[w - 1] = searched(w) ? power_threshold(w * p.shape_mult, lnp_target) : INFINITY;
         p.Tp[w - 1] = searched(w) ? conservative_threshold(p.T[w - 1], w) : INFINITY;
     }
 
@@ -163,7 +173,7 @@ int derive(pulscan_plan& p) {
                 const int g = 1 << lg, Lc = w + 2 * g - 2;
                 if ((tile >> lg) % kSweepR != 0) break;
                 if (l10 >= 0.0 || !std::isfinite(p.T[w - 1]) ||
-                    ln_q(Lc, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
+                    ln_q(Lc * p.shape_mult, (double)conservative_threshold(p.T[w - 1], Lc)) <= ln_pflag) best = lg; else break;
             }
             lgw[w] = (w > 1 && !std::isfinite(p.T[w - 1])) ? lgw[w - 1] : best;   // a width that is not searched follows its neighbour
         }
@@ -276,7 +286,9 @@ int derive(pulscan_plan& p) {
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
     p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
 
-    // ---- normalisation launch shapes
+    // ---- normalisation launch shapes (a child plan searches a spectrum that its parent has normalised and summed)
+    if (p.is_child) { p.main_blocks_per_row = 0; p.has_tail = false; p.use_fast = false; }
+    else {
     const int64_t len_last = p.n - (int64_t)(p.nb - 1) * p.B;
     if (p.B <= 8192) { p.nt_main = 256; p.ept_main = pow2_ceil((p.B + 255) / 256); }
     else { p.nt_main = 1024; p.ept_main = pow2_ceil((p.B + 1023) / 1024); }
@@ -297,6 +309,7 @@ int derive(pulscan_plan& p) {
     p.norm_nt = (std::getenv("PULSCAN_NORM_NT256") == nullptr && !p.norm_staged && p.B >= 512 && p.B <= 4096) ? 128 : 256;
     p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 &&
                  std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
+    }
 
     // ---- workspace layout
     size_t o = 0;
@@ -316,8 +329,29 @@ int derive(pulscan_plan& p) {
         p.off_stage_cand = o; o += align_up((size_t)p.batch * p.nblk * sizeof(pulscan_candidate), 256);
         p.off_stage_count = o; o += 256;
     }
+    // ---- harmonic-summed spectra: one child plan per H = 2..numharm; they run one after the other, so they share one
+    //      region of the workspace, sized for H = 2 (a child's own "power" buffer is Y_H)
+    for (pulscan_plan* c : p.harm) pulscan_plan_destroy(c);
+    p.harm.clear();
+    p.off_child = o; p.child_ws_bytes = 0;
+    for (int H = 2; H <= p.numharm && !p.is_child; ++H) {
+        const int64_t nH = p.n / H;
+        if ((int64_t)p.zmax >= nH) return fail(PULSCAN_EINVAL, "zmax = %d must be < floor(n_bins / %d) = %lld", p.zmax, H, (long long)nH);
+        pulscan_plan* c = pulscan_plan_create(nH, p.batch, p.zmax, p.C, (float)p.sigma_thr);
+        if (!c) return PULSCAN_EINVAL;
+        c->is_child = true; c->shape_mult = H * (H + 1) / 2; c->numharm_tag = H; c->sigma_thr = p.sigma_thr; c->n_trials = p.n_trials;
+        c->z_step = p.z_step; c->log_sampling = p.log_sampling; c->tile_user = p.tile_user; c->log10_p_flag = p.log10_p_flag;
+        c->cell_cap_user = p.cell_cap_user; c->B = p.B;
+        p.harm.push_back(c);
+        const int rc = derive(*c);
+        if (rc) return rc;
+        p.child_ws_bytes = std::max(p.child_ws_bytes, align_up(c->need_bytes, 256));
+    }
+    o += p.child_ws_bytes;
     p.need_bytes = o;
     p.dirty = false;
+    if (p.ws && p.ws_bytes >= p.need_bytes)
+        for (pulscan_plan* c : p.harm) { c->ws = static_cast<char*>(p.ws) + p.off_child; c->ws_bytes = p.child_ws_bytes; }
     return PULSCAN_OK;
 }
 
@@ -463,6 +497,45 @@ int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStr
     return rc;
 }
 
+// Kernels (b) and (c) on a power (or harmonic-summed) spectrum that is ready in d_P; the plan's bitmap and counters must
+// have been zeroed on the stream.  Exactly one of d_candidates / d_hcandidates is non-null.
+int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candidates, pulscan_hcandidate* d_hcandidates,
+                        uint32_t* d_count, cudaStream_t st, cudaEvent_t* ev) {
+    int rc = PULSCAN_OK;
+    char* ws = static_cast<char*>(p.ws);
+    unsigned* d_bitmap = reinterpret_cast<unsigned*>(ws + p.off_bitmap);
+    unsigned* d_flagged = reinterpret_cast<unsigned*>(ws + p.off_flagged);
+    unsigned* d_counters = reinterpret_cast<unsigned*>(ws + p.off_counters);
+    const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
+    if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
+    if (p.mode == 0) {
+        SweepCell* d_cells = reinterpret_cast<SweepCell*>(ws + p.off_cells);
+        boxcar_sweep_kernel<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
+                                                                              p.C, p.nblk, p.d_tau, d_cells, p.cell_cap,
+                                                                              d_bitmap, d_flagged, d_counters);
+        CUDA_TRY(cudaGetLastError());
+        if ((rc = debug_sync("boxcar_sweep_kernel"))) return rc;
+        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
+                                                                                  p.nblk, p.d_tau, p.d_Tp, d_cells, p.cell_cap,
+                                                                                  d_bitmap, d_flagged, d_counters);
+    } else {
+        boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_P, p.pitchP,
+                                                                                p.n, p.tiles_per_row, p.C, p.nblk, p.d_Tp,
+                                                                                d_bitmap, d_flagged, d_counters);
+    }
+    CUDA_TRY(cudaGetLastError());
+    if ((rc = debug_sync(p.mode ? "boxcar_exhaustive_kernel" : "sweep_refine_kernel"))) return rc;
+    if (ev) CUDA_TRY(cudaEventRecord(ev[3], st));
+
+    const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
+    const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
+    block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
+                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.numharm_tag, d_hcandidates,
+                                                                   d_flagged, d_counters, d_candidates, d_count);
+    CUDA_TRY(cudaGetLastError());
+    return PULSCAN_OK;
+}
+
 int check_plan_ready(pulscan_plan* plan) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     int rc = derive(*plan);
@@ -470,6 +543,11 @@ int check_plan_ready(pulscan_plan* plan) {
     if (!plan->ws) return fail(PULSCAN_ENOWORKSPACE, "no workspace attached (pulscan_plan_set_workspace)");
     if (plan->ws_bytes < plan->need_bytes)
         return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes attached, %zu needed", plan->ws_bytes, plan->need_bytes);
+    for (pulscan_plan* c : plan->harm) {
+        c->ws = static_cast<char*>(plan->ws) + plan->off_child; c->ws_bytes = plan->child_ws_bytes;
+        c->sm_count = plan->sm_count;
+        if ((rc = ensure_device(*c))) return rc;
+    }
     return ensure_device(*plan);
 }
 
@@ -589,6 +667,7 @@ int pulscan_plan_set_workspace(pulscan_plan* plan, void* d_workspace, size_t byt
     if (bytes < plan->need_bytes)
         return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes given, %zu needed", bytes, plan->need_bytes);
     plan->ws = d_workspace; plan->ws_bytes = bytes;
+    for (pulscan_plan* c : plan->harm) { c->ws = static_cast<char*>(d_workspace) + plan->off_child; c->ws_bytes = plan->child_ws_bytes; }
     return PULSCAN_OK;
 }
 
@@ -651,34 +730,66 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     if (rc) return rc;
     if (ev) CUDA_TRY(cudaEventRecord(ev[2], st));
 
-    const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
-    if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
-    if (p.mode == 0) {
-        SweepCell* d_cells = reinterpret_cast<SweepCell*>(ws + p.off_cells);
-        boxcar_sweep_kernel<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
-                                                                              p.C, p.nblk, p.d_tau, d_cells, p.cell_cap,
-                                                                              d_bitmap, d_flagged, d_counters);
-        CUDA_TRY(cudaGetLastError());
-        if ((rc = debug_sync("boxcar_sweep_kernel"))) return rc;
-        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
-                                                                                  p.nblk, p.d_tau, p.d_Tp, d_cells, p.cell_cap,
-                                                                                  d_bitmap, d_flagged, d_counters);
-    } else {
-        boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_P, p.pitchP,
-                                                                                p.n, p.tiles_per_row, p.C, p.nblk, p.d_Tp,
-                                                                                d_bitmap, d_flagged, d_counters);
-    }
-    CUDA_TRY(cudaGetLastError());
-    if ((rc = debug_sync(p.mode ? "boxcar_exhaustive_kernel" : "sweep_refine_kernel"))) return rc;
-    if (ev) CUDA_TRY(cudaEventRecord(ev[3], st));
-
-    const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
-    const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
-    block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
-                                                                   p.lnp_thr, p.r_block, d_flagged, d_counters, d_candidates, d_count);
-    CUDA_TRY(cudaGetLastError());
+    rc = enqueue_sweep_exact(p, d_P, d_candidates, nullptr, d_count, st, ev);
+    if (rc) return rc;
     if (ev) CUDA_TRY(cudaEventRecord(ev[4], st));
     return debug_sync("block_exact_kernel");
+}
+
+int pulscan_plan_set_harmonics(pulscan_plan* plan, int32_t numharm) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (numharm < 1 || numharm > 4) return fail(PULSCAN_EINVAL, "numharm = %d out of range [1, 4]", numharm);
+    if ((int64_t)plan->zmax >= plan->n / numharm)
+        return fail(PULSCAN_EINVAL, "zmax = %d must be < floor(n_bins / numharm) = %lld", plan->zmax, (long long)(plan->n / numharm));
+    plan->numharm = numharm; plan->dirty = true;
+    return PULSCAN_OK;
+}
+
+int64_t pulscan_plan_max_hcandidates(const pulscan_plan* plan) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    int64_t total = 0;
+    for (int H = 1; H <= plan->numharm; ++H) total += (int64_t)plan->batch * ((plan->n / H + plan->C - 1) / plan->C);
+    return total;
+}
+
+int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_hcandidate* d_hcandidates, uint32_t* d_count,
+                             void* cuda_stream) {
+    int rc = check_plan_ready(plan);
+    if (rc) return rc;
+    if (!d_spectra || !d_hcandidates || !d_count) return fail(PULSCAN_EINVAL, "null pointer");
+    if (reinterpret_cast<uintptr_t>(d_spectra) & 7) return fail(PULSCAN_EINVAL, "d_spectra must be 8-byte aligned");
+    if (reinterpret_cast<uintptr_t>(d_hcandidates) & 3 || reinterpret_cast<uintptr_t>(d_count) & 3)
+        return fail(PULSCAN_EINVAL, "d_hcandidates / d_count must be 4-byte aligned");
+    pulscan_plan& p = *plan;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char* ws = static_cast<char*>(p.ws);
+    float* d_P = reinterpret_cast<float*>(ws + p.off_P);
+    unsigned* d_counters = reinterpret_cast<unsigned*>(ws + p.off_counters);
+    CUDA_TRY(cudaMemsetAsync(ws + p.off_bitmap, 0, p.bitmap_bytes, st));
+    CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
+    CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
+    rc = enqueue_norm(p, d_spectra, d_P, st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1);      // (a)
+    if (rc) return rc;
+    if ((rc = enqueue_sweep_exact(p, d_P, nullptr, d_hcandidates, d_count, st, nullptr))) return rc;           // Y_1 = P
+    for (pulscan_plan* cp : p.harm) {                                                                            // Y_2 …
+        pulscan_plan& c = *cp;
+        c.mode = p.mode; c.r_block = p.r_block;
+        char* cws = static_cast<char*>(c.ws);
+        float* d_Y = reinterpret_cast<float*>(cws + c.off_P);
+        CUDA_TRY(cudaMemsetAsync(cws + c.off_bitmap, 0, c.bitmap_bytes, st));
+        CUDA_TRY(cudaMemsetAsync(cws + c.off_counters, 0, 256, st));
+        const long long total = (long long)c.batch * c.n;
+        const int grid = (int)std::min<long long>((total + kHarmThreads - 1) / kHarmThreads, (long long)p.sm_count * 16);
+        switch (c.numharm_tag) {
+            case 2: harmonic_sum_kernel<2><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, d_Y, c.pitchP, c.n, total); break;
+            case 3: harmonic_sum_kernel<3><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, d_Y, c.pitchP, c.n, total); break;
+            default: harmonic_sum_kernel<4><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, d_Y, c.pitchP, c.n, total); break;
+        }
+        CUDA_TRY(cudaGetLastError());
+        if ((rc = debug_sync("harmonic_sum_kernel"))) return rc;
+        if ((rc = enqueue_sweep_exact(c, d_Y, nullptr, d_hcandidates, d_count, st, nullptr))) return rc;
+    }
+    return PULSCAN_OK;
 }
 
 int pulscan_search_host(pulscan_plan* plan, const void* h_spectra, pulscan_candidate* h_candidates, uint32_t* h_count,
@@ -788,6 +899,7 @@ int pulscan_plan_get_profile(pulscan_plan* plan, int32_t slot, float* h_ms) {
 
 int pulscan_plan_destroy(pulscan_plan* plan) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    for (pulscan_plan* c : plan->harm) pulscan_plan_destroy(c);
     release_profiling(*plan);
     release_device(*plan);
     delete plan;

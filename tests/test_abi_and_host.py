@@ -68,6 +68,8 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_tuning(p.handle, 1000, 0.0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 2048, -1.0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_width_sampling(p.handle, 0, 0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_harmonics(p.handle, 0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_harmonics(p.handle, 5) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_cell_capacity(p.handle, -1) == binding.PULSCAN_EINVAL
     ws0 = p.workspace_bytes
     assert lib.pulscan_plan_set_cell_capacity(p.handle, 1 << 20) == binding.PULSCAN_OK
@@ -162,3 +164,14 @@ def test_width_sampling_masks_thresholds(binding):
     step = binding.Plan(50000, 1, 40, 100, 6.0, z_step=5).thresholds()
     assert [w for w in range(1, 41) if np.isfinite(step[w - 1])] == [1, 6, 11, 16, 21, 26, 31, 36]   # Alg. 4
     assert "sweep level" in binding.Plan(50000, 1, 40, 100, 6.0, log_sampling=True).describe()
+
+
+def test_harmonics_sizes(binding):
+    p1 = binding.Plan(10001, 3, 16, 50, 6.0)
+    p4 = binding.Plan(10001, 3, 16, 50, 6.0, numharm=4)
+    assert binding.HCANDIDATE_DTYPE.itemsize == 24
+    assert p1.max_hcandidates == p1.max_candidates == 3 * 201
+    assert p4.max_hcandidates == 3 * (201 + 100 + 67 + 50)      # ceil(floor(n/H)/C) blocks of Y_1..Y_4 (R29)
+    assert p4.workspace_bytes > p1.workspace_bytes              # room for Y_H and the scratch of its search
+    with pytest.raises(binding.PulscanError):
+        binding.Plan(100, 1, 30, 10, 6.0, numharm=4)            # zmax must be < floor(n/numharm)

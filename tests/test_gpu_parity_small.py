@@ -147,6 +147,41 @@ def test_r_block_matches_oracle(orc):
     assert np.array_equal(gpu["bin"], exact["bin"] // 100 * 100) and np.array_equal(gpu["sigma"], exact["sigma"])
 
 
+def _assert_same_hcandidates(gpu, ora, context):
+    gk = list(zip(gpu["numharm"].tolist(), gpu["spectrum"].tolist(), gpu["bin"].tolist(), gpu["width"].tolist()))
+    ok = list(zip(ora["numharm"].tolist(), ora["spectrum"].tolist(), ora["bin"].tolist(), ora["width"].tolist()))
+    assert gk == ok, (f"{context}: gpu {len(gk)} vs oracle {len(ok)}; only gpu {sorted(set(gk) - set(ok))[:8]}; "
+                      f"only oracle {sorted(set(ok) - set(gk))[:8]}")
+    rel = np.abs(gpu["power"].astype(np.float64) - ora["power"]) / ora["power"]
+    assert rel.max() <= 1e-5, f"{context}: power rel err {rel.max():.3g}"
+    assert np.abs(gpu["sigma"].astype(np.float64) - ora["sigma"]).max() <= 1e-3, context
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,batch,zmax,B,C,thr,numharm,log_sampling", [
+    (20001, 2, 40, 2048, 100, 4.0, 4, False), (9001, 2, 200, 4096, 200, 4.0, 3, False), (30011, 1, 64, 8192, 300, 4.5, 4, True),
+    (4099, 3, 16, 1024, 64, 3.5, 2, False)])
+def test_harmonic_search_matches_oracle(orc, n, batch, zmax, B, C, thr, numharm, log_sampling, mode):
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(batch, n, seed=n + numharm)
+    for h in range(1, 5):                                  # power at bin 501 and its harmonics, two bins wide
+        if h * 501 + 2 < n:
+            spec[0, h * 501: h * 501 + 2] *= 3.0
+    bump(spec, batch - 1, n // 2, min(zmax, 30), 1.8)
+    plan = binding.Plan(n, batch, zmax, C, thr, norm_block=B, mode=mode, numharm=numharm, log_sampling=log_sampling)
+    plan.attach("cuda")
+    plan.search_harmonics(spec)
+    gpu = plan.hcandidates()
+    plan.search(spec)                                      # the plain search of the same plan is unaffected
+    plain = plan.candidates()
+    plan.destroy()
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, numharm, log_sampling=log_sampling)
+    assert len(ora) > 0 and set(ora["numharm"].tolist()) == set(range(1, numharm + 1))
+    _assert_same_hcandidates(gpu, ora, f"n={n} numharm={numharm} mode={mode}")
+    h1 = gpu[gpu["numharm"] == 1]
+    assert np.array_equal(h1["bin"], plain["bin"]) and np.array_equal(h1["sigma"], plain["sigma"])
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)
