@@ -46,6 +46,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--log10-p-flag", type=float, default=0.0)
+    ap.add_argument("--numharm", type=int, default=1, help="also search the harmonic-summed spectra Y_2..Y_numharm "
+                    "(PAPER.md:L201-220; pulscan_search_harmonics; not the headline)")
     ap.add_argument("--z-step", type=int, default=1, help="search every z_step-th drift only (PAPER.md:L152; not the headline)")
     ap.add_argument("--log-sampling", action="store_true", help="search z = 0, 1, 2, 4, ... only (PAPER.md:L411; not the headline)")
     return ap.parse_args()
@@ -215,18 +217,20 @@ def run_ours(args):
     steps, warm = args.steps, max(args.warmup, 3)
 
     plan = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
-                        tile=args.tile, log10_p_flag=args.log10_p_flag, z_step=args.z_step, log_sampling=args.log_sampling)
+                        tile=args.tile, log10_p_flag=args.log10_p_flag, z_step=args.z_step, log_sampling=args.log_sampling,
+                        numharm=args.numharm)
     plan.attach(dev)
+    run_search = plan.search_harmonics if args.numharm > 1 else plan.search
     plan.set_profiling(warm + steps)
     stream = torch.cuda.current_stream()
     for _ in range(warm):
-        plan.search(X, stream)
+        run_search(X, stream)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize(); pdist.barrier(); torch.cuda.synchronize()
     with ClockSampler(torch.cuda.current_device()) as clk:
         e0.record(stream)
         for _ in range(steps):
-            plan.search(X, stream)
+            run_search(X, stream)
         e1.record(stream)
         torch.cuda.synchronize(); pdist.barrier(); torch.cuda.synchronize()
     ms_total = pdist.max_over_ranks(e0.elapsed_time(e1))
@@ -238,6 +242,17 @@ def run_ours(args):
     flagged = int(stats[0])
 
     # per-kernel device times of the timed steps (CUDA events recorded by the library on the launching stream)
+    if args.numharm > 1:   # the per-stage events belong to pulscan_search: report the whole step only
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
+                              "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                              "dtype": "f32", "data": "synthetic", "config": dict(config_dict(wl, world, args), numharm=args.numharm),
+                              "bin_widths_per_sec": value * wl.zmax, "candidates_per_step": n_cand, "clocks": clk.summary(),
+                              "gpu_launches": (plan.launches_per_search + 4 * (args.numharm - 1)) * steps}), flush=True)
+        plan.destroy()
+        if world > 1:
+            tdist.destroy_process_group()
+        return 0
     prof = np.array([plan.profile(s) for s in range(warm, warm + steps)], dtype=np.float64).mean(axis=0)
     kernels = {"norm_power_kernel": (prof[1], 12 * bins), "boxcar_sweep_kernel": (prof[2], 4 * bins),
                "block_exact_kernel": (prof[3], None)}

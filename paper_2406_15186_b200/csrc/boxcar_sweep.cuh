@@ -151,7 +151,10 @@ __device__ __forceinline__ float scan_sel5(const float (&s)[5], int q) {
     return v;
 }
 
-template <class AfterLoads>
+// FINE = true additionally keeps the prefix inside each quad (x[3q+t] = the quad's first t+1 powers) and writes the arrays
+// with g = 1 and g = 2 (PG0 = PP itself, PG1): needed when a level's covers must be finer than 4 bins — harmonic-summed
+// spectra, whose noise level per bin is H(H+1)/2, and very low σ thresholds.
+template <bool FINE, class AfterLoads>
 __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* raw, float* sG, ScanSmem& ss,
                                            AfterLoads after_loads) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -161,12 +164,18 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
         const int i0 = pass * kScanPass + kScanPer * tid;
         const bool act = i0 < len;
         float s[5];
+        float x[FINE ? 15 : 1];
         if (act) {
             const float4* zq = reinterpret_cast<const float4*>(raw) + (i0 >> 2);
 #pragma unroll
             for (int q = 0; q < 5; ++q) {
                 const float4 v = zq[q];
-                s[q] = (v.x + v.y) + (v.z + v.w);
+                if (FINE) {
+                    x[3 * q] = v.x; x[3 * q + 1] = v.x + v.y; x[3 * q + 2] = x[3 * q + 1] + v.z;
+                    s[q] = x[3 * q + 2] + v.w;
+                } else {
+                    s[q] = (v.x + v.y) + (v.z + v.w);
+                }
             }
 #pragma unroll
             for (int q = 1; q < 5; ++q) s[q] += s[q - 1];
@@ -201,10 +210,26 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
 #pragma unroll
             for (int q = 0; q < 5; ++q) s[q] += off;            // s[q] = PP[4(u+q)]
             const int u = (i0 >> 2) + 1;
+            if (FINE) {                                         // x[3q+t] = PP[i0 + 4q + t + 1], t = 0..2
+#pragma unroll
+                for (int q = 0; q < 5; ++q) {
+                    const float oq = q ? s[q - 1] : off;
+                    x[3 * q] += oq; x[3 * q + 1] += oq; x[3 * q + 2] += oq;
+                }
+            }
             for (int a = 0; a < sp.narr; ++a) {
                 const int lg = sp.arr_lg[a];
                 float* dst = sG + sp.arr_off[a];
-                if (lg == 2) {
+                if (FINE && lg == 0) {                          // PG0[i] = PP[i]: entries i0+1 … i0+20 (the pad holds 16)
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) {
+                        float* d = dst + i0 + 4 * q + 1;
+                        if (i0 + 4 * q + 4 <= len + kPadG) { d[0] = x[3 * q]; d[1] = x[3 * q + 1]; d[2] = x[3 * q + 2]; d[3] = s[q]; }
+                    }
+                } else if (FINE && lg == 1) {                   // PG1[k] = PP[2k]: entries i0/2+1 … i0/2+10
+#pragma unroll
+                    for (int q = 0; q < 5; ++q) { dst[(i0 >> 1) + 2 * q + 1] = x[3 * q + 1]; dst[(i0 >> 1) + 2 * q + 2] = s[q]; }
+                } else if (lg == 2) {
 #pragma unroll
                     for (int q = 0; q < 5; ++q) dst[u + q] = s[q];
                 } else if (lg == 3) {
@@ -355,6 +380,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
 // counters[2] = cells appended (the refine kernel's work count), counters[3] = cells dropped because the list was full
 // (their tile's blocks are all marked instead, which is always allowed: kernel (c) decides).
 // Dynamic shared memory: [kSweepBufs × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
+template <bool FINE>
 __global__ void __launch_bounds__(kSweepThreads, PULSCAN_SWEEP_OCC)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
@@ -406,7 +432,7 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             for (int i = (int)nv + tid; i < sp.len; i += kSweepThreads) raw[i] = 0.f;
             __syncthreads();
         }
-        const float pp_max = scan_tile(sp, raw, sG, ctl.scan, [&] {
+        const float pp_max = scan_tile<FINE>(sp, raw, sG, ctl.scan, [&] {
             const long long nxt = item + kSweepBufs * stride;
             if (tid == 0 && nxt < n_items) sweep_issue_tile(sp, nxt, P, pitchP, tiles_per_row, raw, &ctl.mbar[b]);
         });

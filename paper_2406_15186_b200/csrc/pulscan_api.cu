@@ -86,6 +86,7 @@ struct pulscan_plan {
     std::vector<float> tau;    // per-level cover thresholds
     SweepParams sp{};
     int tiles_per_row = 0;
+    bool sweep_fine = false;   // some level has g < 4: the sweep keeps the full-resolution prefix sum
     int refine_grid = 0;
     int sweep_grid = 0;        // persistent CTAs of the pruned sweep: SM count × resident CTAs per SM
     size_t smem_sweep = 0, smem_refine = 0, smem_exh = 0, smem_exact = 0;
@@ -158,9 +159,9 @@ int derive(pulscan_plan& p) {
     int tile = p.tile_user ? p.tile_user : (p.zmax <= 512 ? 4096 : 8192);
     // ---- group size per width: the largest g = 2^lg whose worst cover (w + 2g − 2 bins) of pure noise passes the
     //      width's threshold with probability ≤ p_flag; made non-decreasing in w by a suffix minimum.
-    //      g = 4 is always allowed (at very low σ thresholds its covers simply pass often and the refine kernel and
-    //      kernel (c) do the work).  If the width range then needs more than kMaxLevels levels, p_flag is relaxed
-    //      tenfold at a time: it affects speed only.
+    //      Levels with g < 4 (narrow widths of harmonic-summed spectra, very low σ thresholds) make the sweep use its
+    //      full-resolution scan (boxcar_sweep_kernel<true>).  If the width range needs more than kMaxLevels levels,
+    //      p_flag is relaxed tenfold at a time: it affects speed only.
     const int lg_cap = 6;
     std::vector<int> lgw(p.zmax + 2, 0);
     std::vector<SweepLevel> lvls;
@@ -168,8 +169,8 @@ int derive(pulscan_plan& p) {
     for (double l10 = p.log10_p_flag;; l10 += 1.0) {
         const double ln_pflag = l10 * 2.302585092994046;
         for (int w = 1; w <= p.zmax; ++w) {
-            int best = 2;                 // the scan produces PP at multiples of 4 only: the finest group is 4 bins
-            for (int lg = 3; lg <= lg_cap; ++lg) {
+            int best = 0;                 // g = 1: the cover is the window itself
+            for (int lg = 1; lg <= lg_cap; ++lg) {
                 const int g = 1 << lg, Lc = w + 2 * g - 2;
                 if ((tile >> lg) % kSweepR != 0) break;
                 if (l10 >= 0.0 || !std::isfinite(p.T[w - 1]) ||
@@ -269,6 +270,8 @@ int derive(pulscan_plan& p) {
         sp.lv[l] = lv;
     }
     sp.ntasks = task;
+    p.sweep_fine = false;
+    for (int a = 0; a < sp.narr; ++a) p.sweep_fine = p.sweep_fine || sp.arr_lg[a] < 2;
     if (task > kMaxWarpTasks) return fail(PULSCAN_EINVAL, "sweep tile of %d bins needs %d warp-tasks (limit %d)", tile, task, kMaxWarpTasks);
     sp.ntau = (int)p.tau.size();
     sp.smem_floats = kSweepBufs * sp.z_floats + off;
@@ -371,17 +374,24 @@ int ensure_device(pulscan_plan& p) {
     CUDA_TRY(cudaMemcpy(p.d_T, p.T.data(), p.T.size() * sizeof(double), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(p.d_Tp, p.Tp.data(), p.Tp.size() * sizeof(float), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(p.d_tau, p.tau.data(), p.tau.size() * sizeof(float), cudaMemcpyHostToDevice));
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_sweep));
-    CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_refine));
+    const auto sweep_fn = p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>;
+    // The limit is a property of the function, shared by every plan of the process (and by a plan's harmonic children):
+    // allow the device maximum once instead of this plan's own size, which a later plan could lower again.
+    constexpr int kMaxDynSmem = 227 * 1024;
+    CUDA_TRY(cudaFuncSetAttribute(sweep_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     int occ = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, boxcar_sweep_kernel, kSweepThreads, p.smem_sweep));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_fn, kSweepThreads, p.smem_sweep));
     if (occ < 1) return fail(PULSCAN_ECUDA, "boxcar_sweep_kernel does not fit an SM with %zu bytes of shared memory", p.smem_sweep);
     p.sweep_grid = (int)std::min<long long>((long long)p.tiles_per_row * p.batch, (long long)p.sm_count * occ);
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_refine_kernel, kRefineThreads, p.smem_refine));
     if (occ < 1) return fail(PULSCAN_ECUDA, "sweep_refine_kernel does not fit an SM with %zu bytes of shared memory", p.smem_refine);
     p.refine_grid = p.sm_count * std::min(occ, 16);
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exh));
-    CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_exact));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    if (p.smem_sweep > (size_t)kMaxDynSmem || p.smem_exh > (size_t)kMaxDynSmem || p.smem_exact > (size_t)kMaxDynSmem)
+        return fail(PULSCAN_EINVAL, "plan needs more shared memory than an SM has (sweep %zu, exhaustive %zu, exact %zu bytes)",
+                    p.smem_sweep, p.smem_exh, p.smem_exact);
     p.device_ready = true;
     return PULSCAN_OK;
 }
@@ -510,7 +520,7 @@ int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candid
     if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
     if (p.mode == 0) {
         SweepCell* d_cells = reinterpret_cast<SweepCell*>(ws + p.off_cells);
-        boxcar_sweep_kernel<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
+        (p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>)<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
                                                                               p.C, p.nblk, p.d_tau, d_cells, p.cell_cap,
                                                                               d_bitmap, d_flagged, d_counters);
         CUDA_TRY(cudaGetLastError());

@@ -82,6 +82,24 @@ def test_batched_configs_full(orc, cfg, n_noise):
     torch.cuda.empty_cache()
 
 
+def test_config2_harmonics_log_sampling_full(orc):
+    """The paper's GPU configuration (Fig. 10: numharm 4, log-sampled z) on BASELINE config 2's spectrum, full size."""
+    wl = synth.CONFIGS[2]
+    X, inj = synth.make_spectra(wl)
+    plan = binding.Plan(wl.n_bins, 1, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block, numharm=4,
+                        log_sampling=True)
+    plan.attach("cuda")
+    plan.search_harmonics(X.cuda())
+    rec = plan.hcandidates()
+    plan.destroy()
+    ora = orc.search_harmonics(X.numpy(), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold, 4, log_sampling=True)
+    key = lambda r: list(zip(r["numharm"].tolist(), r["bin"].tolist(), r["width"].tolist()))
+    assert key(rec) == key(ora) and len(ora) > 0
+    assert np.all(np.abs(rec["power"] - ora["power"]) <= 1e-5 * ora["power"])
+    assert np.all(np.abs(rec["sigma"] - ora["sigma"]) <= 1e-3)
+    assert set(rec["width"].tolist()) <= {1, 2, 3, 5, 9, 17, 33, 65, 129}
+
+
 def test_host_buffer_entry_point_matches_device_entry_point():
     wl = synth.CONFIGS[3].scaled(batch=6, frac_injected=0.5)
     X, _ = synth.make_spectra(wl, device="cuda")
