@@ -78,6 +78,13 @@ def _load():
         lib.orc_search_harmonics.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                              ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
                                              ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64]
+        lib.orc_median_of_medians.restype = ctypes.c_double
+        lib.orc_median_of_medians.argtypes = [c_dp, ctypes.c_int64]
+        lib.orc_normalise_power_mom.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, c_dp]
+        lib.orc_search_general.restype = ctypes.c_int64
+        lib.orc_search_general.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                           ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
+                                           ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64]
         lib.orc_search.restype = ctypes.c_int64
         lib.orc_search.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                    ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64]
@@ -210,7 +217,7 @@ def harmonic_sum(P, H: int) -> np.ndarray:
 
 def search_harmonics(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshold: float, numharm: int,
                      n_trials: float = 1.0, n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False,
-                     r_block: bool = False) -> np.ndarray:
+                     r_block: bool = False, median_of_medians: bool = False) -> np.ndarray:
     """The search on every harmonic-summed spectrum Y_1 … Y_numharm (§2.3): records carry `numharm`; ordered by
     (numharm, spectrum, bin); at most one per candidate block of each summed spectrum."""
     s = np.ascontiguousarray(spectra, dtype=np.complex64)
@@ -222,8 +229,23 @@ def search_harmonics(spectra, zmax: int, norm_block: int, block_width: int, sigm
     cap = sum(batch * ((n // H + C - 1) // C) for H in range(1, int(numharm) + 1))
     out = np.zeros(cap, dtype=CANDIDATE_DTYPE)
     f = s.view(np.float32)
-    found = _load().orc_search_harmonics(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
-                                         int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
-                                         int(bool(log_sampling)), int(bool(r_block)), int(numharm),
-                                         out.ctypes.data_as(ctypes.c_void_p), cap)
+    found = _load().orc_search_general(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
+                                       int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
+                                       int(bool(log_sampling)), int(bool(r_block)), int(numharm),
+                                       int(bool(median_of_medians)), out.ctypes.data_as(ctypes.c_void_p), cap)
     return out[: int(found)].copy()
+
+
+def median_of_medians(values) -> float:
+    """Alg. 1's reduction of 4^k or 2·4^k values (reading R30); the input is not modified."""
+    v = np.array(values, dtype=np.float64)
+    return float(_load().orc_median_of_medians(_dp(v), v.size))
+
+
+def normalise_power_mom(spectrum, norm_block: int) -> np.ndarray:
+    """Steps 1-3 with the paper's GPU normalisation (Alg. 1: approximate median and MAD, scale 1.4826)."""
+    f = _as_interleaved(spectrum).reshape(-1)
+    n = f.size // 2
+    P = np.empty(n, dtype=np.float64)
+    _load().orc_normalise_power_mom(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), n, int(norm_block), _dp(P))
+    return P

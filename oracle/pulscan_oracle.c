@@ -172,6 +172,57 @@ double orc_sigma_from_lnp(double lnp) {
     return 0.5 * (lo + hi);
 }
 
+/* ---- Algorithm 1: the paper's GPU normalisation, an APPROXIMATE median ("median of medians",
+ * L232 "threads recursively find the median of 4 non-overlapping elements").  Followed step by step:
+ *   local_median(a,b,c,d) = (a+b+c+d − min − max)/2                                             (L627-631)
+ *   for strides ← count/4, count/16, …, 1:  sdata[i] ← local_median(sdata[i], sdata[i+stride], sdata[i+2·stride],
+ *                                                                    sdata[i+3·stride]),  i < stride        (L636-642)
+ * Reading R30: the count must be 4^k or 2·4^k; a last level of two values returns their mean (the median of two).
+ * The input is overwritten. */
+static double orc_local_median(double a, double b, double c, double d) {
+    double mn = fmin(fmin(fmin(a, b), c), d);
+    double mx = fmax(fmax(fmax(a, b), c), d);
+    return (a + b + c + d - mn - mx) / 2.0;
+}
+
+double orc_median_of_medians(double* sdata, int64_t count) {
+    while (count >= 4) {
+        int64_t stride = count / 4;
+        for (int64_t i = 0; i < stride; ++i)
+            sdata[i] = orc_local_median(sdata[i], sdata[i + stride], sdata[i + 2 * stride], sdata[i + 3 * stride]);
+        count = stride;
+    }
+    if (count == 2) return 0.5 * (sdata[0] + sdata[1]);
+    return sdata[0];
+}
+
+/* Alg. 1's Procedure (L643-649) for every chunk of B bins, per component (L140): median ← median_of_medians(chunk);
+ * MAD ← median_of_medians(|chunk − median|) (the listing omits the absolute value, R5); scale_factor ← 1.4826 (the
+ * 5-digit constant the listing prints); normalised ← (chunk − median)/(scale_factor·MAD); then P = |X'|²/2 (R2).
+ * Reading R30: chunk j is bins [jB, (j+1)B); the n mod B bins after the last chunk are normalised with the last chunk's
+ * median and MAD (Alg. 1 reduces exactly one chunk of 4·blockDim values); MAD = 0 → 0 (R7).  Needs n ≥ B. */
+void orc_normalise_power_mom(const float* spec, int64_t n, int64_t B, double* P) {
+    int64_t nb = n / B;
+    double* buf = (double*)malloc((size_t)B * sizeof(double));
+    for (int64_t j = 0; j < nb; ++j) {
+        int64_t lo = j * B;
+        int64_t hi = (j == nb - 1) ? n : (j + 1) * B;
+        double med[2], scale[2];
+        for (int comp = 0; comp < 2; ++comp) {
+            for (int64_t k = 0; k < B; ++k) buf[k] = (double)spec[2 * (lo + k) + comp];
+            med[comp] = orc_median_of_medians(buf, B);
+            for (int64_t k = 0; k < B; ++k) buf[k] = fabs((double)spec[2 * (lo + k) + comp] - med[comp]);
+            scale[comp] = 1.4826 * orc_median_of_medians(buf, B);
+        }
+        for (int64_t k = lo; k < hi; ++k) {
+            double x = (scale[0] > 0.0 && isfinite(scale[0])) ? ((double)spec[2 * k] - med[0]) / scale[0] : 0.0;
+            double y = (scale[1] > 0.0 && isfinite(scale[1])) ? ((double)spec[2 * k + 1] - med[1]) / scale[1] : 0.0;
+            P[k] = 0.5 * (x * x + y * y);
+        }
+    }
+    free(buf);
+}
+
 /* Power S at which a width-w boxcar reaches ln p = lnp_target (used only to check threshold tables). */
 double orc_power_threshold(int32_t w, double lnp_target) {
     double lo = 0.0, hi = (double)w + 10.0;
@@ -302,9 +353,22 @@ int64_t orc_harmonic_sum(const double* P, int64_t n, int32_t H, double* Y) {
  * orc_search_ex, applied to each Y_H on its own (bins are those of Y_H, i.e. of the fundamental); a width needs
  * w < floor(n/H) to exist.  Records carry numharm = H and come out ordered by (H, spectrum, bin).  Normalisation happens
  * once, on the full-resolution spectrum, before the decimation (Table 4's kernel order L571-578). */
+int64_t orc_search_general(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                           int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                           int32_t r_block, int32_t numharm, int32_t norm_mode, orc_candidate* out, int64_t cap);
+
 int64_t orc_search_harmonics(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                              int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
                              int32_t r_block, int32_t numharm, orc_candidate* out, int64_t cap) {
+    return orc_search_general(spectra, batch, n, pitch, zmax, B, C, sigma_threshold, n_trials, z_step, log_sampling, r_block,
+                              numharm, 0, out, cap);
+}
+
+/* … and with norm_mode = 1 the normalisation is the paper's GPU one (Alg. 1, orc_normalise_power_mom) instead of the exact
+ * median/MAD; everything after the power spectrum is unchanged. */
+int64_t orc_search_general(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                           int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                           int32_t r_block, int32_t numharm, int32_t norm_mode, orc_candidate* out, int64_t cap) {
     double ln_trials = log(n_trials);
     double lnp_thr = orc_ln_sf(sigma_threshold);
     double* P = (double*)malloc((size_t)n * sizeof(double));
@@ -313,7 +377,8 @@ int64_t orc_search_harmonics(const float* spectra, int64_t batch, int64_t n, int
     for (int32_t H = 1; H <= numharm; ++H) {
         int32_t kappa = H * (H + 1) / 2;
         for (int64_t b = 0; b < batch; ++b) {
-            orc_normalise_power(spectra + 2 * b * pitch, n, B, P);
+            if (norm_mode) orc_normalise_power_mom(spectra + 2 * b * pitch, n, B, P);
+            else orc_normalise_power(spectra + 2 * b * pitch, n, B, P);
             int64_t nH = orc_harmonic_sum(P, n, H, Y);
             int64_t nblk = (nH + C - 1) / C;
             orc_candidate* blockbest = (orc_candidate*)malloc((size_t)nblk * sizeof(orc_candidate));
