@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--log10-p-flag", type=float, default=0.0)
     ap.add_argument("--numharm", type=int, default=1, help="also search the harmonic-summed spectra Y_2..Y_numharm "
                     "(PAPER.md:L201-220; pulscan_search_harmonics; not the headline)")
+    ap.add_argument("--fast-norm", action="store_true", help="the paper's approximate median-of-medians normalisation "
+                    "(Alg. 1, PAPER.md:L624-650) instead of the exact one (not the headline: results differ)")
     ap.add_argument("--z-step", type=int, default=1, help="search every z_step-th drift only (PAPER.md:L152; not the headline)")
     ap.add_argument("--log-sampling", action="store_true", help="search z = 0, 1, 2, 4, ... only (PAPER.md:L411; not the headline)")
     return ap.parse_args()
@@ -63,12 +65,13 @@ def workload(args):
 
 def config_dict(wl, n_gpus, args=None):
     sampling = "every width 1..zmax"
+    norm = "median of medians, Alg. 1 (approximate)" if (args is not None and args.fast_norm) else "exact median/MAD"
     if args is not None and args.log_sampling:
         sampling = "drifts z = 0, 1, 2, 4, ... (PAPER.md:L411)"
     elif args is not None and args.z_step != 1:
         sampling = f"every {args.z_step}-th drift (PAPER.md:L152)"
     return {
-        "widths_searched": sampling,
+        "widths_searched": sampling, "normalisation": norm,
         "workload": f"BASELINE.json configs[{int(wl.name[3]) - 1}] ({wl.name}): {wl.batch} spectra x {wl.n_bins} complex64 bins "
                     f"per GPU, zmax={wl.zmax}, norm_block={wl.norm_block}, block_width={wl.block_width}, "
                     f"sigma_threshold={wl.sigma_threshold}",
@@ -218,7 +221,7 @@ def run_ours(args):
 
     plan = binding.Plan(wl.n_bins, wl.batch, wl.zmax, wl.block_width, wl.sigma_threshold, norm_block=wl.norm_block,
                         tile=args.tile, log10_p_flag=args.log10_p_flag, z_step=args.z_step, log_sampling=args.log_sampling,
-                        numharm=args.numharm)
+                        numharm=args.numharm, median_of_medians=args.fast_norm)
     plan.attach(dev)
     run_search = plan.search_harmonics if args.numharm > 1 else plan.search
     plan.set_profiling(warm + steps)

@@ -115,6 +115,14 @@ int64_t pulscan_plan_max_hcandidates(const pulscan_plan* plan);
 int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_hcandidate* d_hcandidates, uint32_t* d_count,
                              void* cuda_stream);
 
+/* Normalisation method.  0 (default): exact median and MAD per block and component (L140-148, Eq. 8).  1: the paper's GPU
+ * method, Algorithm 1 "Median of Medians Normalisation" (L624-650; §2.5) — an approximation: the median of a chunk is
+ * estimated by recursively taking the median of 4 strided elements, the MAD likewise, scale factor 1.4826 (L648).  Needs
+ * norm_block = a power of two in [256, 16384] (set it first) and n_bins ≥ norm_block; the n_bins mod norm_block bins after
+ * the last chunk use the last chunk's statistics (reading R30).  Powers come out ≈ 12 % low in noise (the median of 4
+ * over-estimates the median of the skewed |deviation| distribution), so it is a fast mode, not the parity path. */
+int pulscan_plan_set_normalisation(pulscan_plan* plan, int32_t mode);
+
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
  * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);

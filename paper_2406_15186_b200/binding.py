@@ -32,6 +32,7 @@ SIGNATURES = {
     "pulscan_plan_set_pitch": (ctypes.c_int, [_P, ctypes.c_int64]),
     "pulscan_plan_set_mode": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_width_sampling": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int32]),
+    "pulscan_plan_set_normalisation": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_r_block": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_harmonics": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_max_hcandidates": (ctypes.c_int64, [_P]),
@@ -102,7 +103,8 @@ class Plan:
     def __init__(self, n_bins: int, batch: int, zmax: int, block_width: int, sigma_threshold: float,
                  norm_block: Optional[int] = None, n_trials: Optional[float] = None, pitch: Optional[int] = None,
                  mode: int = 0, tile: int = 0, log10_p_flag: float = 0.0, host_staging: bool = False,
-                 cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False, numharm: int = 1):
+                 cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False, numharm: int = 1,
+                 median_of_medians: bool = False):
         self.lib = load_library()
         self.n_bins, self.batch, self.zmax, self.block_width = int(n_bins), int(batch), int(zmax), int(block_width)
         self.handle = self.lib.pulscan_plan_create(n_bins, batch, zmax, block_width, sigma_threshold)
@@ -124,6 +126,8 @@ class Plan:
             _check(self.lib.pulscan_plan_set_width_sampling(self.handle, z_step, int(bool(log_sampling))))
         if r_block:
             _check(self.lib.pulscan_plan_set_r_block(self.handle, 1))
+        if median_of_medians:
+            _check(self.lib.pulscan_plan_set_normalisation(self.handle, 1))
         if numharm != 1:
             _check(self.lib.pulscan_plan_set_harmonics(self.handle, numharm))
         self.numharm = int(numharm)

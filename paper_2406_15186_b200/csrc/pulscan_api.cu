@@ -17,6 +17,7 @@
 #include "boxcar_sweep.cuh"
 #include "harmonic_sum.cuh"
 #include "norm_power.cuh"
+#include "norm_power_mom.cuh"
 #include "norm_power_v2.cuh"
 #include "significance.cuh"
 
@@ -64,6 +65,7 @@ struct pulscan_plan {
     double sigma_thr = 0, n_trials = 1.0;
     int64_t pitch = 0;
     int32_t mode = 0;
+    int32_t norm_mode = 0;                   // 0 exact median/MAD; 1 the paper's median-of-medians approximation (Alg. 1)
     int32_t numharm = 1;                     // harmonic-summed spectra searched by pulscan_search_harmonics (L201-220)
     int32_t shape_mult = 1;                  // H(H+1)/2 of the spectrum this plan searches: a width-w sum is Gamma(w·shape_mult)
     int32_t numharm_tag = 1;                 // the H written into pulscan_hcandidate records by this plan
@@ -488,6 +490,27 @@ int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStr
                  unsigned* d_redo_count) {
     const float2* spec = reinterpret_cast<const float2*>(d_spectra);
     int rc = PULSCAN_OK;
+    if (p.norm_mode == 1) {   // Alg. 1: one kernel for every chunk, the last one of a row included
+        const long long grid = (long long)p.nb * p.batch;
+        if (grid > 2147483647LL) return fail(PULSCAN_EINVAL, "too many normalisation blocks for one launch");
+#define PULSCAN_MOM_CASE(E, NT_)                                                                                      \
+    case (E) * (NT_):                                                                                                 \
+        norm_power_mom_kernel<E, NT_><<<(int)grid, NT_, 0, st>>>(spec, p.pitch, p.n, p.nb, d_power, p.pitchP);       \
+        break;
+        switch (p.B) {
+            PULSCAN_MOM_CASE(4, 64)
+            PULSCAN_MOM_CASE(4, 128)
+            PULSCAN_MOM_CASE(8, 128)
+            PULSCAN_MOM_CASE(16, 128)
+            PULSCAN_MOM_CASE(32, 128)
+            PULSCAN_MOM_CASE(32, 256)
+            PULSCAN_MOM_CASE(64, 256)
+            default: return fail(PULSCAN_EINVAL, "median-of-medians normalisation needs norm_block = 256 … 16384, a power of two");
+        }
+#undef PULSCAN_MOM_CASE
+        CUDA_TRY(cudaGetLastError());
+        return debug_sync("norm_power_mom_kernel");
+    }
     if (p.main_blocks_per_row > 0) {
         const long long grid = (long long)p.main_blocks_per_row * p.batch;
         if (grid > 2147483647LL) return fail(PULSCAN_EINVAL, "too many normalisation blocks for one launch");
@@ -629,6 +652,19 @@ int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t 
 int pulscan_plan_set_r_block(pulscan_plan* plan, int32_t enable) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     plan->r_block = enable != 0;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_normalisation(pulscan_plan* plan, int32_t mode) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (mode != 0 && mode != 1) return fail(PULSCAN_EINVAL, "mode must be 0 (exact median/MAD) or 1 (median of medians, Alg. 1)");
+    if (mode == 1) {
+        const int B = plan->B;
+        if (B < 256 || B > 16384 || (B & (B - 1)) != 0)
+            return fail(PULSCAN_EINVAL, "median-of-medians normalisation needs norm_block = 256 … 16384, a power of two (it is %d)", B);
+        if (plan->n < B) return fail(PULSCAN_EINVAL, "median-of-medians normalisation needs n_bins >= norm_block");
+    }
+    plan->norm_mode = mode;
     return PULSCAN_OK;
 }
 
@@ -886,7 +922,8 @@ int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_str
 int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan) {
     if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
     if (derive(*const_cast<pulscan_plan*>(plan))) return -1;
-    return (plan->main_blocks_per_row > 0 ? (plan->use_fast ? 2 : 1) : 0) + (plan->has_tail ? 1 : 0) + (plan->mode == 0 ? 3 : 2);
+    const int norm = plan->norm_mode == 1 ? 1 : (plan->main_blocks_per_row > 0 ? (plan->use_fast ? 2 : 1) : 0) + (plan->has_tail ? 1 : 0);
+    return norm + (plan->mode == 0 ? 3 : 2);
 }
 
 int pulscan_plan_set_profiling(pulscan_plan* plan, int32_t n_slots) {

@@ -68,6 +68,12 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_tuning(p.handle, 1000, 0.0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 2048, -1.0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_width_sampling(p.handle, 0, 0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_normalisation(p.handle, 2) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_norm_block(p.handle, 3000) == binding.PULSCAN_OK
+    assert lib.pulscan_plan_set_normalisation(p.handle, 1) == binding.PULSCAN_EINVAL      # Alg. 1 needs a power of two
+    assert lib.pulscan_plan_set_norm_block(p.handle, 1024) == binding.PULSCAN_OK
+    assert lib.pulscan_plan_set_normalisation(p.handle, 1) == binding.PULSCAN_OK
+    assert lib.pulscan_plan_set_normalisation(p.handle, 0) == binding.PULSCAN_OK
     assert lib.pulscan_plan_set_harmonics(p.handle, 0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_harmonics(p.handle, 5) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_cell_capacity(p.handle, -1) == binding.PULSCAN_EINVAL

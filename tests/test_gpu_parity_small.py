@@ -182,6 +182,41 @@ def test_harmonic_search_matches_oracle(orc, n, batch, zmax, B, C, thr, numharm,
     assert np.array_equal(h1["bin"], plain["bin"]) and np.array_equal(h1["sigma"], plain["sigma"])
 
 
+@pytest.mark.parametrize("n,B", [(4 * 256 + 3, 256), (3 * 512, 512), (5 * 1024 + 1000, 1024), (2 * 2048 + 1, 2048), (12289, 4096),
+                                 (16385, 8192), (40000, 16384)])
+def test_median_of_medians_power_matches_oracle(orc, n, B):
+    """Fast mode (Alg. 1): the kernel against the oracle's step-by-step Alg. 1."""
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(3, n, seed=n + B)
+    spec[1] = spec[1] * 1e-3 + (5.0 - 2.0j)     # offset and scale differ per row
+    plan = binding.Plan(n, 3, min(8, n - 1), 16, 6.0, norm_block=B, median_of_medians=True)
+    plan.attach("cuda")
+    P = plan.normalise_power(spec).cpu().numpy().astype(np.float64)
+    assert plan.launches_per_search == 4        # one normalisation kernel + sweep + refine + exact
+    plan.destroy()
+    for b in range(3):
+        ref = orc.normalise_power_mom(spec[b].cpu().numpy(), B)
+        err = np.abs(P[b] - ref)
+        assert np.all(err <= 1e-5 * ref + 1e-6), f"row {b}: max err {err.max()} at {err.argmax()} (ref {ref[err.argmax()]})"
+
+
+@pytest.mark.parametrize("n,batch,zmax,B,C,thr,numharm", [(20001, 2, 40, 2048, 100, 4.0, 1), (9001, 2, 100, 4096, 200, 4.0, 3),
+                                                          (32769, 1, 32, 1024, 64, 4.0, 1)])
+def test_search_with_median_of_medians_matches_oracle(orc, n, batch, zmax, B, C, thr, numharm):
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(batch, n, seed=n * 3 + zmax)
+    bump(spec, 0, n // 3, 6, 3.0)
+    bump(spec, batch - 1, n // 2, min(zmax, 60), 1.8)
+    plan = binding.Plan(n, batch, zmax, C, thr, norm_block=B, numharm=numharm, median_of_medians=True)
+    plan.attach("cuda")
+    plan.search_harmonics(spec)
+    gpu = plan.hcandidates()
+    plan.destroy()
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, numharm, median_of_medians=True)
+    assert len(ora) > 0
+    _assert_same_hcandidates(gpu, ora, f"median of medians n={n} numharm={numharm}")
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)
