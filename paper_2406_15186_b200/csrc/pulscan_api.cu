@@ -72,6 +72,7 @@ struct pulscan_plan {
     bool is_child = false;                   // a plan for one Y_H, owned by the plan the user created; it never normalises
     std::vector<pulscan_plan*> harm;         // children for H = 2..numharm
     size_t off_child = 0, child_ws_bytes = 0;
+    std::vector<size_t> child_off;           // offset of each child's region inside [off_child, off_child + child_ws_bytes)
     int32_t r_block = 0;                     // report the candidate block's first bin instead of the exact bin (L222-226)
     int32_t z_step = 1, log_sampling = 0;   // which widths are searched (all are summed): Alg. 4
     int32_t tile_user = 0;
@@ -134,6 +135,13 @@ float round_down_float(double x) {
 // float32 rounding of the addends themselves.
 float conservative_threshold(double T, int terms) {
     return round_down_float(T * (1.0 - 2.0 * (double)terms * 5.9604644775390625e-8 - 2e-6));
+}
+
+void attach_children(pulscan_plan& p) {
+    for (size_t k = 0; k < p.harm.size(); ++k) {
+        p.harm[k]->ws = static_cast<char*>(p.ws) + p.off_child + p.child_off[k];
+        p.harm[k]->ws_bytes = align_up(p.harm[k]->need_bytes, 256);
+    }
 }
 
 int derive(pulscan_plan& p) {
@@ -334,11 +342,11 @@ int derive(pulscan_plan& p) {
         p.off_stage_cand = o; o += align_up((size_t)p.batch * p.nblk * sizeof(pulscan_candidate), 256);
         p.off_stage_count = o; o += 256;
     }
-    // ---- harmonic-summed spectra: one child plan per H = 2..numharm; they run one after the other, so they share one
-    //      region of the workspace, sized for H = 2 (a child's own "power" buffer is Y_H)
+    // ---- harmonic-summed spectra: one child plan per H = 2..numharm, each with its own region of the workspace (a child's
+    //      "power" buffer is Y_H)
     for (pulscan_plan* c : p.harm) pulscan_plan_destroy(c);
     p.harm.clear();
-    p.off_child = o; p.child_ws_bytes = 0;
+    p.off_child = o; p.child_ws_bytes = 0; p.child_off.clear();
     for (int H = 2; H <= p.numharm && !p.is_child; ++H) {
         const int64_t nH = p.n / H;
         if ((int64_t)p.zmax >= nH) return fail(PULSCAN_EINVAL, "zmax = %d must be < floor(n_bins / %d) = %lld", p.zmax, H, (long long)nH);
@@ -350,13 +358,13 @@ int derive(pulscan_plan& p) {
         p.harm.push_back(c);
         const int rc = derive(*c);
         if (rc) return rc;
-        p.child_ws_bytes = std::max(p.child_ws_bytes, align_up(c->need_bytes, 256));
+        p.child_off.push_back(p.child_ws_bytes);                   // every Y_H keeps its own buffer: one decimation pass writes all
+        p.child_ws_bytes += align_up(c->need_bytes, 256);
     }
     o += p.child_ws_bytes;
     p.need_bytes = o;
     p.dirty = false;
-    if (p.ws && p.ws_bytes >= p.need_bytes)
-        for (pulscan_plan* c : p.harm) { c->ws = static_cast<char*>(p.ws) + p.off_child; c->ws_bytes = p.child_ws_bytes; }
+    if (p.ws && p.ws_bytes >= p.need_bytes) attach_children(p);
     return PULSCAN_OK;
 }
 
@@ -576,9 +584,8 @@ int check_plan_ready(pulscan_plan* plan) {
     if (!plan->ws) return fail(PULSCAN_ENOWORKSPACE, "no workspace attached (pulscan_plan_set_workspace)");
     if (plan->ws_bytes < plan->need_bytes)
         return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes attached, %zu needed", plan->ws_bytes, plan->need_bytes);
+    attach_children(*plan);
     for (pulscan_plan* c : plan->harm) {
-        c->ws = static_cast<char*>(plan->ws) + plan->off_child; c->ws_bytes = plan->child_ws_bytes;
-        c->sm_count = plan->sm_count;
         if ((rc = ensure_device(*c))) return rc;
     }
     return ensure_device(*plan);
@@ -713,7 +720,7 @@ int pulscan_plan_set_workspace(pulscan_plan* plan, void* d_workspace, size_t byt
     if (bytes < plan->need_bytes)
         return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes given, %zu needed", bytes, plan->need_bytes);
     plan->ws = d_workspace; plan->ws_bytes = bytes;
-    for (pulscan_plan* c : plan->harm) { c->ws = static_cast<char*>(d_workspace) + plan->off_child; c->ws_bytes = plan->child_ws_bytes; }
+    attach_children(*plan);
     return PULSCAN_OK;
 }
 
@@ -817,23 +824,30 @@ int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_
     rc = enqueue_norm(p, d_spectra, d_P, st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1);      // (a)
     if (rc) return rc;
     if ((rc = enqueue_sweep_exact(p, d_P, nullptr, d_hcandidates, d_count, st, nullptr))) return rc;           // Y_1 = P
-    for (pulscan_plan* cp : p.harm) {                                                                            // Y_2 …
-        pulscan_plan& c = *cp;
-        c.mode = p.mode; c.r_block = p.r_block;
-        char* cws = static_cast<char*>(c.ws);
-        float* d_Y = reinterpret_cast<float*>(cws + c.off_P);
-        CUDA_TRY(cudaMemsetAsync(cws + c.off_bitmap, 0, c.bitmap_bytes, st));
-        CUDA_TRY(cudaMemsetAsync(cws + c.off_counters, 0, 256, st));
-        const long long total = (long long)c.batch * c.n;
+    if (!p.harm.empty()) {                                                                                      // Y_2 … in one pass
+        HarmonicOut ho{};
+        for (size_t k = 0; k < p.harm.size(); ++k) {
+            pulscan_plan& c = *p.harm[k];
+            ho.Y[k] = reinterpret_cast<float*>(static_cast<char*>(c.ws) + c.off_P);
+            ho.pitch[k] = c.pitchP; ho.nH[k] = c.n;
+        }
+        const long long total = (long long)p.batch * ho.nH[0];
         const int grid = (int)std::min<long long>((total + kHarmThreads - 1) / kHarmThreads, (long long)p.sm_count * 16);
-        switch (c.numharm_tag) {
-            case 2: harmonic_sum_kernel<2><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, d_Y, c.pitchP, c.n, total); break;
-            case 3: harmonic_sum_kernel<3><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, d_Y, c.pitchP, c.n, total); break;
-            default: harmonic_sum_kernel<4><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, d_Y, c.pitchP, c.n, total); break;
+        switch ((int)p.harm.size() + 1) {
+            case 2: harmonic_sum_kernel<2><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, ho, total); break;
+            case 3: harmonic_sum_kernel<3><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, ho, total); break;
+            default: harmonic_sum_kernel<4><<<grid, kHarmThreads, 0, st>>>(d_P, p.pitchP, ho, total); break;
         }
         CUDA_TRY(cudaGetLastError());
         if ((rc = debug_sync("harmonic_sum_kernel"))) return rc;
-        if ((rc = enqueue_sweep_exact(c, d_Y, nullptr, d_hcandidates, d_count, st, nullptr))) return rc;
+    }
+    for (pulscan_plan* cp : p.harm) {
+        pulscan_plan& c = *cp;
+        c.mode = p.mode; c.r_block = p.r_block;
+        char* cws = static_cast<char*>(c.ws);
+        CUDA_TRY(cudaMemsetAsync(cws + c.off_bitmap, 0, c.bitmap_bytes, st));
+        CUDA_TRY(cudaMemsetAsync(cws + c.off_counters, 0, 256, st));
+        if ((rc = enqueue_sweep_exact(c, reinterpret_cast<float*>(cws + c.off_P), nullptr, d_hcandidates, d_count, st, nullptr))) return rc;
     }
     return PULSCAN_OK;
 }
