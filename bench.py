@@ -251,7 +251,7 @@ def run_ours(args):
                               "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                               "dtype": "f32", "data": "synthetic", "config": dict(config_dict(wl, world, args), numharm=args.numharm),
                               "bin_widths_per_sec": value * wl.zmax, "candidates_per_step": n_cand, "clocks": clk.summary(),
-                              "gpu_launches": (plan.launches_per_search + 4 * (args.numharm - 1)) * steps}), flush=True)
+                              "gpu_launches": (plan.launches_per_search + 1 + 3 * (args.numharm - 1)) * steps}), flush=True)
         plan.destroy()
         if world > 1:
             tdist.destroy_process_group()

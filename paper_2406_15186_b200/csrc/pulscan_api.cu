@@ -893,6 +893,11 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
              "pulscan plan: n_bins=%lld batch=%d zmax=%d block_width=%d norm_block=%d sigma_threshold=%g n_trials=%g pitch=%lld mode=%s\n",
              (long long)p.n, p.batch, p.zmax, p.C, p.B, p.sigma_thr, p.n_trials, (long long)p.pitch, p.mode ? "exhaustive" : "pruned");
     s += line;
+    snprintf(line, sizeof line, "options: widths searched = %s, location = %s, normalisation = %s, numharm = %d\n",
+             p.log_sampling ? "z = 0, 1, 2, 4, ... (L411)" : (p.z_step == 1 ? "every width" : "every z_step-th drift (L152)"),
+             p.r_block ? "R-Block (L222-226)" : "exact bin", p.norm_mode ? "median of medians (Alg. 1)" : "exact median/MAD",
+             p.numharm);
+    s += line;
     snprintf(line, sizeof line, "norm: %d blocks/row, main %s<EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.use_fast ? "single-histogram" : "general",
              p.use_fast ? p.B / p.norm_nt : p.ept_main, p.use_fast ? p.norm_nt : p.nt_main, p.main_blocks_per_row,
              p.has_tail ? "" : " (no tail launch)");
