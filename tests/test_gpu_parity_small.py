@@ -160,7 +160,7 @@ def _assert_same_hcandidates(gpu, ora, context):
 @pytest.mark.parametrize("mode", [0, 1])
 @pytest.mark.parametrize("n,batch,zmax,B,C,thr,numharm,log_sampling", [
     (20001, 2, 40, 2048, 100, 4.0, 4, False), (9001, 2, 200, 4096, 200, 4.0, 3, False), (30011, 1, 64, 8192, 300, 4.5, 4, True),
-    (4099, 3, 16, 1024, 64, 3.5, 2, False)])
+    (4099, 3, 16, 1024, 64, 3.5, 2, False), (40001, 1, 600, 8192, 700, 4.5, 2, False)])   # the last: 8192-bin tiles, two scan passes
 def test_harmonic_search_matches_oracle(orc, n, batch, zmax, B, C, thr, numharm, log_sampling, mode):
     from paper_2406_15186_b200 import binding
     spec = noise_spectra(batch, n, seed=n + numharm)
