@@ -123,6 +123,13 @@ int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_
  * over-estimates the median of the skewed |deviation| distribution), so it is a fast mode, not the parity path. */
 int pulscan_plan_set_normalisation(pulscan_plan* plan, int32_t mode);
 
+/* What is emitted per candidate block.  per_width = 0 (default): the width with the largest σ (step 6 above, R13), at most
+ * one record per block.  per_width = 1: the paper's GPU output, one record per (block, searched width) whose maximum reaches
+ * the threshold (Alg. 4 "write out local candidate", ranked by σ afterwards, L322) — `capacity` records must then
+ * be provided for d_candidates / d_hcandidates (pulscan_plan_max_candidates() returns it); *d_count reports the number
+ * found and only the first `capacity` of them are written. */
+int pulscan_plan_set_emission(pulscan_plan* plan, int32_t per_width, int64_t capacity);
+
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
  * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);

@@ -85,6 +85,11 @@ def _load():
         lib.orc_search_general.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                            ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
                                            ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64]
+        lib.orc_search_opts.restype = ctypes.c_int64
+        lib.orc_search_opts.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                        ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
+                                        ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p,
+                                        ctypes.c_int64]
         lib.orc_search.restype = ctypes.c_int64
         lib.orc_search.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                    ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64]
@@ -217,22 +222,24 @@ def harmonic_sum(P, H: int) -> np.ndarray:
 
 def search_harmonics(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshold: float, numharm: int,
                      n_trials: float = 1.0, n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False,
-                     r_block: bool = False, median_of_medians: bool = False) -> np.ndarray:
+                     r_block: bool = False, median_of_medians: bool = False, per_width: bool = False) -> np.ndarray:
     """The search on every harmonic-summed spectrum Y_1 … Y_numharm (§2.3): records carry `numharm`; ordered by
-    (numharm, spectrum, bin); at most one per candidate block of each summed spectrum."""
+    (numharm, spectrum, bin); at most one per candidate block of each summed spectrum — or, with per_width, one per
+    (block, searched width) above the threshold (Alg. 4), ordered by (numharm, spectrum, block, width)."""
     s = np.ascontiguousarray(spectra, dtype=np.complex64)
     if s.ndim == 1:
         s = s[None, :]
     batch, pitch = s.shape
     n = pitch if n_bins is None else int(n_bins)
     C = int(block_width)
-    cap = sum(batch * ((n // H + C - 1) // C) for H in range(1, int(numharm) + 1))
+    cap = sum(batch * ((n // H + C - 1) // C) for H in range(1, int(numharm) + 1)) * (int(zmax) if per_width else 1)
     out = np.zeros(cap, dtype=CANDIDATE_DTYPE)
     f = s.view(np.float32)
-    found = _load().orc_search_general(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
-                                       int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
-                                       int(bool(log_sampling)), int(bool(r_block)), int(numharm),
-                                       int(bool(median_of_medians)), out.ctypes.data_as(ctypes.c_void_p), cap)
+    found = _load().orc_search_opts(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
+                                    int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
+                                    int(bool(log_sampling)), int(bool(r_block)), int(numharm),
+                                    int(bool(median_of_medians)), int(bool(per_width)),
+                                    out.ctypes.data_as(ctypes.c_void_p), cap)
     return out[: int(found)].copy()
 
 

@@ -366,9 +366,23 @@ int64_t orc_search_harmonics(const float* spectra, int64_t batch, int64_t n, int
 
 /* … and with norm_mode = 1 the normalisation is the paper's GPU one (Alg. 1, orc_normalise_power_mom) instead of the exact
  * median/MAD; everything after the power spectrum is unchanged. */
+int64_t orc_search_opts(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                        int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                        int32_t r_block, int32_t numharm, int32_t norm_mode, int32_t per_width, orc_candidate* out, int64_t cap);
+
 int64_t orc_search_general(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                            int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
                            int32_t r_block, int32_t numharm, int32_t norm_mode, orc_candidate* out, int64_t cap) {
+    return orc_search_opts(spectra, batch, n, pitch, zmax, B, C, sigma_threshold, n_trials, z_step, log_sampling, r_block,
+                           numharm, norm_mode, 0, out, cap);
+}
+
+/* … and with per_width != 0 the paper's GPU output: instead of the best width per block (R13), one record per
+ * (block, searched width) whose maximum reaches the threshold (Alg. 4: thread 0 "writes out [the] local candidate"
+ * of every searched z; L322 "highest sigma candidate" is picked afterwards).  Ordered by (H, spectrum, block, width). */
+int64_t orc_search_opts(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                        int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                        int32_t r_block, int32_t numharm, int32_t norm_mode, int32_t per_width, orc_candidate* out, int64_t cap) {
     double ln_trials = log(n_trials);
     double lnp_thr = orc_ln_sf(sigma_threshold);
     double* P = (double*)malloc((size_t)n * sizeof(double));
@@ -415,12 +429,35 @@ int64_t orc_search_general(const float* spectra, int64_t batch, int64_t n, int64
                 }
                 free(sums); free(M); free(I);
             }
-            for (int64_t c = 0; c < nblk; ++c) {
+            for (int64_t c = 0; c < nblk && !per_width; ++c) {
                 if (blockbest[c].spectrum < 0) continue;
                 if (found < cap) out[found] = blockbest[c];
                 ++found;
             }
             free(blockbest);
+            if (per_width) { /* plain serial loop: every (block, searched width) above the threshold */
+                double* sums = (double*)malloc((size_t)C * sizeof(double));
+                double* M = (double*)malloc((size_t)zmax * sizeof(double));
+                int64_t* I = (int64_t*)malloc((size_t)zmax * sizeof(int64_t));
+                for (int64_t c = 0; c < nblk; ++c) {
+                    orc_block_maxima(Y, nH, zmax, C, c, sums, M, I);
+                    for (int32_t w = 1; w <= zmax; ++w) {
+                        if (I[w - 1] < 0 || !orc_width_searched(w, z_step, log_sampling)) continue;
+                        double lnp = orc_ln_q(w * kappa, M[w - 1]) + ln_trials;
+                        if (lnp > 0.0) lnp = 0.0;
+                        if (lnp > lnp_thr) continue;
+                        orc_candidate r;
+                        memset(&r, 0, sizeof r);
+                        r.spectrum = (int32_t)b;
+                        r.bin = r_block ? (int32_t)(c * C) : (int32_t)I[w - 1];
+                        r.width = w; r.numharm = H; r.power = M[w - 1]; r.lnp = lnp;
+                        r.sigma = orc_sigma_from_lnp(lnp);
+                        if (found < cap) out[found] = r;
+                        ++found;
+                    }
+                }
+                free(sums); free(M); free(I);
+            }
         }
     }
     free(P); free(Y);

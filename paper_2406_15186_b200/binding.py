@@ -34,6 +34,7 @@ SIGNATURES = {
     "pulscan_plan_set_width_sampling": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int32]),
     "pulscan_plan_set_normalisation": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_r_block": (ctypes.c_int, [_P, ctypes.c_int32]),
+    "pulscan_plan_set_emission": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int64]),
     "pulscan_plan_set_harmonics": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_max_hcandidates": (ctypes.c_int64, [_P]),
     "pulscan_search_harmonics": (ctypes.c_int, [_P, _P, _P, _P, _P]),
@@ -104,7 +105,7 @@ class Plan:
                  norm_block: Optional[int] = None, n_trials: Optional[float] = None, pitch: Optional[int] = None,
                  mode: int = 0, tile: int = 0, log10_p_flag: float = 0.0, host_staging: bool = False,
                  cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False, numharm: int = 1,
-                 median_of_medians: bool = False):
+                 median_of_medians: bool = False, per_width_capacity: int = 0):
         self.lib = load_library()
         self.n_bins, self.batch, self.zmax, self.block_width = int(n_bins), int(batch), int(zmax), int(block_width)
         self.handle = self.lib.pulscan_plan_create(n_bins, batch, zmax, block_width, sigma_threshold)
@@ -126,6 +127,9 @@ class Plan:
             _check(self.lib.pulscan_plan_set_width_sampling(self.handle, z_step, int(bool(log_sampling))))
         if r_block:
             _check(self.lib.pulscan_plan_set_r_block(self.handle, 1))
+        if per_width_capacity:
+            _check(self.lib.pulscan_plan_set_emission(self.handle, 1, per_width_capacity))
+        self.capacity = int(per_width_capacity)
         if median_of_medians:
             _check(self.lib.pulscan_plan_set_normalisation(self.handle, 1))
         if numharm != 1:
@@ -209,17 +213,19 @@ class Plan:
 
     def hcandidates(self) -> np.ndarray:
         """Synchronise and return the records of the last search_harmonics, sorted by (numharm, spectrum, bin)."""
-        n = int(self.d_count.item())
+        n = self.last_count = int(self.d_count.item())
+        n = min(n, self.capacity) if self.capacity else n
         raw = self.d_hcandidates[: n * HCANDIDATE_DTYPE.itemsize].cpu().numpy()
         rec = raw.view(HCANDIDATE_DTYPE).copy()
-        return rec[np.lexsort((rec["bin"], rec["spectrum"], rec["numharm"]))]
+        return rec[np.lexsort((rec["width"], rec["bin"], rec["spectrum"], rec["numharm"]))]
 
     def candidates(self) -> np.ndarray:
         """Synchronise and return the records of the last search, sorted by (spectrum, bin)."""
-        n = int(self.d_count.item())
+        n = self.last_count = int(self.d_count.item())     # with per-width emission: the number found, possibly > capacity
+        n = min(n, self.capacity) if self.capacity else n
         raw = self.d_candidates[: n * CANDIDATE_DTYPE.itemsize].cpu().numpy()
         rec = raw.view(CANDIDATE_DTYPE).copy()
-        return rec[np.lexsort((rec["bin"], rec["spectrum"]))]
+        return rec[np.lexsort((rec["width"], rec["bin"], rec["spectrum"]))]
 
     def search_host(self, h_spectra: torch.Tensor, h_candidates: Optional[np.ndarray] = None,
                     stream: Optional[torch.cuda.Stream] = None) -> np.ndarray:

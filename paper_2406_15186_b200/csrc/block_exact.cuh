@@ -31,10 +31,30 @@ struct ExactSmemHdr {
     double best_s[kExactThreads / 32];
 };
 
+// Append one record (20-byte or, for the harmonic search, 24-byte); records beyond `capacity` are counted, not written.
+__device__ __forceinline__ void emit_candidate(long long row, int32_t bin, int w, double S, double lnp, int numharm,
+                                               pulscan_candidate* __restrict__ out, pulscan_hcandidate* __restrict__ out_h,
+                                               unsigned* __restrict__ out_count, unsigned capacity) {
+    const float sigma = (float)sigma_from_lnp(lnp);
+    const unsigned slot = atomicAdd(out_count, 1u);
+    if (slot >= capacity) return;
+    if (out_h) {
+        pulscan_hcandidate r;
+        r.spectrum = (int32_t)row; r.bin = bin; r.width = w; r.numharm = numharm;
+        r.power = (float)S; r.sigma = sigma;
+        out_h[slot] = r;
+    } else {
+        pulscan_candidate r;
+        r.spectrum = (int32_t)row; r.bin = bin; r.width = w;
+        r.power = (float)S; r.sigma = sigma;
+        out[slot] = r;
+    }
+}
+
 __global__ void __launch_bounds__(kExactThreads)
 block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, int zmax, int C, long long nblk,
                    const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int numharm,
-                   pulscan_hcandidate* __restrict__ out_h,
+                   pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity,
                    const unsigned* __restrict__ flagged, const unsigned* __restrict__ counters,
                    pulscan_candidate* __restrict__ out, unsigned* __restrict__ out_count) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -102,7 +122,10 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
             if (arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
                 double lnp = ln_q(w * shape_mult, best) + ln_trials;   // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220)
                 if (lnp > 0.0) lnp = 0.0;
-                if (lnp < my_lnp) { my_lnp = lnp; my_w = w; my_i = arg; my_s = best; } // ascending w: ties keep the smaller
+                if (per_width) {   // the paper's GPU output: one candidate per (block, searched width) above the threshold (Alg. 4)
+                    if (lnp <= lnp_thr)
+                        emit_candidate(row, r_block ? (int32_t)lo : (int32_t)(lo + arg), w, best, lnp, numharm, out, out_h, out_count, capacity);
+                } else if (lnp < my_lnp) { my_lnp = lnp; my_w = w; my_i = arg; my_s = best; } // ascending w: ties keep the smaller
             }
         }
         // block arg-min over (ln p, w)
@@ -126,22 +149,8 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
                     my_lnp = ol; my_w = ow; my_i = hdr.best_i[q]; my_s = hdr.best_s[q];
                 }
             }
-            if (my_w > 0 && my_lnp <= lnp_thr) {
-                const int32_t bin = r_block ? (int32_t)lo : (int32_t)(lo + my_i);   // R-Block: block index × block width (L222-226)
-                const float sigma = (float)sigma_from_lnp(my_lnp);
-                const unsigned slot = atomicAdd(out_count, 1u);
-                if (out_h) {
-                    pulscan_hcandidate r;
-                    r.spectrum = (int32_t)row; r.bin = bin; r.width = my_w; r.numharm = numharm;
-                    r.power = (float)my_s; r.sigma = sigma;
-                    out_h[slot] = r;
-                } else {
-                    pulscan_candidate r;
-                    r.spectrum = (int32_t)row; r.bin = bin; r.width = my_w;
-                    r.power = (float)my_s; r.sigma = sigma;
-                    out[slot] = r;
-                }
-            }
+            if (my_w > 0 && my_lnp <= lnp_thr)   // R-Block: block index × block width (L222-226)
+                emit_candidate(row, r_block ? (int32_t)lo : (int32_t)(lo + my_i), my_w, my_s, my_lnp, numharm, out, out_h, out_count, capacity);
         }
         __syncthreads();
     }

@@ -65,6 +65,9 @@ struct pulscan_plan {
     double sigma_thr = 0, n_trials = 1.0;
     int64_t pitch = 0;
     int32_t mode = 0;
+    int32_t per_width = 0;                   // emit one candidate per (block, searched width) instead of the best width per block
+    unsigned out_capacity = 0xFFFFFFFFu;     // records the output array can hold (per-width emission only; otherwise never exceeded)
+    int64_t user_capacity = 0;
     int32_t norm_mode = 0;                   // 0 exact median/MAD; 1 the paper's median-of-medians approximation (Alg. 1)
     int32_t numharm = 1;                     // harmonic-summed spectra searched by pulscan_search_harmonics (L201-220)
     int32_t shape_mult = 1;                  // H(H+1)/2 of the spectrum this plan searches: a width-w sum is Gamma(w·shape_mult)
@@ -571,7 +574,7 @@ int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candid
     const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
     const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
     block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
-                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.numharm_tag, d_hcandidates,
+                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity,
                                                                    d_flagged, d_counters, d_candidates, d_count);
     CUDA_TRY(cudaGetLastError());
     return PULSCAN_OK;
@@ -675,6 +678,16 @@ int pulscan_plan_set_normalisation(pulscan_plan* plan, int32_t mode) {
     return PULSCAN_OK;
 }
 
+int pulscan_plan_set_emission(pulscan_plan* plan, int32_t per_width, int64_t capacity) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (per_width != 0 && per_width != 1) return fail(PULSCAN_EINVAL, "per_width must be 0 or 1");
+    if (per_width && (capacity < 1 || capacity > 0x7FFFFFFFll)) return fail(PULSCAN_EINVAL, "per-width emission needs a capacity in [1, 2^31)");
+    plan->per_width = per_width;
+    plan->user_capacity = per_width ? capacity : 0;
+    plan->out_capacity = per_width ? (unsigned)capacity : 0xFFFFFFFFu;
+    return PULSCAN_OK;
+}
+
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (tile_bins != 0 && (tile_bins < 1024 || tile_bins > 16384 || tile_bins % 512 != 0))
@@ -696,6 +709,7 @@ int pulscan_plan_set_cell_capacity(pulscan_plan* plan, int64_t cells) {
 
 int64_t pulscan_plan_max_candidates(const pulscan_plan* plan) {
     if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    if (plan->per_width) return plan->user_capacity;
     return (int64_t)plan->batch * ((plan->n + plan->C - 1) / plan->C);
 }
 
@@ -800,6 +814,7 @@ int pulscan_plan_set_harmonics(pulscan_plan* plan, int32_t numharm) {
 
 int64_t pulscan_plan_max_hcandidates(const pulscan_plan* plan) {
     if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    if (plan->per_width) return plan->user_capacity;
     int64_t total = 0;
     for (int H = 1; H <= plan->numharm; ++H) total += (int64_t)plan->batch * ((plan->n / H + plan->C - 1) / plan->C);
     return total;
@@ -843,7 +858,7 @@ int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_
     }
     for (pulscan_plan* cp : p.harm) {
         pulscan_plan& c = *cp;
-        c.mode = p.mode; c.r_block = p.r_block;
+        c.mode = p.mode; c.r_block = p.r_block; c.per_width = p.per_width; c.out_capacity = p.out_capacity;
         char* cws = static_cast<char*>(c.ws);
         CUDA_TRY(cudaMemsetAsync(cws + c.off_bitmap, 0, c.bitmap_bytes, st));
         CUDA_TRY(cudaMemsetAsync(cws + c.off_counters, 0, 256, st));

@@ -74,6 +74,9 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_norm_block(p.handle, 1024) == binding.PULSCAN_OK
     assert lib.pulscan_plan_set_normalisation(p.handle, 1) == binding.PULSCAN_OK
     assert lib.pulscan_plan_set_normalisation(p.handle, 0) == binding.PULSCAN_OK
+    assert lib.pulscan_plan_set_emission(p.handle, 1, 0) == binding.PULSCAN_EINVAL         # per-width output needs a capacity
+    assert lib.pulscan_plan_set_emission(p.handle, 1, 1234) == binding.PULSCAN_OK and p.max_candidates == 1234
+    assert lib.pulscan_plan_set_emission(p.handle, 0, 0) == binding.PULSCAN_OK and p.max_candidates == 2 * 200
     assert lib.pulscan_plan_set_harmonics(p.handle, 0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_harmonics(p.handle, 5) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_cell_capacity(p.handle, -1) == binding.PULSCAN_EINVAL

@@ -217,6 +217,36 @@ def test_search_with_median_of_medians_matches_oracle(orc, n, batch, zmax, B, C,
     _assert_same_hcandidates(gpu, ora, f"median of medians n={n} numharm={numharm}")
 
 
+@pytest.mark.parametrize("numharm,log_sampling", [(1, False), (1, True), (3, False)])
+def test_per_width_emission_matches_oracle(orc, numharm, log_sampling):
+    """The paper's GPU output (Alg. 4): one record per (block, searched width) above the threshold."""
+    from paper_2406_15186_b200 import binding
+    n, batch, zmax, B, C, thr = 20001, 2, 40, 2048, 100, 4.0
+    spec = noise_spectra(batch, n, seed=777)
+    bump(spec, 0, n // 3, 6, 3.0)
+    bump(spec, 1, n // 2, 30, 1.8)
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, numharm, log_sampling=log_sampling, per_width=True)
+    ora = ora[np.lexsort((ora["width"], ora["bin"], ora["spectrum"], ora["numharm"]))]
+    plan = binding.Plan(n, batch, zmax, C, thr, norm_block=B, numharm=numharm, log_sampling=log_sampling,
+                        per_width_capacity=len(ora) + 10)
+    plan.attach("cuda")
+    assert plan.max_hcandidates == plan.max_candidates == len(ora) + 10
+    plan.search_harmonics(spec)
+    gpu = plan.hcandidates()
+    assert plan.last_count == len(ora) > 20
+    _assert_same_hcandidates(gpu, ora, f"per-width numharm={numharm} log={log_sampling}")
+    plan.destroy()
+    # too small an array: the count still reports everything found, only `capacity` records are written (all genuine)
+    small = binding.Plan(n, batch, zmax, C, thr, norm_block=B, numharm=numharm, log_sampling=log_sampling, per_width_capacity=7)
+    small.attach("cuda")
+    small.search_harmonics(spec)
+    part = small.hcandidates()
+    assert small.last_count == len(ora) and len(part) == 7
+    keys = set(zip(ora["numharm"].tolist(), ora["spectrum"].tolist(), ora["bin"].tolist(), ora["width"].tolist()))
+    assert all(k in keys for k in zip(part["numharm"].tolist(), part["spectrum"].tolist(), part["bin"].tolist(), part["width"].tolist()))
+    small.destroy()
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)

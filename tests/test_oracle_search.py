@@ -102,6 +102,27 @@ def test_r_block_reports_block_index_times_width(orc):
         assert np.array_equal(approx[f], exact[f])
 
 
+def test_per_width_emission_is_every_block_width_above_threshold(orc):
+    # Alg. 4: one candidate per (chunk, searched z); L322: the highest sigma one is picked afterwards
+    n, zmax, B, C, thr = 1025, 12, 256, 64, 2.5
+    rng = np.random.default_rng(21)
+    spec = (rng.normal(0, 30, n) + 1j * rng.normal(0, 30, n)).astype(np.complex64)
+    spec[300:306] *= 3.5
+    allw = orc.search_harmonics(spec, zmax, B, C, thr, 1, per_width=True)
+    best = orc.search(spec, zmax, B, C, thr)
+    M, I = orc.block_maxima(orc.normalise_power(spec, B), zmax, C)
+    want = []
+    for c in range(M.shape[0]):
+        for w in range(1, zmax + 1):
+            if I[c, w - 1] >= 0 and stats.chi2.logsf(2 * M[c, w - 1], 2 * w) <= special.log_ndtr(-thr):
+                want.append((int(I[c, w - 1]), w))
+    assert list(zip(allw["bin"].tolist(), allw["width"].tolist())) == want and len(want) > len(best)
+    for r in best:                                             # the default output = the highest-sigma record of each block
+        mine = allw[allw["bin"] // C == r["bin"] // C]
+        top = mine[np.argmax(mine["sigma"])]
+        assert (top["bin"], top["width"]) == (r["bin"], r["width"]) and top["sigma"] == r["sigma"]
+
+
 def test_bonferroni_trials_shift(orc):
     rng = np.random.default_rng(4)
     spec = (rng.normal(0, 1, 600) + 1j * rng.normal(0, 1, 600)).astype(np.complex64)
