@@ -247,6 +247,28 @@ def test_per_width_emission_matches_oracle(orc, numharm, log_sampling):
     small.destroy()
 
 
+def test_time_series_pipeline_on_one_stream(orc):
+    """cuFFT (torch.fft.rfft) feeding pulscan_search on a side stream: the oracle gets the spectrum the search saw."""
+    from paper_2406_15186_b200 import binding, pipeline
+    wl = synth.CONFIGS[1]
+    g = torch.Generator(device="cpu").manual_seed(11)
+    t = torch.arange(wl.n_samples, dtype=torch.float64) * wl.tsamp
+    x = torch.randn(2, wl.n_samples, generator=g, dtype=torch.float32)
+    x[1] += (0.08 * torch.cos(2 * torch.pi * (173.2 * t + 0.5 * (12 / wl.t_obs ** 2) * t ** 2))).float()
+    plan = binding.Plan(wl.n_bins, 2, wl.zmax, wl.block_width, 5.0, norm_block=wl.norm_block)
+    plan.attach("cuda")
+    side = torch.cuda.Stream()
+    xd = x.cuda()
+    side.wait_stream(torch.cuda.current_stream())
+    spectrum = pipeline.search_time_series(plan, xd, side)
+    side.synchronize()
+    gpu = plan.candidates()
+    plan.destroy()
+    ora = oracle_search(orc, spectrum, wl.zmax, wl.norm_block, wl.block_width, 5.0)
+    assert len(ora) > 0 and ora[np.argmax(ora["sigma"])]["spectrum"] == 1
+    assert_same_candidates(gpu, ora, "time series -> rfft -> search on one stream")
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)
