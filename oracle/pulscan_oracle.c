@@ -11,8 +11,12 @@
  *
  * Parity pins (tests/test_oracle_*.py): numpy.median / scipy MAD / Φ⁻¹(¾); brute-force and closed-form
  * boxcar sums; mpmath 50-digit χ² tails and normal quantiles (tests/golden/significance_pins.txt);
- * scipy.special.gammaincc / chi2.sf / norm.isf; Exp(1) statistics of normalised noise; injection recovery.
- * Parity unpinned: the paper's Bonferroni trial count (R15) — a plan parameter, default 1.
+ * scipy.special.gammaincc / chi2.sf / norm.isf; Exp(1) statistics of normalised noise; injection recovery;
+ * the searched-width sets against the paper's printed list (L411) and Alg. 4's remainder rule; the harmonic sum against a
+ * ramp's closed form, a numpy reshape route and the χ² degrees of freedom the paper states (KS test); Alg. 1 against a
+ * numpy.median route and a hand example; the sampled / harmonic / per-width searches against a scipy route.
+ * Parity unpinned: the paper's Bonferroni trial count (R15) — a plan parameter, default 1; the paper's own candidate lists
+ * and the J1227-4853 values of Table 3 (data absent).
  *
  * Precision: float32 inputs are widened to double once; everything else is double.
  */
