@@ -268,6 +268,8 @@ def run_ours(args):
         "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "traffic": (traffic_per_bin * bins) if traffic_per_bin else None, "peak_source": peak_src,
         "traffic_source": "profiles/traffic.json (ncu dram__bytes_read+write per bin x bins of this launch)" if traffic_per_bin else None,
+        "limiter": ("LSU data pipe at 71 % of its wavefront rate (ncu, profiles/r01d_summary.md): shared-memory atomics of the "
+                    "exact histogram select" if dom == "norm_power_kernel" and not args.fast_norm else None),
         "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": dom_ms,
         "kernel_ms_all": {"memsets": prof[0], "norm_power_kernel": prof[1], "boxcar_sweep_kernel": prof[2],
                           "block_exact_kernel": prof[3]},
