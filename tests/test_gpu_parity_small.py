@@ -269,6 +269,19 @@ def test_time_series_pipeline_on_one_stream(orc):
     assert_same_candidates(gpu, ora, "time series -> rfft -> search on one stream")
 
 
+@pytest.mark.parametrize("n,batch,zmax,B,C,thr", [(200001, 2, 4096, 8192, 4096, 5.0), (150000, 1, 3000, 4096, 100, 4.5),
+                                                  (65537, 3, 1, 1024, 64, 4.0), (70000, 2, 513, 2048, 7, 4.5),
+                                                  (33000, 1, 31, 512, 20000, 3.5)])
+def test_pruned_equals_exhaustive_at_the_limits(n, batch, zmax, B, C, thr):
+    """Beyond what the oracle finishes in seconds (zmax up to PULSCAN_MAX_ZMAX): the pruned sweep against the exhaustive one."""
+    spec = noise_spectra(batch, n, seed=n + zmax)
+    bump(spec, 0, n // 3, min(zmax, 200), 1.6)
+    bump(spec, batch - 1, n // 2, 3, 4.0)
+    a, stats = gpu_search(spec, zmax, B, C, thr, mode=0)
+    b, _ = gpu_search(spec, zmax, B, C, thr, mode=1)
+    assert len(a) > 0 and np.array_equal(a, b) and stats[3] == 0
+
+
 def test_full_cell_list_falls_back_to_marking_tiles(orc):
     spec = noise_spectra(2, 50001, seed=99)
     ref, st_ref = gpu_search(spec, 64, 2048, 128, 3.0)
