@@ -4,7 +4,7 @@
 //  * the block (B complex64 = 8·B bytes) is staged in shared memory by ONE TMA bulk copy and every pass re-reads it
 //    with conflict-free LDS.64, so the values never occupy registers;
 //  * ONE histogram pass per component serves the median AND the MAD.  The 2048 value-linear buckets span
-//    mean ± 2.5·sd of a 128-bin sample (warp 0 computes it while the others zero the histograms);
+//    mean ± 2·sd of a 128-bin sample (warp 0 computes it while the others zero the histograms);
 //    bucket = RN(2047·sat(v·scale + off)), taken from the mantissa of fma(t, 2047·2⁻²², 2.0f), whose bit pattern
 //    0x40000000 | idx turns into the histogram byte offset with one shift (the 0x4 falls off the top);
 //  * the median's bucket jm comes from a two-level scan (16-bucket chunk sums by all threads, then one warp per
@@ -40,7 +40,10 @@ constexpr int kV2KPT = 16;             // buckets per chunk
 constexpr int kV2NCH = kV2NB / kV2KPT; // chunks per component (128)
 constexpr int kV2ListCap = 128;        // gathered members per component
 constexpr int kV2ClsCap = 64;          // median-net / shell members per component (2 per lane)
-constexpr float kV2Range = 2.5f;       // histogram spans mean ± kV2Range·sd of the sample
+#ifndef PULSCAN_V2_RANGE
+#define PULSCAN_V2_RANGE 2.0f   /* measured at cfg 3: 2.5 → 3.25 ms, 2.0 → 3.20 ms, 1.75 → 3.16 ms but 127 blocks redone, 1.5 → 48 k redone */
+#endif
+constexpr float kV2Range = PULSCAN_V2_RANGE;       // histogram spans mean ± kV2Range·sd of the sample
 constexpr float kV2IdxScale = 2047.0f * 2.384185791015625e-07f;  // 2047·2⁻²²
 
 struct alignas(16) V2Ctl {
