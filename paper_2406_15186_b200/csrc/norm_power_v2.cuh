@@ -29,6 +29,9 @@
 
 #include "norm_power.cuh"
 
+#ifndef PULSCAN_NORM_OCC128_SMALL
+#define PULSCAN_NORM_OCC128_SMALL 10   /* EPT <= 16 fits 48 registers without spills: cfg 5 kernel (a) 8.85 -> 8.61 ms */
+#endif
 #ifndef PULSCAN_NORM_OCC128
 #define PULSCAN_NORM_OCC128 8
 #endif
@@ -386,7 +389,7 @@ constexpr size_t v2_smem_bytes() {
 // global memory (the second and third time out of L1/L2, where a block read microseconds earlier still is), which
 // leaves 19 KB of shared memory per CTA so that more blocks are in flight per SM to cover the warp-serial phases.
 template <int EPT, int NT, bool STAGED>
-__global__ void __launch_bounds__(NT, STAGED ? ((EPT * NT <= 4096) ? 4 : 2) : (NT == 128 ? PULSCAN_NORM_OCC128 : (EPT * NT <= 4096) ? 6 : 4))
+__global__ void __launch_bounds__(NT, STAGED ? ((EPT * NT <= 4096) ? 4 : 2) : (NT == 128 ? (EPT <= 16 ? PULSCAN_NORM_OCC128_SMALL : PULSCAN_NORM_OCC128) : (EPT * NT <= 4096) ? 6 : 4))
 norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int blocks_per_row, float* __restrict__ P,
                      long long pitchP, unsigned* __restrict__ redo, unsigned* __restrict__ redo_count,
                      const char* __restrict__ lim_lo, const char* __restrict__ lim_hi) {
