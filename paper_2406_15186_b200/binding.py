@@ -238,8 +238,9 @@ class Plan:
         cnt = ctypes.c_uint32(0)
         _check(self.lib.pulscan_search_host(self.handle, h_spectra.data_ptr(), h_candidates.ctypes.data,
                                             ctypes.addressof(cnt), _stream_ptr(stream)))
-        rec = h_candidates[: cnt.value]
-        return rec[np.lexsort((rec["bin"], rec["spectrum"]))]
+        self.last_count = int(cnt.value)                     # with per-width emission: the number found, possibly > capacity
+        rec = h_candidates[: min(self.last_count, self.capacity) if self.capacity else self.last_count]
+        return rec[np.lexsort((rec["width"], rec["bin"], rec["spectrum"]))]
 
     def normalise_power(self, d_spectra: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
         """Steps 1-2 only: float32 power [batch, n_bins] (a view of the padded [batch, power_pitch] buffer)."""

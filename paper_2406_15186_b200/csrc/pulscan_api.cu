@@ -93,6 +93,7 @@ struct pulscan_plan {
     SweepParams sp{};
     int tiles_per_row = 0;
     bool sweep_fine = false;   // some level has g < 4: the sweep keeps the full-resolution prefix sum
+    std::string pruned_error;  // non-empty: the pruned sweep could not be sized for this plan (mode 1 still works)
     int refine_grid = 0;
     int sweep_grid = 0;        // persistent CTAs of the pruned sweep: SM count × resident CTAs per SM
     size_t smem_sweep = 0, smem_refine = 0, smem_exh = 0, smem_exact = 0;
@@ -110,11 +111,14 @@ struct pulscan_plan {
     size_t ws_bytes = 0;
     size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_redo = 0, off_cells = 0, off_stage_in = 0, off_stage_cand = 0,
            off_stage_count = 0, bitmap_bytes = 0, need_bytes = 0;
-    // device tables (plan-owned, small)
+    // device tables: T_w (double), T'_w and τ (float); they live in the caller's workspace (off_tables) and are uploaded by
+    // pulscan_plan_set_workspace, so that the plan owns no device memory at all
+    size_t off_tables = 0;
     double* d_T = nullptr;
     float* d_Tp = nullptr;
     float* d_tau = nullptr;
-    bool device_ready = false;
+    bool finalized = false;    // workspace attached, tables uploaded, launch shapes fixed for the current device
+    int device = -1;           // the device the plan was finalized on
     int sm_count = 148;
     // optional per-kernel timing: 5 events per slot (start, memsets done, (a) done, (b) done, (c) done)
     int prof_slots = 0, prof_next = 0;
@@ -163,6 +167,7 @@ int derive(pulscan_plan& p) {
         const int z = w - 1;
         return p.log_sampling ? (z == 0 || (z & (z - 1)) == 0) : (z % p.z_step == 0);
     };
+    p.pruned_error.clear();
     for (int w = 1; w <= p.zmax; ++w) {
         p.T[w - 1] = searched(w) ? power_threshold(w * p.shape_mult, lnp_target) : INFINITY;
         p.Tp[w - 1] = searched(w) ? conservative_threshold(p.T[w - 1], w) : INFINITY;
@@ -195,6 +200,7 @@ int derive(pulscan_plan& p) {
         lvls.clear();
         lgmax = 0;
         bool fits = true;
+        int ntasks_all = 0;
         for (int w = 1; w <= p.zmax && fits;) {
             const int lg = lgw[w], g = 1 << lg;
             auto m_range = [&](int w2, int& m_lo, int& m_hi) {
@@ -202,9 +208,9 @@ int derive(pulscan_plan& p) {
                 else { m_lo = (w + g - 1) / g; m_hi = (w2 >= 2) ? (w2 - 2) / g + 2 : 1; }
             };
             int w2 = w, m_lo = 0, m_hi = 0;
-            while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lg) {   // extend the run while the m range fits 32 steps of 4
-                m_range(w2 + 1, m_lo, m_hi);
-                if (m_hi - m_lo + 1 > 128) break;
+            while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lg) {   // extend the run while the m range fits 32 steps of 4, counted
+                m_range(w2 + 1, m_lo, m_hi);                  // from m_lo rounded down to 4 (sweep_task's hit mask has 32 bits)
+                if ((m_hi - (m_lo & ~3) + 4) / 4 > 32) break;
                 ++w2;
             }
             m_range(w2, m_lo, m_hi);
@@ -215,10 +221,13 @@ int derive(pulscan_plan& p) {
             lv.nsteps = (m_hi - lv.m_start + 4) / 4;
             lv.nk = tile >> lg;
             lv.nwt = (lv.nk + 32 * kSweepR - 1) / (32 * kSweepR);
+            if (lv.nsteps > 32) return fail(PULSCAN_EINVAL, "internal: sweep level with %d steps (limit 32)", lv.nsteps);
+            ntasks_all += lv.nwt;
             lvls.push_back(lv);
             lgmax = std::max(lgmax, lg);
             w = w2 + 1;
         }
+        if (fits && ntasks_all > kMaxWarpTasks) fits = false;   // too many fine levels for one tile: coarser groups
         if (fits) {   // shared memory of the two tile buffers + one decimated array per distinct group size
             const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
             size_t fl = kSweepBufs * ((size_t)len + kScanPer + 4);
@@ -230,7 +239,14 @@ int derive(pulscan_plan& p) {
                 }
             if (fl * 4 + sizeof(SweepCtl) + 2048 <= 227 * 1024) break;
         }
-        if (l10 >= 0.0) return fail(PULSCAN_EINVAL, "zmax = %d with tile = %d does not fit the sweep's shared memory", p.zmax, tile);
+        if (l10 >= 0.0) {   // cannot happen inside the documented parameter ranges; the exhaustive mode does not need the levels
+            char msg[256];
+            snprintf(msg, sizeof msg, "zmax = %d with tile = %d does not fit the pruned sweep (shared memory or %d warp-tasks per tile)",
+                     p.zmax, tile, kMaxWarpTasks);
+            p.pruned_error = msg;
+            lvls.clear(); lgmax = 0;
+            break;
+        }
     }
     SweepParams& sp = p.sp;
     std::memset(&sp, 0, sizeof sp);
@@ -340,9 +356,14 @@ int derive(pulscan_plan& p) {
     p.cell_cap = (unsigned)std::min<unsigned long long>(1ull << 28, std::max<unsigned long long>(65536, (unsigned long long)p.batch * p.n / 256));
     if (p.cell_cap_user) p.cell_cap = p.cell_cap_user;
     p.off_cells = o; o += align_up((size_t)p.cell_cap * sizeof(SweepCell), 256);
+    p.off_tables = o;
+    o += align_up(p.T.size() * sizeof(double), 256) + align_up(p.Tp.size() * sizeof(float), 256) +
+         align_up(std::max<size_t>(1, p.tau.size()) * sizeof(float), 256);
     if (p.host_staging) {
         p.off_stage_in = o; o += align_up((size_t)p.batch * p.pitch * 8, 256);
-        p.off_stage_cand = o; o += align_up((size_t)p.batch * p.nblk * sizeof(pulscan_candidate), 256);
+        // per-width emission writes up to the caller's capacity, which may exceed one record per block
+        const size_t recs = std::max<size_t>((size_t)p.batch * p.nblk, (size_t)p.user_capacity);
+        p.off_stage_cand = o; o += align_up(recs * sizeof(pulscan_candidate), 256);
         p.off_stage_count = o; o += 256;
     }
     // ---- harmonic-summed spectra: one child plan per H = 2..numharm, each with its own region of the workspace (a child's
@@ -371,8 +392,14 @@ int derive(pulscan_plan& p) {
     return PULSCAN_OK;
 }
 
-int ensure_device(pulscan_plan& p) {
-    if (p.device_ready) return PULSCAN_OK;
+// Everything pulscan_search needs from the CUDA runtime besides launches, done once when the workspace is attached: device
+// check, upload of the three small tables into the workspace, dynamic shared-memory limits of the kernels (an attribute of the
+// function ON THE CURRENT DEVICE, so it is set at every finalisation rather than once per process), launch shapes from the
+// occupancy API.  Synchronous; never called from pulscan_search.
+int set_kernel_attributes(const pulscan_plan& p);
+
+int finalize_device(pulscan_plan& p) {
+    p.finalized = false;
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     cudaDeviceProp prop;
@@ -380,19 +407,22 @@ int ensure_device(pulscan_plan& p) {
     if (prop.major != 10)
         return fail(PULSCAN_EARCH, "device %s is compute capability %d.%d; libpulscan is built for sm_100a only", prop.name,
                     prop.major, prop.minor);
+    p.device = dev;
     p.sm_count = prop.multiProcessorCount;
-    CUDA_TRY(cudaMalloc(&p.d_T, p.T.size() * sizeof(double)));
-    CUDA_TRY(cudaMalloc(&p.d_Tp, p.Tp.size() * sizeof(float)));
-    CUDA_TRY(cudaMalloc(&p.d_tau, std::max<size_t>(1, p.tau.size()) * sizeof(float)));
+    char* ws = static_cast<char*>(p.ws);
+    p.d_T = reinterpret_cast<double*>(ws + p.off_tables);
+    p.d_Tp = reinterpret_cast<float*>(ws + p.off_tables + align_up(p.T.size() * sizeof(double), 256));
+    p.d_tau = reinterpret_cast<float*>(reinterpret_cast<char*>(p.d_Tp) + align_up(p.Tp.size() * sizeof(float), 256));
     CUDA_TRY(cudaMemcpy(p.d_T, p.T.data(), p.T.size() * sizeof(double), cudaMemcpyHostToDevice));
     CUDA_TRY(cudaMemcpy(p.d_Tp, p.Tp.data(), p.Tp.size() * sizeof(float), cudaMemcpyHostToDevice));
-    CUDA_TRY(cudaMemcpy(p.d_tau, p.tau.data(), p.tau.size() * sizeof(float), cudaMemcpyHostToDevice));
-    const auto sweep_fn = p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>;
-    // The limit is a property of the function, shared by every plan of the process (and by a plan's harmonic children):
-    // allow the device maximum once instead of this plan's own size, which a later plan could lower again.
+    if (!p.tau.empty()) CUDA_TRY(cudaMemcpy(p.d_tau, p.tau.data(), p.tau.size() * sizeof(float), cudaMemcpyHostToDevice));
     constexpr int kMaxDynSmem = 227 * 1024;
-    CUDA_TRY(cudaFuncSetAttribute(sweep_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    if (p.smem_sweep > (size_t)kMaxDynSmem || p.smem_exh > (size_t)kMaxDynSmem || p.smem_exact > (size_t)kMaxDynSmem)
+        return fail(PULSCAN_EINVAL, "plan needs more shared memory than an SM has (sweep %zu, exhaustive %zu, exact %zu bytes)",
+                    p.smem_sweep, p.smem_exh, p.smem_exact);
+    int rc = set_kernel_attributes(p);
+    if (rc) return rc;
+    const auto sweep_fn = p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>;
     int occ = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_fn, kSweepThreads, p.smem_sweep));
     if (occ < 1) return fail(PULSCAN_ECUDA, "boxcar_sweep_kernel does not fit an SM with %zu bytes of shared memory", p.smem_sweep);
@@ -400,27 +430,40 @@ int ensure_device(pulscan_plan& p) {
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_refine_kernel, kRefineThreads, p.smem_refine));
     if (occ < 1) return fail(PULSCAN_ECUDA, "sweep_refine_kernel does not fit an SM with %zu bytes of shared memory", p.smem_refine);
     p.refine_grid = p.sm_count * std::min(occ, 16);
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    if (p.smem_sweep > (size_t)kMaxDynSmem || p.smem_exh > (size_t)kMaxDynSmem || p.smem_exact > (size_t)kMaxDynSmem)
-        return fail(PULSCAN_EINVAL, "plan needs more shared memory than an SM has (sweep %zu, exhaustive %zu, exact %zu bytes)",
-                    p.smem_sweep, p.smem_exh, p.smem_exact);
-    p.device_ready = true;
+    p.finalized = true;
     return PULSCAN_OK;
 }
 
 void release_profiling(pulscan_plan& p) {
-    for (cudaEvent_t e : p.prof_events) cudaEventDestroy(e);
+    for (cudaEvent_t e : p.prof_events)
+        if (e) cudaEventDestroy(e);
     p.prof_events.clear();
     p.prof_next = 0;
 }
 
-void release_device(pulscan_plan& p) {
-    if (p.d_T) cudaFree(p.d_T);
-    if (p.d_Tp) cudaFree(p.d_Tp);
-    if (p.d_tau) cudaFree(p.d_tau);
-    p.d_T = nullptr; p.d_Tp = nullptr; p.d_tau = nullptr;
-    p.device_ready = false;
+// A setter changed something the derived tables or the workspace layout depend on: the plan must be finalised again
+// (pulscan_plan_set_workspace) before the next search.  Host only: the plan owns no device memory.
+void invalidate(pulscan_plan& p) {
+    p.dirty = true;
+    p.finalized = false;
+    for (pulscan_plan* c : p.harm) c->finalized = false;
+}
+
+// Dynamic shared-memory limits above 48 KB are an attribute of (function, device): set for every kernel that may need one,
+// each time a plan is finalised on a device (idempotent, host-side, cheap).
+int set_kernel_attributes(const pulscan_plan& p) {
+    (void)p;
+    constexpr int kMaxDynSmem = 227 * 1024;
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<16, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)v2_smem_bytes<16, 256, true>()));
+    CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<32, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)v2_smem_bytes<32, 256, true>()));
+    return PULSCAN_OK;
 }
 
 template <int NT>
@@ -456,12 +499,6 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
     const char* lim_hi = lim_lo + ((size_t)(p.batch - 1) * p.pitch + p.n) * 8;
 #define PULSCAN_V2_LAUNCH(E, NT_, ST)                                                                                 \
     {                                                                                                                 \
-        static bool attr_set = false;                                                                                 \
-        if (!attr_set) {                                                                                              \
-            CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<E, NT_, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                                          (int)v2_smem_bytes<E, NT_, ST>()));                                         \
-            attr_set = true;                                                                                          \
-        }                                                                                                             \
         norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                              \
             spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo, redo_count, lim_lo, lim_hi);                     \
     }
@@ -553,6 +590,7 @@ int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candid
     const long long grid_b = (long long)p.tiles_per_row * p.batch;                 // (b)
     if (grid_b > 2147483647LL) return fail(PULSCAN_EINVAL, "too many sweep tiles for one launch");
     if (p.mode == 0) {
+        if (!p.pruned_error.empty()) return fail(PULSCAN_EINVAL, "%s; use mode 1 (exhaustive)", p.pruned_error.c_str());
         SweepCell* d_cells = reinterpret_cast<SweepCell*>(ws + p.off_cells);
         (p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>)<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
                                                                               p.C, p.nblk, p.d_tau, d_cells, p.cell_cap,
@@ -580,18 +618,14 @@ int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candid
     return PULSCAN_OK;
 }
 
+// The search entry points only look at host state here: no CUDA call, no allocation.
 int check_plan_ready(pulscan_plan* plan) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
-    int rc = derive(*plan);
-    if (rc) return rc;
     if (!plan->ws) return fail(PULSCAN_ENOWORKSPACE, "no workspace attached (pulscan_plan_set_workspace)");
-    if (plan->ws_bytes < plan->need_bytes)
-        return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes attached, %zu needed", plan->ws_bytes, plan->need_bytes);
-    attach_children(*plan);
-    for (pulscan_plan* c : plan->harm) {
-        if ((rc = ensure_device(*c))) return rc;
-    }
-    return ensure_device(*plan);
+    if (plan->dirty || !plan->finalized)
+        return fail(PULSCAN_ENOWORKSPACE, "the plan was changed after pulscan_plan_set_workspace: attach the workspace again "
+                                          "(pulscan_plan_workspace_bytes may have changed)");
+    return PULSCAN_OK;
 }
 
 } // namespace
@@ -626,21 +660,21 @@ int pulscan_plan_set_norm_block(pulscan_plan* plan, int32_t norm_block) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (norm_block < 2 || norm_block > PULSCAN_MAX_NORM_BLOCK)
         return fail(PULSCAN_EINVAL, "norm_block = %d out of range [2, %d]", norm_block, PULSCAN_MAX_NORM_BLOCK);
-    plan->B = norm_block; plan->dirty = true; release_device(*plan);
+    plan->B = norm_block; invalidate(*plan);
     return PULSCAN_OK;
 }
 
 int pulscan_plan_set_trials(pulscan_plan* plan, double n_trials) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (!(n_trials >= 1.0) || !std::isfinite(n_trials)) return fail(PULSCAN_EINVAL, "n_trials must be finite and ≥ 1");
-    plan->n_trials = n_trials; plan->dirty = true; release_device(*plan);
+    plan->n_trials = n_trials; invalidate(*plan);
     return PULSCAN_OK;
 }
 
 int pulscan_plan_set_pitch(pulscan_plan* plan, int64_t pitch_bins) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (pitch_bins < plan->n) return fail(PULSCAN_EINVAL, "pitch = %lld < n_bins = %lld", (long long)pitch_bins, (long long)plan->n);
-    plan->pitch = pitch_bins; plan->dirty = true;
+    plan->pitch = pitch_bins; invalidate(*plan);
     return PULSCAN_OK;
 }
 
@@ -655,7 +689,7 @@ int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t 
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (z_step < 1) return fail(PULSCAN_EINVAL, "z_step = %d < 1", z_step);
     plan->z_step = z_step; plan->log_sampling = logarithmic != 0;
-    plan->dirty = true; release_device(*plan);
+    invalidate(*plan);
     return PULSCAN_OK;
 }
 
@@ -685,6 +719,7 @@ int pulscan_plan_set_emission(pulscan_plan* plan, int32_t per_width, int64_t cap
     plan->per_width = per_width;
     plan->user_capacity = per_width ? capacity : 0;
     plan->out_capacity = per_width ? (unsigned)capacity : 0xFFFFFFFFu;
+    if (plan->host_staging) invalidate(*plan);   // the staging area for the records is sized from the capacity
     return PULSCAN_OK;
 }
 
@@ -696,14 +731,14 @@ int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_
         return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -2]");
     plan->tile_user = tile_bins;
     plan->log10_p_flag = (log10_p_flag == 0.0) ? -3.0 : log10_p_flag;
-    plan->dirty = true; release_device(*plan);
+    invalidate(*plan);
     return PULSCAN_OK;
 }
 
 int pulscan_plan_set_cell_capacity(pulscan_plan* plan, int64_t cells) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (cells < 0 || cells > (1ll << 28)) return fail(PULSCAN_EINVAL, "cell capacity out of range [0, 2^28]");
-    plan->cell_cap_user = (unsigned)cells; plan->dirty = true;
+    plan->cell_cap_user = (unsigned)cells; invalidate(*plan);
     return PULSCAN_OK;
 }
 
@@ -721,7 +756,7 @@ size_t pulscan_plan_workspace_bytes(const pulscan_plan* plan) {
 
 int pulscan_plan_enable_host_staging(pulscan_plan* plan, int32_t enable) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
-    plan->host_staging = enable != 0; plan->dirty = true;
+    plan->host_staging = enable != 0; invalidate(*plan);
     return PULSCAN_OK;
 }
 
@@ -735,7 +770,9 @@ int pulscan_plan_set_workspace(pulscan_plan* plan, void* d_workspace, size_t byt
         return fail(PULSCAN_ENOWORKSPACE, "workspace too small: %zu bytes given, %zu needed", bytes, plan->need_bytes);
     plan->ws = d_workspace; plan->ws_bytes = bytes;
     attach_children(*plan);
-    return PULSCAN_OK;
+    for (pulscan_plan* c : plan->harm)
+        if ((rc = finalize_device(*c))) return rc;
+    return finalize_device(*plan);
 }
 
 int64_t pulscan_plan_power_pitch(const pulscan_plan* plan) {
@@ -750,10 +787,8 @@ int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_
     if (!d_spectra || !d_power) return fail(PULSCAN_EINVAL, "null pointer");
     if (reinterpret_cast<uintptr_t>(d_spectra) & 7) return fail(PULSCAN_EINVAL, "d_spectra must be 8-byte aligned");
     if (reinterpret_cast<uintptr_t>(d_power) & 15) return fail(PULSCAN_EINVAL, "d_power must be 16-byte aligned");
-    rc = ensure_device(*plan);
-    if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (plan->ws && plan->ws_bytes >= plan->need_bytes) { // workspace attached: same kernels as pulscan_search
+    if (plan->ws && plan->finalized) { // workspace attached: same kernels as pulscan_search
         char* ws = static_cast<char*>(plan->ws);
         unsigned* d_counters = reinterpret_cast<unsigned*>(ws + plan->off_counters);
         CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
@@ -780,10 +815,6 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
 
     cudaEvent_t* ev = nullptr;
     if (p.prof_slots > 0) {
-        if (p.prof_events.empty()) {
-            p.prof_events.resize((size_t)p.prof_slots * 5);
-            for (cudaEvent_t& e : p.prof_events) CUDA_TRY(cudaEventCreate(&e));
-        }
         ev = &p.prof_events[(size_t)(p.prof_next % p.prof_slots) * 5];
         ++p.prof_next;
         CUDA_TRY(cudaEventRecord(ev[0], st));
@@ -808,7 +839,7 @@ int pulscan_plan_set_harmonics(pulscan_plan* plan, int32_t numharm) {
     if (numharm < 1 || numharm > 4) return fail(PULSCAN_EINVAL, "numharm = %d out of range [1, 4]", numharm);
     if ((int64_t)plan->zmax >= plan->n / numharm)
         return fail(PULSCAN_EINVAL, "zmax = %d must be < floor(n_bins / numharm) = %lld", plan->zmax, (long long)(plan->n / numharm));
-    plan->numharm = numharm; plan->dirty = true;
+    plan->numharm = numharm; invalidate(*plan);
     return PULSCAN_OK;
 }
 
@@ -884,8 +915,10 @@ int pulscan_search_host(pulscan_plan* plan, const void* h_spectra, pulscan_candi
     if (rc) return rc;
     CUDA_TRY(cudaMemcpyAsync(h_count, d_cnt, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
-    if (*h_count)
-        CUDA_TRY(cudaMemcpyAsync(h_candidates, d_cand, (size_t)*h_count * sizeof(pulscan_candidate), cudaMemcpyDeviceToHost, st));
+    // per-width emission: *h_count is the number FOUND; only the first `capacity` records exist (and fit h_candidates)
+    const size_t ncopy = std::min<size_t>(*h_count, p.per_width ? (size_t)p.user_capacity : (size_t)*h_count);
+    if (ncopy)
+        CUDA_TRY(cudaMemcpyAsync(h_candidates, d_cand, ncopy * sizeof(pulscan_candidate), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     return PULSCAN_OK;
 }
@@ -964,6 +997,16 @@ int pulscan_plan_set_profiling(pulscan_plan* plan, int32_t n_slots) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (n_slots < 0 || n_slots > 65536) return fail(PULSCAN_EINVAL, "n_slots out of range [0, 65536]");
     release_profiling(*plan);
+    plan->prof_slots = 0;
+    plan->prof_events.resize((size_t)n_slots * 5);
+    for (cudaEvent_t& e : plan->prof_events) {
+        e = nullptr;
+        const cudaError_t err = cudaEventCreate(&e);
+        if (err != cudaSuccess) {
+            release_profiling(*plan);
+            return fail(PULSCAN_ECUDA, "cudaEventCreate failed: %s", cudaGetErrorString(err));
+        }
+    }
     plan->prof_slots = n_slots;
     return PULSCAN_OK;
 }
@@ -982,7 +1025,6 @@ int pulscan_plan_destroy(pulscan_plan* plan) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     for (pulscan_plan* c : plan->harm) pulscan_plan_destroy(c);
     release_profiling(*plan);
-    release_device(*plan);
     delete plan;
     return PULSCAN_OK;
 }

@@ -150,6 +150,22 @@ def test_sweep_levels_cover_every_width_exactly_once(binding, zmax, thr, lpf):
     p.destroy()
 
 
+@pytest.mark.parametrize("zmax", [128, 200, 512, 1024, 4096])
+@pytest.mark.parametrize("thr", [1.5, 2.0, 2.5, 3.0, 3.5, 4.0, 6.0])
+def test_low_thresholds_give_valid_plans_with_at_most_32_steps_per_level(binding, zmax, thr):
+    """A level's hit mask has 32 bits (one per 4-wide step over the cover length m): the host must never build a level with
+    33 steps (m_lo not a multiple of 4 and 128 cover lengths), and low thresholds with large zmax must still give a plan
+    (too many fine levels for one tile relax the per-cover flag probability instead of failing)."""
+    for z_step in (1, 127):
+        p = binding.Plan(1 << 20, 1, zmax, 200, thr, z_step=z_step)
+        d = p.describe()
+        steps = [int(x) for x in re.findall(r"steps=(\d+)", d)]
+        tasks = [int(x) for x in re.findall(r"warp-tasks/tile=(\d+)", d)]
+        assert steps and max(steps) <= 32, d
+        assert sum(tasks) <= 128, d
+        p.destroy()
+
+
 def test_pruning_bound_is_an_upper_bound_property():
     # the sweep's premise: P >= 0, so a window's sum is bounded by the sum of the aligned groups covering it
     rng = np.random.default_rng(0)

@@ -112,6 +112,21 @@ def test_pruned_equals_exhaustive_on_noise_with_low_threshold(orc):
     assert_same_candidates(a, oracle_search(orc, spec, 64, 2048, 128, 3.0), "thr=3 noise")
 
 
+@pytest.mark.parametrize("zmax,thr,z_step,n", [(128, 2.0, 1, 30011), (200, 3.0, 1, 30011), (512, 2.5, 1, 30011), (128, 3.0, 127, 30011),
+                                               (256, 2.0, 127, 30011), (1024, 2.0, 1, 20001), (1024, 3.0, 1, 20001),
+                                               (4096, 4.0, 1, 30011)])
+def test_low_threshold_wide_levels_pruned_equals_exhaustive_equals_oracle(orc, zmax, thr, z_step, n):
+    """Levels spanning up to 128 cover lengths (32 steps of 4, the last step included) and plans that need the relaxed flag
+    probability: low thresholds with large zmax, and a z_step that leaves one searched width alone in a level's last step."""
+    spec = noise_spectra(1, n, seed=zmax * 31 + z_step)
+    bump(spec, 0, n // 2, min(zmax, 128), 1.6)
+    C = 256
+    a, _ = gpu_search(spec, zmax, 4096, C, thr, mode=0, z_step=z_step)
+    b, _ = gpu_search(spec, zmax, 4096, C, thr, mode=1, z_step=z_step)
+    assert np.array_equal(a, b) and len(a) > 0
+    assert_same_candidates(a, oracle_search(orc, spec, zmax, 4096, C, thr, z_step=z_step), f"zmax={zmax} thr={thr} z_step={z_step}")
+
+
 @pytest.mark.parametrize("tile,lpf", [(1024, -2.0), (2048, -3.0), (8192, -7.0), (16384, -9.0)])
 def test_tuning_never_changes_results(orc, tile, lpf):
     spec = noise_spectra(1, 40000, seed=123)
@@ -338,3 +353,75 @@ def test_config1_full(orc):
     assert_same_candidates(gpu, ora, "config 1")
     top = gpu[np.argmax(gpu["sigma"])]
     assert (int(top["bin"]), int(top["width"])) == (727, 14)
+
+
+def test_first_search_of_a_fresh_plan_is_graph_capturable(orc):
+    """pulscan_search allocates nothing and never synchronises, its FIRST call included (everything that needs the runtime
+    happens in pulscan_plan_set_workspace): the first search of a fresh plan is captured into a CUDA graph on a side
+    stream, replayed on two new inputs, and each replay gives the oracle's list."""
+    from paper_2406_15186_b200 import binding
+    n, batch, zmax, B, C, thr = 20001, 2, 40, 2048, 100, 4.0
+    inputs = []
+    for k in range(3):
+        spec = noise_spectra(batch, n, seed=900 + k)
+        bump(spec, k % batch, 3000 + 2500 * k, 10 + 5 * k, 2.5)
+        inputs.append(spec)
+    buf = torch.empty_like(inputs[0])
+    plan = binding.Plan(n, batch, zmax, C, thr, norm_block=B)
+    plan.attach("cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    buf.copy_(inputs[0])
+    torch.cuda.synchronize()
+    with torch.cuda.graph(graph, stream=side):
+        plan.search(buf, torch.cuda.current_stream())       # the first pulscan_search this plan ever sees
+    for k in (1, 2):
+        buf.copy_(inputs[k])
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        gpu = plan.candidates()
+        ora = oracle_search(orc, inputs[k], zmax, B, C, thr)
+        assert len(ora) > 0
+        assert_same_candidates(gpu, ora, f"graph replay {k}")
+    plan.destroy()
+
+
+def test_setter_after_attach_needs_a_new_attach():
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(1, 20001, seed=31)
+    plan = binding.Plan(20001, 1, 40, 100, 4.0, norm_block=2048)
+    plan.attach("cuda")
+    plan.search(spec)
+    assert plan.lib.pulscan_plan_set_trials(plan.handle, 10.0) == 0
+    with pytest.raises(binding.PulscanError) as e:
+        plan.search(spec)
+    assert e.value.code == binding.PULSCAN_ENOWORKSPACE
+    plan.attach("cuda")
+    plan.search(spec)
+    plan.set_mode(1)                                         # no derived state depends on the mode: no new attach needed
+    plan.search(spec)
+    torch.cuda.synchronize()
+    plan.destroy()
+
+
+def test_host_staging_with_per_width_emission(orc):
+    """pulscan_search_host under per-(block, width) emission: the staging area follows the caller's capacity and only
+    min(found, capacity) records are copied back."""
+    from paper_2406_15186_b200 import binding
+    n, batch, zmax, B, C, thr = 20001, 1, 40, 2048, 5000, 3.0       # 5 blocks, capacity far above one record per block
+    spec = noise_spectra(batch, n, seed=778)
+    bump(spec, 0, n // 3, 6, 3.0)
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, 1, per_width=True)
+    assert len(ora) > 5 * 8
+    for cap in (len(ora) + 5, 9):
+        plan = binding.Plan(n, batch, zmax, C, thr, norm_block=B, host_staging=True, per_width_capacity=cap)
+        plan.attach("cuda")
+        hc = np.zeros(cap + 64, dtype=binding.CANDIDATE_DTYPE)       # 64 guard records behind the capacity
+        got = plan.search_host(spec.cpu().pin_memory(), hc[:cap])
+        assert plan.last_count == len(ora) and len(got) == min(cap, len(ora))
+        assert not hc[cap:].view(np.uint8).any()                       # nothing written beyond the caller's capacity
+        keys = set(zip(ora["bin"].tolist(), ora["width"].tolist()))
+        assert all(k in keys for k in zip(got["bin"].tolist(), got["width"].tolist())) and np.all(got["width"] >= 1)
+        plan.destroy()
