@@ -21,6 +21,10 @@ CASES = [
     (16, "52.6057"), (32, "80"), (64, "128"), (100, "180"), (128, "207.9386"), (200, "300"), (200, "391"),
     (256, "363.9496"), (512, "659.6351"), (1024, "1227.8128"), (1200, "1419.6481"), (1200, "1500"), (1200, "1600"),
     (1200, "3000"), (5, "5"), (10, "10"), (50, "30"), (200, "150"), (7, "0.5"), (1, "700"), (3, "1000"),
+    # Gamma shapes the harmonic search reaches (w·H(H+1)/2: 2000 at zmax 200 / numharm 4, 12000 at zmax 1200, 40960 at
+    # PULSCAN_MAX_ZMAX): a power just above the σ = 6 threshold, a strong one, and one below the mean (largest term inside the sum)
+    (2000, "2281"), (2000, "2600"), (2000, "1950"), (12000, "12672"), (12000, "13500"), (12000, "11900"),
+    (40960, "42190"), (40960, "44000"), (40960, "40800"),
 ]
 
 

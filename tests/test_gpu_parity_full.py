@@ -1,6 +1,6 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (one pulscan_search over the
-whole batch), checked against the oracle on sampled spectra (every spectrum of configs 1-2; a seeded sample that
-always includes injected spectra for configs 3-5) plus properties that hold for the whole batch."""
+whole batch), checked against the oracle on EVERY spectrum of every config, plus properties that hold for the whole batch
+(injection recovery, false-alarm count)."""
 import numpy as np
 import pytest
 import torch
@@ -21,16 +21,25 @@ def full_search(wl, X):
     return rec, flagged
 
 
-def check_sample(orc, wl, X, rec, inj, n_noise, seed):
-    injected = sorted({i.spectrum for i in inj})
-    rng = np.random.default_rng(seed)
-    noise = [b for b in rng.permutation(wl.batch).tolist() if b not in injected][:n_noise]
-    sample = sorted(set(injected[:12] + noise))
-    for b in sample:
-        ora = orc.search(X[b].cpu().numpy(), wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
-        ora["spectrum"] = b
-        assert_same_candidates(rec[rec["spectrum"] == b], ora, f"{wl.name} spectrum {b}")
-    return sample
+def check_every_spectrum(orc, wl, X, rec, chunk=16):
+    """The GPU list against the oracle on EVERY spectrum of the batch; rows go to the host a chunk at a time."""
+    n_ora = 0
+    for b0 in range(0, wl.batch, chunk):
+        rows = X[b0:b0 + chunk].cpu().numpy()
+        ora = orc.search(rows, wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold)
+        ora["spectrum"] += b0
+        sub = rec[(rec["spectrum"] >= b0) & (rec["spectrum"] < b0 + len(rows))]
+        assert_same_candidates(sub, ora, f"{wl.name} spectra {b0}..{b0 + len(rows) - 1}")
+        n_ora += len(ora)
+    assert n_ora == len(rec)
+    return n_ora
+
+
+def swept_band(wl, i):
+    """Bins the injected tone passes through: r(τ) = r0 + z·τ + ½·w·τ², τ = t/T ∈ [0, 1] (Eq. 1; R24)."""
+    tau = np.linspace(0.0, 1.0, 4001)
+    r = i.f0 * wl.t_obs + i.z * tau + 0.5 * i.jerk * tau ** 2
+    return float(r.min()), float(r.max())
 
 
 def check_properties(wl, rec, inj):
@@ -40,16 +49,29 @@ def check_properties(wl, rec, inj):
     assert rec["bin"].min() >= 0 and np.all(rec["bin"] + rec["width"] <= wl.n_bins)
     assert rec["width"].min() >= 1 and rec["width"].max() <= wl.zmax
     assert np.all(rec["sigma"] >= wl.sigma_threshold - 1e-3) and np.all(rec["power"] > 0)
-    # injected signals strong enough to matter are recovered as the top candidate of their spectrum near the expected bin
+    # Injected signals strong enough to matter are the TOP candidate of their spectrum, inside the band they sweep (loosely:
+    # Pulscan's own location tracks a matched filter's within ~9 bins on average, Table 2).
+    checked = 0
     for i in inj:
+        if sum(1 for j in inj if j.spectrum == i.spectrum) != 1:
+            continue                                       # config 2 puts three signals in one spectrum: checked by the oracle only
         mine = rec[rec["spectrum"] == i.spectrum]
         expected_power = i.amp ** 2 * wl.n_samples / 4
-        if expected_power < 150 or abs(i.z) + 1 > wl.zmax or abs(i.jerk) > 0:
-            continue
+        lo, hi = swept_band(wl, i)
+        if i.jerk == 0.0:
+            if expected_power < 150 or abs(i.z) + 1 > wl.zmax:
+                continue
+            margin_lo, margin_hi, min_sigma = max(8.0, 0.15 * abs(i.z)), 8.0, wl.sigma_threshold
+        else:                                              # config 4: quadratic drift, band up to ~2700 bins for zmax 1200
+            margin_lo, margin_hi, min_sigma = 64.0, 16.0, wl.sigma_threshold + 1.0
         assert len(mine), f"injection {i} not detected"
-        near = mine[np.abs(mine["bin"] - i.expected_start_bin(wl.t_obs)) <= max(8, 0.15 * abs(i.z))]
-        assert len(near), (i, mine[np.argsort(-mine["sigma"])][:3])
-        assert near["sigma"].max() >= 0.5 * mine["sigma"].max() or len({j.spectrum for j in inj if j.spectrum == i.spectrum}) >= 1
+        top = mine[np.argmax(mine["sigma"])]
+        assert lo - margin_lo <= top["bin"] <= hi + margin_hi, (i, (lo, hi), top)
+        assert top["sigma"] >= min_sigma, (i, top)
+        if i.jerk == 0.0:                                  # the width tracks the drift (loosely; L459-463)
+            assert 0.5 * (abs(i.z) + 1) - 4 <= top["width"] <= 1.5 * (abs(i.z) + 1) + 8, (i, top)
+        checked += 1
+    return checked
 
 
 def test_config2_full(orc):
@@ -61,17 +83,22 @@ def test_config2_full(orc):
     assert_same_candidates(rec, ora, "config 2")
     assert len(inj) == 3 and sorted(abs(i.z) for i in inj) == [20.0, 80.0, 180.0]
     check_properties(wl, rec, inj)
+    for i in inj:                                       # three signals in one spectrum: each has a candidate at its band
+        lo, hi = swept_band(wl, i)
+        near = rec[(rec["bin"] >= lo - max(8.0, 0.15 * abs(i.z))) & (rec["bin"] <= hi + 8)]
+        assert len(near) and near["sigma"].max() >= 8.0, (i, near)
     assert flagged >= len(rec)
 
 
-@pytest.mark.parametrize("cfg,n_noise", [(3, 6), (4, 0), (5, 10)])
-def test_batched_configs_full(orc, cfg, n_noise):
+@pytest.mark.parametrize("cfg,min_checked", [(3, 18), (4, 64), (5, 5)])
+def test_batched_configs_full(orc, cfg, min_checked):
+    """BASELINE configs 3-5 in the launch configuration bench.py times (one pulscan_search over the whole batch), the
+    candidate list compared with the oracle on every one of the 256 / 64 / 2048 spectra."""
     wl = synth.CONFIGS[cfg]
     X, inj = synth.make_spectra(wl, device="cuda")
     rec, flagged = full_search(wl, X)
-    sample = check_sample(orc, wl, X, rec, inj, n_noise, seed=cfg)
-    assert len(sample) >= min(12, len({i.spectrum for i in inj}))
-    check_properties(wl, rec, inj)
+    assert check_every_spectrum(orc, wl, X, rec) == len(rec) > 0
+    assert check_properties(wl, rec, inj) >= min_checked
     # noise-only false alarms: <= n·zmax·sf(thr) per spectrum is an upper bound (overlapping windows are correlated)
     from scipy import stats
     injected = {i.spectrum for i in inj}

@@ -105,3 +105,38 @@ def test_harmonics_add_up(orc):
     got = orc.search_harmonics(spec, 4, 1024, 50, 3.0, 4)
     best = {H: got[(got["numharm"] == H) & (np.abs(got["bin"] - r0) <= 1)]["sigma"].max() for H in (1, 4)}
     assert best[4] > best[1] + 1.5
+
+
+def test_per_width_emission_with_harmonics_matches_library_route(orc):
+    """orc_search_opts(per_width = 1) at numharm 3: every (H, block, width) whose maximum passes chi2.logsf(2S, H(H+1)w) (L220;
+    Alg. 4), through numpy/scipy only; and the default output is the highest-sigma record of each (H, block)."""
+    n, zmax, B, C, thr, numharm = 1025, 9, 256, 40, 2.5, 3
+    rng = np.random.default_rng(31)
+    spec = (rng.normal(0, 30, n) + 1j * rng.normal(0, 30, n)).astype(np.complex64)
+    for h in range(1, 4):
+        spec[h * 41: h * 41 + 2] *= 3.0
+    got = orc.search_harmonics(spec, zmax, B, C, thr, numharm, per_width=True)
+    P = orc.normalise_power(spec, B)        # pinned on its own (tests/test_oracle_normalise.py)
+    want = []
+    for H in range(1, numharm + 1):
+        Y = reshape_route(P, H)
+        nH = Y.size
+        pre = np.concatenate([[0.0], np.cumsum(Y)])
+        for c in range((nH + C - 1) // C):
+            lo, hi = c * C, min((c + 1) * C, nH)
+            for w in range(1, zmax + 1):
+                i = np.arange(lo, min(hi, nH - w + 1))
+                if i.size == 0:
+                    continue
+                S = pre[i + w] - pre[i]
+                k = int(np.argmax(S))
+                if stats.chi2.logsf(2 * S[k], H * (H + 1) * w) <= special.log_ndtr(-thr):
+                    want.append((H, int(i[k]), w, S[k]))
+    assert [(int(g["numharm"]), int(g["bin"]), int(g["width"])) for g in got] == [w[:3] for w in want]
+    assert len({w[0] for w in want}) == numharm and len(want) > 30
+    assert np.allclose(got["power"], [w[3] for w in want], rtol=1e-11)
+    best = orc.search_harmonics(spec, zmax, B, C, thr, numharm)
+    for r in best:
+        mine = got[(got["numharm"] == r["numharm"]) & (got["bin"] // C == r["bin"] // C)]
+        top = mine[np.argmax(mine["sigma"])]
+        assert (top["bin"], top["width"], top["sigma"]) == (r["bin"], r["width"], r["sigma"])

@@ -69,3 +69,61 @@ def test_search_with_mom_differs_only_through_the_normalisation(orc):
     assert 0 < len(a) <= len(b)                               # powers ≈ 12 % low: the marginal candidates drop out
     top_a, top_b = a[np.argmax(a["sigma"])], b[np.argmax(b["sigma"])]
     assert abs(int(top_a["bin"]) - int(top_b["bin"])) <= 2 and 0.0 < top_b["sigma"] - top_a["sigma"] < 1.5
+
+
+def mom_power_numpy_route(spec, B):
+    """orc_normalise_power_mom through the numpy route: every bin of every chunk, the tail after the last chunk included (R30)."""
+    n = spec.size
+    nb = n // B
+    P = np.empty(n)
+    for j in range(nb):
+        lo, hi = j * B, (n if j == nb - 1 else (j + 1) * B)
+        comps = []
+        for part in (spec.real, spec.imag):
+            chunk = part[lo:lo + B].astype(np.float64)
+            m = numpy_route(chunk)
+            s = 1.4826 * numpy_route(np.abs(chunk - m))
+            comps.append((part[lo:hi].astype(np.float64) - m) / s)
+        P[lo:hi] = 0.5 * (comps[0] ** 2 + comps[1] ** 2)
+    return P
+
+
+@pytest.mark.parametrize("n,B", [(4 * 1024 + 5, 1024), (3 * 256, 256), (2 * 2048 + 1000, 2048), (8192 + 1, 8192), (5 * 512 + 511, 512)])
+def test_normalise_power_mom_matches_numpy_route_on_every_bin(orc, n, B):
+    rng = np.random.default_rng(n + B)
+    spec = (rng.normal(2.0, 30, n) + 1j * rng.normal(-1.0, 7, n)).astype(np.complex64)
+    P = orc.normalise_power_mom(spec, B)
+    want = mom_power_numpy_route(spec, B)
+    assert np.allclose(P, want, rtol=1e-11, atol=0.0)
+
+
+def test_search_with_mom_matches_library_route(orc):
+    """orc_search_opts(norm_mode = 1): Alg. 1 powers through the numpy route, then cumsum differences, chi2.logsf, norm.isf."""
+    from scipy import special
+    n, zmax, B, C, thr = 1024 + 300, 10, 256, 48, 2.5
+    rng = np.random.default_rng(77)
+    spec = (rng.normal(0, 30, n) + 1j * rng.normal(0, 30, n)).astype(np.complex64)
+    spec[400:405] *= 3.5
+    got = orc.search_harmonics(spec, zmax, B, C, thr, 1, median_of_medians=True)
+    P = mom_power_numpy_route(spec, B)
+    pre = np.concatenate([[0.0], np.cumsum(P)])
+    ref = []
+    for c in range((n + C - 1) // C):
+        lo, hi = c * C, min((c + 1) * C, n)
+        best = None
+        for w in range(1, zmax + 1):
+            i = np.arange(lo, min(hi, n - w + 1))
+            if i.size == 0:
+                continue
+            S = pre[i + w] - pre[i]
+            k = int(np.argmax(S))
+            lnp = min(0.0, stats.chi2.logsf(2 * S[k], 2 * w))
+            if best is None or lnp < best[0]:
+                best = (lnp, int(i[k]), w, S[k])
+        if best is not None and best[0] <= special.log_ndtr(-thr):
+            ref.append(best)
+    assert len(got) == len(ref) > 0
+    for g, r in zip(got, ref):
+        assert (g["bin"], g["width"]) == (r[1], r[2])
+        assert g["power"] == pytest.approx(r[3], rel=1e-10)
+        assert g["sigma"] == pytest.approx(stats.norm.isf(np.exp(r[0])), abs=1e-7)
