@@ -90,6 +90,13 @@ def _load():
                                         ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
                                         ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_void_p,
                                         ctypes.c_int64]
+        lib.orc_search_all.restype = ctypes.c_int64
+        lib.orc_search_all.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                       ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_int32, ctypes.c_int32,
+                                       ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                       ctypes.c_void_p, ctypes.c_int64]
+        lib.orc_power_to_logp.restype = ctypes.c_double
+        lib.orc_power_to_logp.argtypes = [ctypes.c_double, ctypes.c_double]
         lib.orc_search.restype = ctypes.c_int64
         lib.orc_search.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
                                    ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p, ctypes.c_int64]
@@ -170,6 +177,11 @@ def ln_q(w: int, S: float) -> float:
     return float(_load().orc_ln_q(int(w), float(S)))
 
 
+def power_to_logp(power: float, dof: float) -> float:
+    """Alg. 3: the paper's polynomial approximation of ln p, in the paper's units (χ² power, d.o.f.)."""
+    return float(_load().orc_power_to_logp(float(power), float(dof)))
+
+
 def ln_sf(x: float) -> float:
     return float(_load().orc_ln_sf(float(x)))
 
@@ -222,10 +234,12 @@ def harmonic_sum(P, H: int) -> np.ndarray:
 
 def search_harmonics(spectra, zmax: int, norm_block: int, block_width: int, sigma_threshold: float, numharm: int,
                      n_trials: float = 1.0, n_bins: int | None = None, z_step: int = 1, log_sampling: bool = False,
-                     r_block: bool = False, median_of_medians: bool = False, per_width: bool = False) -> np.ndarray:
+                     r_block: bool = False, median_of_medians: bool = False, per_width: bool = False,
+                     poly_logp: bool = False) -> np.ndarray:
     """The search on every harmonic-summed spectrum Y_1 … Y_numharm (§2.3): records carry `numharm`; ordered by
     (numharm, spectrum, bin); at most one per candidate block of each summed spectrum — or, with per_width, one per
-    (block, searched width) above the threshold (Alg. 4), ordered by (numharm, spectrum, block, width)."""
+    (block, searched width) above the threshold (Alg. 4), ordered by (numharm, spectrum, block, width).
+    poly_logp: every ln p from Alg. 3's polynomial instead of the exact χ² tail."""
     s = np.ascontiguousarray(spectra, dtype=np.complex64)
     if s.ndim == 1:
         s = s[None, :]
@@ -235,11 +249,11 @@ def search_harmonics(spectra, zmax: int, norm_block: int, block_width: int, sigm
     cap = sum(batch * ((n // H + C - 1) // C) for H in range(1, int(numharm) + 1)) * (int(zmax) if per_width else 1)
     out = np.zeros(cap, dtype=CANDIDATE_DTYPE)
     f = s.view(np.float32)
-    found = _load().orc_search_opts(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
-                                    int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
-                                    int(bool(log_sampling)), int(bool(r_block)), int(numharm),
-                                    int(bool(median_of_medians)), int(bool(per_width)),
-                                    out.ctypes.data_as(ctypes.c_void_p), cap)
+    found = _load().orc_search_all(f.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), batch, n, pitch, int(zmax),
+                                   int(norm_block), C, float(sigma_threshold), float(n_trials), int(z_step),
+                                   int(bool(log_sampling)), int(bool(r_block)), int(numharm),
+                                   int(bool(median_of_medians)), int(bool(per_width)), int(bool(poly_logp)),
+                                   out.ctypes.data_as(ctypes.c_void_p), cap)
     return out[: int(found)].copy()
 
 

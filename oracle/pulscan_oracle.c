@@ -14,7 +14,9 @@
  * scipy.special.gammaincc / chi2.sf / norm.isf; Exp(1) statistics of normalised noise; injection recovery;
  * the searched-width sets against the paper's printed list (L411) and Alg. 4's remainder rule; the harmonic sum against a
  * ramp's closed form, a numpy reshape route and the χ² degrees of freedom the paper states (KS test); Alg. 1 against a
- * numpy.median route and a hand example; the sampled / harmonic / per-width searches against a scipy route.
+ * numpy.median route and a hand example; the sampled / harmonic / per-width searches against a scipy route; Alg. 3 against
+ * the listing's printed numbers (f(0), the dof >= 1.05·pow branch), an exact rational evaluation of the printed polynomial,
+ * and — as the approximation it is — its error against orc_ln_q over (dof, power).
  * Parity unpinned: the paper's Bonferroni trial count (R15) — a plan parameter, default 1; the paper's own candidate lists
  * and the J1227-4853 values of Table 3 (data absent).
  *
@@ -174,6 +176,29 @@ double orc_sigma_from_lnp(double lnp) {
         if (orc_ln_sf(mid) > lnp) lo = mid; else hi = mid;
     }
     return 0.5 * (lo + hi);
+}
+
+/* ---- Algorithm 3 (§2.6, Eq. 10-12): the paper's GPU significance, an APPROXIMATION of ln p
+ * obtained "by linear regression": Device function power_to_logp(pow, dof):
+ *     if dof >= pow × 1.05 then logp ← 0.0
+ *     else x ← 1500 × dof/pow;  f(x) ← A_2·x^16 + A_3·x^15 + … + A_17·x + A_18;  logp ← pow × f(x)/1500
+ * with the 17 coefficients printed in the listing (A_1 = 1500).  Followed term by term in the printed order, in double.
+ * Reading R31: `pow` and `dof` are in the paper's own units, |X'|² summed over the window and its χ² degrees of freedom
+ * (Eq. 9: 2(z+1); L220: H(H+1)(z+1)), i.e. pow = 2S and dof = 2·shape in the mean-1 units of this file (R2): the
+ * listing's own branch "dof >= 1.05·pow → 0" says pow has mean dof, and f(0)/1500 = −0.5035 ≈ −½ is the χ² tail's
+ * exponent −pow/2.  The paper's logarithm is natural (Table 3: GPU ln p = −171.34 beside σ = 18.8). */
+double orc_power_to_logp(double pow_, double dof) {
+    if (dof >= pow_ * 1.05) return 0.0;
+    double x = 1500.0 * dof / pow_;
+    double f = -4.4604059e-46 * pow(x, 16) + 9.4927863e-42 * pow(x, 15)
+             - 9.1470451e-38 * pow(x, 14) + 5.2810851e-34 * pow(x, 13)
+             - 2.0376166e-30 * pow(x, 12) + 5.5480334e-27 * pow(x, 11)
+             - 1.0973877e-23 * pow(x, 10) + 1.5991804e-20 * pow(x, 9)
+             - 1.7231488e-17 * pow(x, 8) + 1.3660070e-14 * pow(x, 7)
+             - 7.8617952e-12 * pow(x, 6) + 3.2136336e-9 * pow(x, 5)
+             - 9.0466418e-7 * pow(x, 4) + 0.00016945948 * pow(x, 3)
+             - 0.021494231 * pow(x, 2) + 2.9515954 * x - 755.24091;
+    return pow_ * f / 1500.0;
 }
 
 /* ---- Algorithm 1: the paper's GPU normalisation, an APPROXIMATE median ("median of medians",
@@ -384,9 +409,34 @@ int64_t orc_search_general(const float* spectra, int64_t batch, int64_t n, int64
 /* … and with per_width != 0 the paper's GPU output: instead of the best width per block (R13), one record per
  * (block, searched width) whose maximum reaches the threshold (Alg. 4: thread 0 "writes out [the] local candidate"
  * of every searched z; L322 "highest sigma candidate" is picked afterwards).  Ordered by (H, spectrum, block, width). */
+int64_t orc_search_all(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                       int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                       int32_t r_block, int32_t numharm, int32_t norm_mode, int32_t per_width, int32_t signif_mode,
+                       orc_candidate* out, int64_t cap);
+
 int64_t orc_search_opts(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
                         int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
                         int32_t r_block, int32_t numharm, int32_t norm_mode, int32_t per_width, orc_candidate* out, int64_t cap) {
+    return orc_search_all(spectra, batch, n, pitch, zmax, B, C, sigma_threshold, n_trials, z_step, log_sampling, r_block,
+                          numharm, norm_mode, per_width, 0, out, cap);
+}
+
+/* ln p of a width-w maximum S of the spectrum summed over H harmonics (shape = w·H(H+1)/2 in mean-1 units):
+ * signif_mode 0: the exact χ² tail (Eq. 9); 1: the paper's GPU approximation, Alg. 3, called with the paper's units
+ * pow = 2S, dof = 2·shape (R31). */
+static double orc_lnp_of(int32_t signif_mode, int32_t shape, double S) {
+    if (signif_mode) return orc_power_to_logp(2.0 * S, 2.0 * (double)shape);
+    return orc_ln_q(shape, S);
+}
+
+/* … and with signif_mode = 1 every ln p comes from Alg. 3's polynomial instead of the exact tail (the paper's GPU-native
+ * configuration: Alg. 1 + Alg. 3 + log-spaced widths + harmonic sum, L544, Fig. 10); the reduction over widths, the
+ * threshold (ln p <= ln sf(σ_thr): "compared with precomputed threshold values", L342-344) and σ = Φ_sf⁻¹(e^{ln p}) then
+ * use that value.  Nothing else changes. */
+int64_t orc_search_all(const float* spectra, int64_t batch, int64_t n, int64_t pitch, int32_t zmax, int64_t B,
+                       int64_t C, double sigma_threshold, double n_trials, int32_t z_step, int32_t log_sampling,
+                       int32_t r_block, int32_t numharm, int32_t norm_mode, int32_t per_width, int32_t signif_mode,
+                       orc_candidate* out, int64_t cap) {
     double ln_trials = log(n_trials);
     double lnp_thr = orc_ln_sf(sigma_threshold);
     double* P = (double*)malloc((size_t)n * sizeof(double));
@@ -413,7 +463,7 @@ int64_t orc_search_opts(const float* spectra, int64_t batch, int64_t n, int64_t 
                     for (int32_t w = 1; w <= zmax; ++w) {
                         if (I[w - 1] < 0) continue;
                         if (!orc_width_searched(w, z_step, log_sampling)) continue;
-                        double lnp = orc_ln_q(w * kappa, M[w - 1]) + ln_trials;
+                        double lnp = orc_lnp_of(signif_mode, w * kappa, M[w - 1]) + ln_trials;
                         if (lnp > 0.0) lnp = 0.0;
                         if (lnp < best_lnp) { best_lnp = lnp; best_w = w; }
                     }
@@ -447,7 +497,7 @@ int64_t orc_search_opts(const float* spectra, int64_t batch, int64_t n, int64_t 
                     orc_block_maxima(Y, nH, zmax, C, c, sums, M, I);
                     for (int32_t w = 1; w <= zmax; ++w) {
                         if (I[w - 1] < 0 || !orc_width_searched(w, z_step, log_sampling)) continue;
-                        double lnp = orc_ln_q(w * kappa, M[w - 1]) + ln_trials;
+                        double lnp = orc_lnp_of(signif_mode, w * kappa, M[w - 1]) + ln_trials;
                         if (lnp > 0.0) lnp = 0.0;
                         if (lnp > lnp_thr) continue;
                         orc_candidate r;
