@@ -123,6 +123,15 @@ int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_
  * over-estimates the median of the skewed |deviation| distribution), so it is a fast mode, not the parity path. */
 int pulscan_plan_set_normalisation(pulscan_plan* plan, int32_t mode);
 
+/* Significance function.  0 (default): the exact χ² tail, ln p = ln Q(shape, S) (L154-158, Eq. 9).  1: the paper's GPU method,
+ * Algorithm 3 "Power to Log Probability Calculation" (L656-662; §2.6 Eq. 10-12): ln p ≈ pow·f(x)/1500 with
+ * x = 1500·dof/pow, f the printed degree-16 polynomial, and ln p = 0 when dof ≥ 1.05·pow; called with the paper's units
+ * pow = 2S, dof = 2·shape (R31).  The reduction over widths, the threshold and sigma then use that value, and the per-width
+ * power thresholds of the sweep follow it.  An APPROXIMATION, error-profiled in DESIGN.md §9: 0 … 4.5 nats less significant
+ * than the exact tail while x ≲ 1000 (widths ≲ 150 at σ 6), divergent beyond (the printed 8-digit coefficients no longer
+ * determine f): a fast mode, not the parity path.  The plan must be attached again afterwards. */
+int pulscan_plan_set_significance(pulscan_plan* plan, int32_t mode);
+
 /* What is emitted per candidate block.  per_width = 0 (default): the width with the largest σ (step 6 above, R13), at most
  * one record per block.  per_width = 1: the paper's GPU output, one record per (block, searched width) whose maximum reaches
  * the threshold (Alg. 4 "write out local candidate", ranked by σ afterwards, L322) — `capacity` records must then
@@ -168,6 +177,17 @@ int pulscan_search_host(pulscan_plan* plan, const void* h_spectra, pulscan_candi
  * [batch][pulscan_plan_power_pitch()] (bins ≥ n_bins of a row are unspecified). */
 int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_power, void* cuda_stream);
 int64_t pulscan_plan_power_pitch(const pulscan_plan* plan);
+
+/* Steps 1-2 in the form the default search keeps them in HBM (for unit tests and profiling): instead of the power of every
+ * bin, d_group_sums receives float32 [batch][pulscan_plan_group_pitch()] with G[k] = (P[4k] + P[4k+1]) + (P[4k+2] + P[4k+3])
+ * (bins ≥ n_bins count as 0; entries ≥ ceil(n_bins/4) are unspecified), and d_block_stats float32
+ * [batch][max(1, n_bins div norm_block)][8] with, per normalisation block, (a, inv, k) of the real parts then of the imaginary
+ * parts (two unused floats): x' = fma(v − a, inv, k) is the normalised component ((v − median)/(κ·MAD)/√2: a = the lower central
+ * value, k = −(median − a)·inv) and P = fma(x', x', y'·y').  Needs norm_block % 4 = 0, the exact normalisation and an
+ * attached workspace; both arrays 32-byte aligned. */
+int pulscan_normalise_group_sums(pulscan_plan* plan, const void* d_spectra, float* d_group_sums, float* d_block_stats,
+                                 void* cuda_stream);
+int64_t pulscan_plan_group_pitch(const pulscan_plan* plan);
 
 /* Introspection (host only).  thresholds: h_T[w−1] = the power at which width w reaches the σ threshold
  * (zmax doubles).  describe: a human-readable dump of the plan (levels of the pruned sweep, sizes); returns the

@@ -34,6 +34,7 @@ SIGNATURES = {
     "pulscan_plan_set_width_sampling": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int32]),
     "pulscan_plan_set_normalisation": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_r_block": (ctypes.c_int, [_P, ctypes.c_int32]),
+    "pulscan_plan_set_significance": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_set_emission": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int64]),
     "pulscan_plan_set_harmonics": (ctypes.c_int, [_P, ctypes.c_int32]),
     "pulscan_plan_max_hcandidates": (ctypes.c_int64, [_P]),
@@ -48,6 +49,8 @@ SIGNATURES = {
     "pulscan_search_host": (ctypes.c_int, [_P, _P, _P, _P, _P]),
     "pulscan_normalise_power": (ctypes.c_int, [_P, _P, _P, _P]),
     "pulscan_plan_power_pitch": (ctypes.c_int64, [_P]),
+    "pulscan_normalise_group_sums": (ctypes.c_int, [_P, _P, _P, _P, _P]),
+    "pulscan_plan_group_pitch": (ctypes.c_int64, [_P]),
     "pulscan_plan_get_thresholds": (ctypes.c_int, [_P, _P]),
     "pulscan_plan_describe": (ctypes.c_int64, [_P, _P, ctypes.c_int64]),
     "pulscan_plan_get_stats": (ctypes.c_int, [_P, _P, _P]),
@@ -105,7 +108,7 @@ class Plan:
                  norm_block: Optional[int] = None, n_trials: Optional[float] = None, pitch: Optional[int] = None,
                  mode: int = 0, tile: int = 0, log10_p_flag: float = 0.0, host_staging: bool = False,
                  cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False, numharm: int = 1,
-                 median_of_medians: bool = False, per_width_capacity: int = 0):
+                 median_of_medians: bool = False, per_width_capacity: int = 0, poly_logp: bool = False):
         self.lib = load_library()
         self.n_bins, self.batch, self.zmax, self.block_width = int(n_bins), int(batch), int(zmax), int(block_width)
         self.handle = self.lib.pulscan_plan_create(n_bins, batch, zmax, block_width, sigma_threshold)
@@ -132,6 +135,8 @@ class Plan:
         self.capacity = int(per_width_capacity)
         if median_of_medians:
             _check(self.lib.pulscan_plan_set_normalisation(self.handle, 1))
+        if poly_logp:
+            _check(self.lib.pulscan_plan_set_significance(self.handle, 1))
         if numharm != 1:
             _check(self.lib.pulscan_plan_set_harmonics(self.handle, numharm))
         self.numharm = int(numharm)
@@ -174,7 +179,11 @@ class Plan:
         return buf.value.decode()
 
     def set_mode(self, mode: int) -> None:
+        """0 pruned, 1 exhaustive.  The workspace layout follows the mode (the exhaustive sweep keeps the per-bin power array),
+        so an attached plan is attached again."""
         _check(self.lib.pulscan_plan_set_mode(self.handle, mode))
+        if self.workspace is not None:
+            self.attach(self.workspace.device)
 
     # ---- device side
     def attach(self, device="cuda") -> "Plan":
@@ -247,6 +256,16 @@ class Plan:
         out = torch.empty((self.batch, self.power_pitch), dtype=torch.float32, device=d_spectra.device)
         _check(self.lib.pulscan_normalise_power(self.handle, d_spectra.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
         return out[:, : self.n_bins]
+
+    def normalise_group_sums(self, d_spectra: torch.Tensor, norm_block: int, stream: Optional[torch.cuda.Stream] = None):
+        """Steps 1-2 as the default search keeps them: (G [batch, ceil(n/4)], stats [batch, nb, 8])."""
+        pitch = int(self.lib.pulscan_plan_group_pitch(self.handle))
+        nb = max(1, self.n_bins // int(norm_block))
+        G = torch.empty((self.batch, pitch), dtype=torch.float32, device=d_spectra.device)
+        st = torch.zeros((self.batch, nb, 8), dtype=torch.float32, device=d_spectra.device)
+        _check(self.lib.pulscan_normalise_group_sums(self.handle, d_spectra.data_ptr(), G.data_ptr(), st.data_ptr(),
+                                                     _stream_ptr(stream)))
+        return G[:, : (self.n_bins + 3) // 4], st
 
     def stats(self, stream: Optional[torch.cuda.Stream] = None) -> np.ndarray:
         h = np.zeros(16, dtype=np.uint32)

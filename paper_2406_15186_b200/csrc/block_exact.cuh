@@ -17,6 +17,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/pulscan.h"
+#include "power_source.cuh"
 #include "significance.cuh"
 
 namespace pulscan {
@@ -52,8 +53,8 @@ __device__ __forceinline__ void emit_candidate(long long row, int32_t bin, int w
 }
 
 __global__ void __launch_bounds__(kExactThreads)
-block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, int zmax, int C, long long nblk,
-                   const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int numharm,
+block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long long nblk,
+                   const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int signif_mode, int numharm,
                    pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity,
                    const unsigned* __restrict__ flagged, const unsigned* __restrict__ counters,
                    pulscan_candidate* __restrict__ out, unsigned* __restrict__ out_count) {
@@ -74,14 +75,14 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
         long long end = hi + zmax - 1;              // last bin any window of the block can touch, exclusive: hi−1+zmax
         if (end > n) end = n;
         const int L = (int)(end - lo);
-        const float* src = P + row * pitchP + lo;
+        PowerSource::Row src(src_pw, row);
 
         // double-precision exclusive prefix sum: pre[j] = Σ_{t<j} P[lo+t]
         const int chunk = (L + kExactThreads - 1) / kExactThreads;
         const int a = tid * chunk;
         const int b = min(a + chunk, L);
         double s = 0.0;
-        for (int j = a; j < b; ++j) s += (double)__ldg(src + j);
+        for (int j = a; j < b; ++j) s += (double)src(lo + j);
         hdr.part[tid] = s;
         __syncthreads();
         if (tid < 32) { // scan of the 512 chunk sums by one warp, 16 each
@@ -102,7 +103,7 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
         __syncthreads();
         {
             double run = hdr.part[tid];
-            for (int j = a; j < b; ++j) { pre[j] = run; run += (double)__ldg(src + j); }
+            for (int j = a; j < b; ++j) { pre[j] = run; run += (double)src(lo + j); }
             if (b == L && a < L) pre[L] = run;
             if (L == 0 && tid == 0) pre[0] = 0.0;
         }
@@ -120,7 +121,8 @@ block_exact_kernel(const float* __restrict__ P, long long pitchP, long long n, i
                 if (v > best) { best = v; arg = i; }
             }
             if (arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
-                double lnp = ln_q(w * shape_mult, best) + ln_trials;   // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220)
+                // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220); signif_mode 1: Alg. 3's polynomial instead of the tail
+                double lnp = lnp_of(signif_mode, w * shape_mult, best) + ln_trials;
                 if (lnp > 0.0) lnp = 0.0;
                 if (per_width) {   // the paper's GPU output: one candidate per (block, searched width) above the threshold (Alg. 4)
                     if (lnp <= lnp_thr)

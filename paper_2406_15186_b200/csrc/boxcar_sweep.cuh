@@ -33,6 +33,8 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+#include "power_source.cuh"
+
 namespace pulscan {
 
 constexpr int kMaxLevels = 8;
@@ -77,7 +79,7 @@ struct SweepParams {
     int arr_lg[kMaxLevels];
     int arr_off[kMaxLevels];
     int npass;       // scan passes per tile = ceil(len / kScanPass)
-    int z_floats;    // floats of ONE landing buffer: len + kScanPer zeros, rounded up to 4
+    int z_floats;    // floats of ONE landing buffer: len + kScanPer zeros (len/4 + kScanPer/4 for group-sum input), rounded up to 4
     int smem_floats; // two landing buffers + decimated arrays
     int ref_span;    // longest span of bins a listed cell covers (sweep_refine_kernel's shared memory per warp)
     SweepLevel lv[kMaxLevels];
@@ -154,9 +156,12 @@ __device__ __forceinline__ float scan_sel5(const float (&s)[5], int q) {
 // FINE = true additionally keeps the prefix inside each quad (x[3q+t] = the quad's first t+1 powers) and writes the arrays
 // with g = 1 and g = 2 (PG0 = PP itself, PG1): needed when a level's covers must be finer than 4 bins — harmonic-summed
 // spectra, whose noise level per bin is H(H+1)/2, and very low σ thresholds.
-template <bool FINE, class AfterLoads>
+// FROMG = true: `raw` holds the tile's group sums G[k] = P[4k] + … + P[4k+3] (written by kernel (a), norm_power.cuh)
+// instead of the powers: a thread's five quad sums are five loads (20-byte lane stride: conflict-free).
+template <bool FINE, bool FROMG, class AfterLoads>
 __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* raw, float* sG, ScanSmem& ss,
                                            AfterLoads after_loads) {
+    static_assert(!(FINE && FROMG), "levels finer than four bins need the powers themselves");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int len = sp.len;
     float carry = 0.f;
@@ -165,7 +170,13 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
         const bool act = i0 < len;
         float s[5];
         float x[FINE ? 15 : 1];
-        if (act) {
+        if (act && FROMG) {
+            const float* gq = raw + (i0 >> 2);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) s[q] = gq[q];
+#pragma unroll
+            for (int q = 1; q < 5; ++q) s[q] += s[q - 1];
+        } else if (act) {
             const float4* zq = reinterpret_cast<const float4*>(raw) + (i0 >> 2);
 #pragma unroll
             for (int q = 0; q < 5; ++q) {
@@ -347,12 +358,14 @@ __device__ __forceinline__ void mark_block(unsigned long long gid, unsigned* __r
 // Thread 0: start the TMA copy of tile `item` into `dst`.  The copy is clipped to the row's allocation (pitchP), so it
 // never touches the next spectrum (R11); P rows start 16-byte aligned and pitchP, tile and len are multiples of 4, so the
 // copy always satisfies TMA's alignment rules.
+template <bool FROMG>
 __device__ __forceinline__ void sweep_issue_tile(const SweepParams& sp, long long item, const float* __restrict__ P,
                                                  long long pitchP, int tiles_per_row, float* dst, uint64_t* mbar) {
     const long long row = item / tiles_per_row;
-    const long long t0 = (item - row * tiles_per_row) * sp.tile;
+    const long long t0 = ((item - row * tiles_per_row) * sp.tile) >> (FROMG ? 2 : 0);   // in elements of the input array
+    const long long want = sp.len >> (FROMG ? 2 : 0);
     const long long avail = pitchP - t0;
-    const uint32_t bytes = (uint32_t)(avail < (long long)sp.len ? avail : (long long)sp.len) * 4u;
+    const uint32_t bytes = (uint32_t)(avail < want ? avail : want) * 4u;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // the buffer's earlier generic accesses precede the copy
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(mbar)), "r"(bytes) : "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -380,7 +393,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
 // counters[2] = cells appended (the refine kernel's work count), counters[3] = cells dropped because the list was full
 // (their tile's blocks are all marked instead, which is always allowed: kernel (c) decides).
 // Dynamic shared memory: [kSweepBufs × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
-template <bool FINE>
+// FROMG = true: P / pitchP are the group-sum array G and its pitch (see scan_tile).
+template <bool FINE, bool FROMG>
 __global__ void __launch_bounds__(kSweepThreads, PULSCAN_SWEEP_OCC)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
@@ -397,7 +411,10 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
     // ---- once per CTA: τ table, zeros after len and in the arrays (PG[0] = 0, pads), task list, the first two copies
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
     for (int i = tid; i < sp.smem_floats - kSweepBufs * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;
-    if (tid < kSweepBufs * kScanPer) raw0[(tid / kScanPer) * sp.z_floats + sp.len + tid % kScanPer] = 0.f;
+    if (tid < kSweepBufs * kScanPer) {   // zeros after the copied elements (a thread's five quads may start before and end after them)
+        const int pos = (FROMG ? (sp.len >> 2) : sp.len) + tid % kScanPer;
+        if (pos < sp.z_floats) raw0[(tid / kScanPer) * sp.z_floats + pos] = 0.f;
+    }
     for (int q = tid; q < sp.ntasks; q += kSweepThreads) {
         int L = 0;
         while (L + 1 < sp.nlevels && q >= sp.lv[L + 1].wt_off) ++L;
@@ -413,7 +430,7 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
         const long long i0 = blockIdx.x;
         for (int b = 0; b < kSweepBufs; ++b)
             if (i0 + b * stride < n_items)
-                sweep_issue_tile(sp, i0 + b * stride, P, pitchP, tiles_per_row, raw0 + b * sp.z_floats, &ctl.mbar[b]);
+                sweep_issue_tile<FROMG>(sp, i0 + b * stride, P, pitchP, tiles_per_row, raw0 + b * sp.z_floats, &ctl.mbar[b]);
     }
 
     // (row, tile index) of the current item, advanced without divisions
@@ -429,12 +446,14 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
         mbar_wait(&ctl.mbar[b], (uint32_t)(it / kSweepBufs) & 1u);
         const long long nv = n - (long long)tix * sp.tile;      // valid bins from the tile's first one
         if (nv < (long long)sp.len) {                            // last tile of a row: nothing beyond the spectrum's end
-            for (int i = (int)nv + tid; i < sp.len; i += kSweepThreads) raw[i] = 0.f;
+            // (group sums: the group holding the last bin is kept, kernel (a) added zeros for its missing bins)
+            const int first = FROMG ? (int)((nv + 3) >> 2) : (int)nv, end = FROMG ? (sp.len >> 2) : sp.len;
+            for (int i = first + tid; i < end; i += kSweepThreads) raw[i] = 0.f;
             __syncthreads();
         }
-        const float pp_max = scan_tile<FINE>(sp, raw, sG, ctl.scan, [&] {
+        const float pp_max = scan_tile<FINE, FROMG>(sp, raw, sG, ctl.scan, [&] {
             const long long nxt = item + kSweepBufs * stride;
-            if (tid == 0 && nxt < n_items) sweep_issue_tile(sp, nxt, P, pitchP, tiles_per_row, raw, &ctl.mbar[b]);
+            if (tid == 0 && nxt < n_items) sweep_issue_tile<FROMG>(sp, nxt, P, pitchP, tiles_per_row, raw, &ctl.mbar[b]);
         });
         const float slack = kSlackUlps * 5.9604644775390625e-8f * pp_max;
 
@@ -471,7 +490,7 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
 // are summed and compared with T'_w.  A window that passes marks the candidate block of its start bin.
 // Dynamic shared memory: (kRefineThreads/32) × (ref_span + 1) doubles.
 __global__ void __launch_bounds__(kRefineThreads)
-sweep_refine_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
+sweep_refine_kernel(const __grid_constant__ SweepParams sp, const PowerSource src_pw, long long n,
                     int tiles_per_row, int C, long long nblk, const float* __restrict__ tau_g,
                     const float* __restrict__ Tp_g, const SweepCell* __restrict__ cells, unsigned cell_cap,
                     unsigned* __restrict__ bitmap, unsigned* __restrict__ flagged, unsigned* __restrict__ counters) {
@@ -490,10 +509,24 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const float* __restr
         const int span = (m4 + 10) << lg;                        // ≤ ref_span
         const long long room = n - base;
         const int valid = (int)(room < (long long)span ? (room < 0 ? 0 : room) : (long long)span);
-        const float* src = P + row * pitchP + base;
+        // Nothing left to find if every candidate block that owns a start bin of this cell is already marked (a strong
+        // signal flags many cells over the same few blocks; kernel (c) evaluates a marked block completely anyway).
+        {
+            const long long s_last = min(base + (8ll << lg), n) - 1;          // last start bin of the cell
+            const long long c0 = base / C, c1 = s_last / C;
+            if (s_last >= base && c1 - c0 < 32) {
+                bool marked = true;
+                if (c0 + lane <= c1) {
+                    const unsigned long long gid = (unsigned long long)(row * nblk + c0 + lane);
+                    marked = (__ldcg(bitmap + (gid >> 5)) >> (gid & 31)) & 1u;
+                }
+                if (__all_sync(0xffffffffu, marked)) continue;
+            }
+        }
+        PowerSource::Row src(src_pw, row);
         // ---- prefix sum in double: stage the span (coalesced loads, several in flight), then each lane scans its own
         //      chunk of L consecutive bins and the chunk totals are scanned across the warp
-        for (int j = lane; j < span; j += 32) pp[j + 1] = (j < valid) ? (double)__ldg(src + j) : 0.0;
+        for (int j = lane; j < span; j += 32) pp[j + 1] = (j < valid) ? (double)src(base + j) : 0.0;
         if (lane == 0) pp[0] = 0.0;
         __syncwarp();
         const int L = (span + 31) >> 5;
@@ -519,6 +552,17 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             const int rr = srcl & 7, mm = m4 + (srcl >> 3);
             const int i0 = rr << lg, e0 = (rr + mm - 1) << lg;
             if (g <= C) {   // nothing left to find if the (one or two) blocks owning the cover's start bins are already marked
+                const unsigned long long ga = (unsigned long long)(row * nblk + (base + i0) / C);
+                const unsigned long long gb = (unsigned long long)(row * nblk + min(base + i0 + g - 1, n - 1) / C);
+                const unsigned wa = __ldcg(bitmap + (ga >> 5)), wb = __ldcg(bitmap + (gb >> 5));
+                if ((wa >> (ga & 31) & 1u) && (wb >> (gb & 31) & 1u)) continue;
+            }
+            if (g >= 8 && g <= C) {   // 32 windows spread over the cover first: a real signal passes here and marks its block(s)
+                const int i = i0 + ((lane << lg) >> 5), ee = e0 + ((((lane * 11) & 31) << lg) >> 5);
+                const int w = ee - i + 1;
+                if (w >= 1 && w >= lv.wlo && w <= lv.whi && ee < valid && pp[ee + 1] - pp[i] >= (double)__ldg(Tp_g + (w - 1)))
+                    mark_block((unsigned long long)(row * nblk + (base + i) / C), bitmap, flagged, counters);
+                __syncwarp();
                 const unsigned long long ga = (unsigned long long)(row * nblk + (base + i0) / C);
                 const unsigned long long gb = (unsigned long long)(row * nblk + min(base + i0 + g - 1, n - 1) / C);
                 const unsigned wa = __ldcg(bitmap + (ga >> 5)), wb = __ldcg(bitmap + (gb >> 5));

@@ -40,6 +40,53 @@ __device__ __forceinline__ unsigned float_key(float v) {
     return b ^ ((b >> 31) ? 0xFFFFFFFFu : 0x80000000u);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// What kernel (a) leaves behind for the rest of the search.  Either (or both) of:
+//   P  float32 [batch][pitchP]: the normalised power of every bin (pulscan_normalise_power, the exhaustive sweep, the
+//      full-resolution sweep of very low thresholds, the harmonic sum);
+//   G  float32 [batch][pitchG]: G[k] = (P[4k] + P[4k+1]) + (P[4k+2] + P[4k+3]), the sums of aligned groups of four bins
+//      (zeros beyond n_bins) — all the streaming sweep needs, a quarter of the bytes — together with
+//   stats float32 [batch][nb][8]: per normalisation block (a, inv, k) of the real and of the imaginary parts, from which
+//      any bin's power is rebuilt bit-identically by norm_power_value() wherever a flagged span needs it.
+struct NormOut {
+    float* P;            // may be null
+    long long pitchP;
+    float* G;            // may be null; needs B % 4 == 0
+    long long pitchG;
+    float* stats;        // null iff G is null
+};
+
+// The normalised power of one bin.  x' = ((v − a) − h)·inv is evaluated as fma(v − a, inv, k), k = −h·inv, and
+// P = fma(x', x', y'·y'); every kernel that produces or rebuilds a power goes through this function.
+__device__ __forceinline__ float norm_power_value(float2 z, float a0, float i0, float k0, float a1, float i1, float k1) {
+    const float x = __fmaf_rn(__fsub_rn(z.x, a0), i0, k0), y = __fmaf_rn(__fsub_rn(z.y, a1), i1, k1);
+    return __fmaf_rn(x, x, __fmul_rn(y, y));
+}
+
+// Quad sums of four rounds of powers: p0..p3 belong to bins lane_bin + (r0 + q)·NT, q = 0..3, where the four lanes
+// 4j..4j+3 of a warp hold four consecutive bins of an aligned group.  A transposing butterfly (3 shuffles for 4 sums)
+// leaves in lane 4j + q the sum of round r0 + q, always added as (p[0] + p[1]) + (p[2] + p[3]) up to commutation.
+__device__ __forceinline__ float quad_sums4(float p0, float p1, float p2, float p3) {
+    const int q = threadIdx.x & 3;
+    float a = (q & 1) ? p1 : p0;
+    const float b = (q & 1) ? p0 : p1;
+    a += __shfl_xor_sync(0xffffffffu, b, 1);
+    float c = (q & 1) ? p3 : p2;
+    const float d = (q & 1) ? p2 : p3;
+    c += __shfl_xor_sync(0xffffffffu, d, 1);
+    float e = (q & 2) ? c : a;
+    const float f = (q & 2) ? a : c;
+    e += __shfl_xor_sync(0xffffffffu, f, 2);
+    return e;
+}
+
+// One round only (block lengths that are not a multiple of 4·NT): every lane of a group ends up with the group's sum.
+__device__ __forceinline__ float quad_sum1(float p) {
+    p += __shfl_xor_sync(0xffffffffu, p, 1);
+    p += __shfl_xor_sync(0xffffffffu, p, 2);
+    return p;
+}
+
 // Monotone non-decreasing map of a value in [lo, hi] to a bucket in [0, 255].  Explicit round-to-nearest
 // intrinsics: the histogram pass and the gather pass must compute the same bucket, so no FMA contraction.
 struct BucketMap {
@@ -220,9 +267,53 @@ __device__ __forceinline__ float normalise_component(float (&v)[EPT], int len, S
 // One normalisation block by the general path: len values at src → powers at dst.  The normalised component
 // ((v − a) − h)·inv is evaluated as fma(v − a, inv, −h·inv) from the re-read input (the registers hold |v − m| by
 // then); norm_power_v2.cuh uses the same expression, so both paths produce identical bits.
+// Write one block's outputs from its statistics: len bins at src → P and/or (G, stats).  Bin tid + r·NT belongs to thread
+// tid; lo is the block's first bin in its row (a multiple of 4 when G is written), `blk` its index in [batch][nb].
 template <int EPT, int NT>
-__device__ __forceinline__ void norm_block_general(const float2* __restrict__ src, int len, float* __restrict__ dst,
-                                                   SelectSmem& sm) {
+__device__ __forceinline__ void norm_block_write(const float2* __restrict__ src, int len, long long row, long long lo, long long blk,
+                                                 const NormOut& out, float a0, float i0, float k0, float a1, float i1, float k1) {
+    const int tid = threadIdx.x;
+    if (out.P) {
+        float* dst = out.P + row * out.pitchP + lo;
+#pragma unroll
+        for (int r = 0; r < EPT; ++r) {
+            const int idx = tid + r * NT;
+            if (idx < len) dst[idx] = norm_power_value(__ldg(src + idx), a0, i0, k0, a1, i1, k1);
+        }
+    }
+    if (out.G) {
+        float* g = out.G + row * out.pitchG + (lo >> 2);
+        auto pw = [&](int r) {
+            const int idx = tid + r * NT;
+            return idx < len ? norm_power_value(__ldg(src + idx), a0, i0, k0, a1, i1, k1) : 0.f;
+        };
+        if constexpr (EPT % 4 == 0) {
+#pragma unroll
+            for (int r0 = 0; r0 < EPT; r0 += 4) {
+                const float e = quad_sums4(pw(r0), pw(r0 + 1), pw(r0 + 2), pw(r0 + 3));
+                const int r = r0 + (tid & 3);
+                if ((tid & ~3) + r * NT < len) g[(tid >> 2) + r * (NT / 4)] = e;   // the group's first bin exists
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < EPT; ++r) {
+                const float e = quad_sum1(pw(r));
+                if ((tid & 3) == 0 && tid + r * NT < len) g[(tid >> 2) + r * (NT / 4)] = e;
+            }
+        }
+        if (tid == 0) {
+            float* st = out.stats + blk * 8;
+            st[0] = a0; st[1] = i0; st[2] = k0; st[3] = a1; st[4] = i1; st[5] = k1;
+        }
+    }
+}
+
+// One normalisation block by the general path: len values at src → outputs.  The statistics are found on
+// register-resident values; the outputs are then computed from the re-read input (the registers hold |v − m| by then)
+// through norm_power_value(), as in norm_power_v2.cuh, so both paths produce identical bits.
+template <int EPT, int NT>
+__device__ __forceinline__ void norm_block_general(const float2* __restrict__ src, int len, long long row, long long lo,
+                                                   long long blk, const NormOut& out, SelectSmem& sm) {
     const int tid = threadIdx.x;
     float re[EPT], im[EPT];
 #pragma unroll
@@ -236,16 +327,7 @@ __device__ __forceinline__ void norm_block_general(const float2* __restrict__ sr
     float a_re, h_re, a_im, h_im;
     const float inv_re = normalise_component<EPT, NT>(re, len, sm, a_re, h_re);
     const float inv_im = normalise_component<EPT, NT>(im, len, sm, a_im, h_im);
-    const float k_re = -h_re * inv_re, k_im = -h_im * inv_im;
-#pragma unroll
-    for (int r = 0; r < EPT; ++r) {
-        const int idx = tid + r * NT;
-        if (idx < len) {
-            const float2 z = __ldg(src + idx);
-            const float x = __fmaf_rn(__fsub_rn(z.x, a_re), inv_re, k_re), y = __fmaf_rn(__fsub_rn(z.y, a_im), inv_im, k_im);
-            dst[idx] = __fmaf_rn(x, x, y * y);
-        }
-    }
+    norm_block_write<EPT, NT>(src, len, row, lo, blk, out, a_re, inv_re, -h_re * inv_re, a_im, inv_im, -h_im * inv_im);
 }
 
 // General kernel: one CTA per normalisation block.  Grid: blocks_per_row · batch CTAs; block j = first_block +
@@ -255,29 +337,29 @@ __device__ __forceinline__ void norm_block_general(const float2* __restrict__ sr
 template <int EPT, int NT>
 __global__ void __launch_bounds__(NT)
 norm_power_kernel(const float2* __restrict__ spectra, long long pitch_in, long long n, int B, int nb, int first_block,
-                  int blocks_per_row, float* __restrict__ P, long long pitchP) {
+                  int blocks_per_row, NormOut out) {
     __shared__ SelectSmem sm;
     const long long row = blockIdx.x / blocks_per_row;
     const int j = first_block + (int)(blockIdx.x % blocks_per_row);
     const long long lo = (long long)j * B;
     const long long hi = (j == nb - 1) ? n : lo + B;
-    norm_block_general<EPT, NT>(spectra + row * pitch_in + lo, (int)(hi - lo), P + row * pitchP + lo, sm);
+    norm_block_general<EPT, NT>(spectra + row * pitch_in + lo, (int)(hi - lo), row, lo, row * nb + j, out, sm);
 }
 
 // Redo kernel: the blocks the fast kernel declined (redo[e] = row·blocks_per_row + j, all of length B), by the general
 // path.  A fixed small grid loops over the list, whose length is only known on the device.
 template <int EPT, int NT>
 __global__ void __launch_bounds__(NT)
-norm_power_redo_kernel(const float2* __restrict__ spectra, long long pitch_in, int B, int blocks_per_row,
-                       float* __restrict__ P, long long pitchP, const unsigned* __restrict__ redo,
-                       const unsigned* __restrict__ redo_count) {
+norm_power_redo_kernel(const float2* __restrict__ spectra, long long pitch_in, int B, int nb, int blocks_per_row,
+                       NormOut out, const unsigned* __restrict__ redo, const unsigned* __restrict__ redo_count) {
     __shared__ SelectSmem sm;
     const unsigned cnt = *redo_count;
     for (unsigned e = blockIdx.x; e < cnt; e += gridDim.x) {
         const unsigned id = redo[e];
         const long long row = id / (unsigned)blocks_per_row;
-        const long long lo = (long long)(id % (unsigned)blocks_per_row) * B;
-        norm_block_general<EPT, NT>(spectra + row * pitch_in + lo, B, P + row * pitchP + lo, sm);
+        const long long j = id % (unsigned)blocks_per_row;
+        const long long lo = j * B;
+        norm_block_general<EPT, NT>(spectra + row * pitch_in + lo, B, row, lo, row * nb + j, out, sm);
         __syncthreads();
     }
 }

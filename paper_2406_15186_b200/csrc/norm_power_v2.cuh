@@ -390,8 +390,8 @@ constexpr size_t v2_smem_bytes() {
 // leaves 19 KB of shared memory per CTA so that more blocks are in flight per SM to cover the warp-serial phases.
 template <int EPT, int NT, bool STAGED>
 __global__ void __launch_bounds__(NT, STAGED ? ((EPT * NT <= 4096) ? 4 : 2) : (NT == 128 ? (EPT <= 16 ? PULSCAN_NORM_OCC128_SMALL : PULSCAN_NORM_OCC128) : (EPT * NT <= 4096) ? 6 : 4))
-norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int blocks_per_row, float* __restrict__ P,
-                     long long pitchP, unsigned* __restrict__ redo, unsigned* __restrict__ redo_count,
+norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int blocks_per_row, int nb, NormOut out,
+                     unsigned* __restrict__ redo, unsigned* __restrict__ redo_count,
                      const char* __restrict__ lim_lo, const char* __restrict__ lim_hi) {
     static_assert(EPT % 2 == 0 && EPT <= 32, "bucket indices are packed in pairs; hit mask has 16 + 16 bits");
     static_assert(NT % 32 == 0 && (EPT * NT) % 128 == 0, "sample stride");
@@ -509,12 +509,33 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         // x' = ((v − a) − h)·inv evaluated as fma(v − a, inv, −h·inv), as in the general path (norm_power.cuh)
         const float a0 = ctl.a[0], a1 = ctl.a[1], i0 = ctl.inv[0], i1 = ctl.inv[1];
         const float k0 = -ctl.h[0] * i0, k1 = -ctl.h[1] * i1;
-        float* dst = P + (long long)row * pitchP + lo_bin;
+        if (out.P) {
+            float* dst = out.P + (long long)row * out.pitchP + lo_bin;
 #pragma unroll
-        for (int r = 0; r < EPT; ++r) {
-            const float2 z = sdat[tid + r * NT];
-            const float x = __fmaf_rn(__fsub_rn(z.x, a0), i0, k0), y = __fmaf_rn(__fsub_rn(z.y, a1), i1, k1);
-            dst[tid + r * NT] = __fmaf_rn(x, x, y * y);
+            for (int r = 0; r < EPT; ++r) dst[tid + r * NT] = norm_power_value(sdat[tid + r * NT], a0, i0, k0, a1, i1, k1);
+        }
+        if (out.G) {   // sums of aligned groups of four bins (lanes 4j..4j+3 hold a group), see norm_power.cuh
+            float* g = out.G + (long long)row * out.pitchG + (lo_bin >> 2) + (tid >> 2);
+            if constexpr (EPT % 4 == 0) {
+#pragma unroll
+                for (int r0 = 0; r0 < EPT; r0 += 4) {
+                    const float e = quad_sums4(norm_power_value(sdat[tid + r0 * NT], a0, i0, k0, a1, i1, k1),
+                                               norm_power_value(sdat[tid + (r0 + 1) * NT], a0, i0, k0, a1, i1, k1),
+                                               norm_power_value(sdat[tid + (r0 + 2) * NT], a0, i0, k0, a1, i1, k1),
+                                               norm_power_value(sdat[tid + (r0 + 3) * NT], a0, i0, k0, a1, i1, k1));
+                    g[(r0 + (tid & 3)) * (NT / 4)] = e;
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < EPT; ++r) {
+                    const float e = quad_sum1(norm_power_value(sdat[tid + r * NT], a0, i0, k0, a1, i1, k1));
+                    if ((tid & 3) == 0) g[r * (NT / 4)] = e;
+                }
+            }
+            if (tid == 0) {
+                float* st = out.stats + ((long long)row * nb + jblk) * 8;
+                st[0] = a0; st[1] = i0; st[2] = k0; st[3] = a1; st[4] = i1; st[5] = k1;
+            }
         }
     } else if (tid == 0) {
         redo[atomicAdd(redo_count, 1u)] = blockIdx.x;   // the general path will do this block

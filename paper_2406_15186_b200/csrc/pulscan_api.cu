@@ -69,6 +69,7 @@ struct pulscan_plan {
     unsigned out_capacity = 0xFFFFFFFFu;     // records the output array can hold (per-width emission only; otherwise never exceeded)
     int64_t user_capacity = 0;
     int32_t norm_mode = 0;                   // 0 exact median/MAD; 1 the paper's median-of-medians approximation (Alg. 1)
+    int32_t signif_mode = 0;                 // 0 exact χ² tail (Eq. 9); 1 the paper's polynomial ln p (Alg. 3)
     int32_t numharm = 1;                     // harmonic-summed spectra searched by pulscan_search_harmonics (L201-220)
     int32_t shape_mult = 1;                  // H(H+1)/2 of the spectrum this plan searches: a width-w sum is Gamma(w·shape_mult)
     int32_t numharm_tag = 1;                 // the H written into pulscan_hcandidate records by this plan
@@ -86,6 +87,8 @@ struct pulscan_plan {
     int64_t nblk = 0;          // candidate blocks per spectrum
     int32_t nb = 0;            // normalisation blocks per spectrum
     int64_t pitchP = 0;
+    int64_t pitchG = 0;        // row pitch of the group-sum array G (floats): ceil(n/4) rounded up to 4
+    bool keep_P = false;       // the per-bin power array stays in the workspace (see derive); otherwise G + statistics only
     double lnp_thr = 0, ln_trials = 0;
     std::vector<double> T;     // T_w
     std::vector<float> Tp;     // conservative float thresholds for the float32 sweep
@@ -109,7 +112,7 @@ struct pulscan_plan {
     // workspace (device, caller-owned)
     void* ws = nullptr;
     size_t ws_bytes = 0;
-    size_t off_P = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_redo = 0, off_cells = 0, off_stage_in = 0, off_stage_cand = 0,
+    size_t off_P = 0, off_G = 0, off_stats = 0, off_bitmap = 0, off_flagged = 0, off_counters = 0, off_redo = 0, off_cells = 0, off_stage_in = 0, off_stage_cand = 0,
            off_stage_count = 0, bitmap_bytes = 0, need_bytes = 0;
     // device tables: T_w (double), T'_w and τ (float); they live in the caller's workspace (off_tables) and are uploaded by
     // pulscan_plan_set_workspace, so that the plan owns no device memory at all
@@ -156,6 +159,7 @@ int derive(pulscan_plan& p) {
     p.nblk = (p.n + p.C - 1) / p.C;
     p.nb = (int32_t)std::max<int64_t>(1, p.n / p.B);
     p.pitchP = (int64_t)align_up((size_t)p.n, 4);
+    p.pitchG = (int64_t)align_up((size_t)((p.n + 3) / 4), 4);
     p.lnp_thr = ln_sf(p.sigma_thr);
     p.ln_trials = std::log(p.n_trials);
     const double lnp_target = p.lnp_thr - p.ln_trials; // ln p_adj ≤ lnp_thr ⇔ ln p ≤ lnp_thr − ln N  (R15, R17)
@@ -169,7 +173,8 @@ int derive(pulscan_plan& p) {
     };
     p.pruned_error.clear();
     for (int w = 1; w <= p.zmax; ++w) {
-        p.T[w - 1] = searched(w) ? power_threshold(w * p.shape_mult, lnp_target) : INFINITY;
+        p.T[w - 1] = !searched(w) ? INFINITY
+                     : p.signif_mode ? power_threshold_poly(w * p.shape_mult, lnp_target) : power_threshold(w * p.shape_mult, lnp_target);
         p.Tp[w - 1] = searched(w) ? conservative_threshold(p.T[w - 1], w) : INFINITY;
     }
 
@@ -257,7 +262,6 @@ int derive(pulscan_plan& p) {
     const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
     sp.len = tile + halo;
     sp.npass = (sp.len + kScanPass - 1) / kScanPass;
-    sp.z_floats = (int)align_up((size_t)(sp.len + kScanPer), 4);
     int off = 0, task = 0;
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = lvls[l];
@@ -275,11 +279,11 @@ int derive(pulscan_plan& p) {
             if (m < lv.m_lo || m > lv.m_hi) { p.tau.push_back(INFINITY); continue; }
             const int wmin = (g == 1) ? m : (m == 1 ? 1 : (m - 2) * g + 2);
             // the lowest threshold among the level's searched widths whose windows have a cover of exactly m groups
-            // (widths wmin … m·g; T_w grows with w); +inf if there is none
+            // (widths wmin … m·g; the exact T_w grows with w, Alg. 3's need not); +inf if there is none
             const int wtop = std::min(lv.whi, m * g);
-            int wq = std::min(std::max(lv.wlo, wmin), lv.whi);
-            while (wq <= wtop && !std::isfinite(p.T[wq - 1])) ++wq;
-            p.tau.push_back(wq <= wtop ? conservative_threshold(p.T[wq - 1], m * g) : INFINITY);
+            double tmin = INFINITY;
+            for (int wq = std::min(std::max(lv.wlo, wmin), lv.whi); wq <= wtop; ++wq) tmin = std::min(tmin, p.T[wq - 1]);
+            p.tau.push_back(std::isfinite(tmin) ? conservative_threshold(tmin, m * g) : INFINITY);
         }
         // with sparse width sampling whole 4-wide steps can be dead (τ = +inf): trim them off both ends
         {
@@ -301,6 +305,15 @@ int derive(pulscan_plan& p) {
     sp.ntasks = task;
     p.sweep_fine = false;
     for (int a = 0; a < sp.narr; ++a) p.sweep_fine = p.sweep_fine || sp.arr_lg[a] < 2;
+    // Does the float32 power of every bin have to exist in HBM?  Not on the default path: kernel (a) then leaves only the sums
+    // of aligned groups of four bins (G, a quarter of the bytes) and six numbers per normalisation block, and the rare-path
+    // kernels rebuild the spans they need from the input spectrum (power_source.cuh).  It stays for: a child plan (its
+    // "power" is the harmonic-summed spectrum Y_H), the exhaustive cross-check mode, levels finer than four bins
+    // (full-resolution sweep), the harmonic search (Y_H is summed from P), the Alg. 1 normalisation kernel, and
+    // normalisation blocks that are not a multiple of four bins.  PULSCAN_KEEP_P forces it (comparison runs).
+    p.keep_P = p.is_child || p.mode == 1 || p.sweep_fine || p.numharm > 1 || p.norm_mode == 1 || (p.B & 3) != 0 ||
+               std::getenv("PULSCAN_KEEP_P") != nullptr;
+    sp.z_floats = p.keep_P ? (int)align_up((size_t)(sp.len + kScanPer), 4) : (int)align_up((size_t)(sp.len / 4 + 8), 4);
     if (task > kMaxWarpTasks) return fail(PULSCAN_EINVAL, "sweep tile of %d bins needs %d warp-tasks (limit %d)", tile, task, kMaxWarpTasks);
     sp.ntau = (int)p.tau.size();
     sp.smem_floats = kSweepBufs * sp.z_floats + off;
@@ -345,7 +358,9 @@ int derive(pulscan_plan& p) {
 
     // ---- workspace layout
     size_t o = 0;
-    p.off_P = o; o += align_up((size_t)p.batch * p.pitchP * 4, 256);
+    p.off_P = o; o += p.keep_P ? align_up((size_t)p.batch * p.pitchP * 4, 256) : 0;
+    p.off_G = o; o += p.keep_P ? 0 : align_up((size_t)p.batch * p.pitchG * 4, 256);
+    p.off_stats = o; o += p.keep_P ? 0 : align_up((size_t)p.batch * p.nb * 8 * sizeof(float), 256);
     p.bitmap_bytes = align_up((size_t)((p.batch * p.nblk + 31) / 32) * 4, 256);
     p.off_bitmap = o; o += p.bitmap_bytes;
     p.off_flagged = o; o += align_up((size_t)p.batch * p.nblk * 4, 256);
@@ -377,6 +392,7 @@ int derive(pulscan_plan& p) {
         pulscan_plan* c = pulscan_plan_create(nH, p.batch, p.zmax, p.C, (float)p.sigma_thr);
         if (!c) return PULSCAN_EINVAL;
         c->is_child = true; c->shape_mult = H * (H + 1) / 2; c->numharm_tag = H; c->sigma_thr = p.sigma_thr; c->n_trials = p.n_trials;
+        c->signif_mode = p.signif_mode;
         c->z_step = p.z_step; c->log_sampling = p.log_sampling; c->tile_user = p.tile_user; c->log10_p_flag = p.log10_p_flag;
         c->cell_cap_user = p.cell_cap_user; c->B = p.B;
         p.harm.push_back(c);
@@ -397,6 +413,13 @@ int derive(pulscan_plan& p) {
 // function ON THE CURRENT DEVICE, so it is set at every finalisation rather than once per process), launch shapes from the
 // occupancy API.  Synchronous; never called from pulscan_search.
 int set_kernel_attributes(const pulscan_plan& p);
+
+using SweepFn = void (*)(const SweepParams, const float*, long long, long long, int, long long, int, long long, const float*,
+                         SweepCell*, unsigned, unsigned*, unsigned*, unsigned*);
+SweepFn sweep_function(const pulscan_plan& p) {
+    if (!p.keep_P) return boxcar_sweep_kernel<false, true>;
+    return p.sweep_fine ? boxcar_sweep_kernel<true, false> : boxcar_sweep_kernel<false, false>;
+}
 
 int finalize_device(pulscan_plan& p) {
     p.finalized = false;
@@ -422,7 +445,7 @@ int finalize_device(pulscan_plan& p) {
                     p.smem_sweep, p.smem_exh, p.smem_exact);
     int rc = set_kernel_attributes(p);
     if (rc) return rc;
-    const auto sweep_fn = p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>;
+    const SweepFn sweep_fn = sweep_function(p);
     int occ = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_fn, kSweepThreads, p.smem_sweep));
     if (occ < 1) return fail(PULSCAN_ECUDA, "boxcar_sweep_kernel does not fit an SM with %zu bytes of shared memory", p.smem_sweep);
@@ -454,8 +477,9 @@ void invalidate(pulscan_plan& p) {
 int set_kernel_attributes(const pulscan_plan& p) {
     (void)p;
     constexpr int kMaxDynSmem = 227 * 1024;
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
@@ -468,11 +492,10 @@ int set_kernel_attributes(const pulscan_plan& p) {
 
 template <int NT>
 int launch_norm(int ept, int grid, cudaStream_t st, const float2* spectra, long long pitch_in, long long n, int B, int nb,
-                int first_block, int blocks_per_row, float* P, long long pitchP) {
+                int first_block, int blocks_per_row, const NormOut& out) {
 #define PULSCAN_NORM_CASE(E)                                                                                      \
     case E:                                                                                                       \
-        norm_power_kernel<E, NT><<<grid, NT, 0, st>>>(spectra, pitch_in, n, B, nb, first_block, blocks_per_row, P, \
-                                                      pitchP);                                                    \
+        norm_power_kernel<E, NT><<<grid, NT, 0, st>>>(spectra, pitch_in, n, B, nb, first_block, blocks_per_row, out); \
         break;
     switch (ept) {
         PULSCAN_NORM_CASE(1)
@@ -493,17 +516,17 @@ int launch_norm(int ept, int grid, cudaStream_t st, const float2* spectra, long 
 constexpr int kRedoGrid = 148;
 
 // Fast kernel for the full blocks + redo kernel (general path) for the blocks it declined.
-int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* spec, float* P, unsigned* redo,
+int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* spec, const NormOut& out, unsigned* redo,
                      unsigned* redo_count) {
     const char* lim_lo = reinterpret_cast<const char*>(spec);
     const char* lim_hi = lim_lo + ((size_t)(p.batch - 1) * p.pitch + p.n) * 8;
 #define PULSCAN_V2_LAUNCH(E, NT_, ST)                                                                                 \
     {                                                                                                                 \
         norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                              \
-            spec, p.pitch, p.main_blocks_per_row, P, p.pitchP, redo, redo_count, lim_lo, lim_hi);                     \
+            spec, p.pitch, p.main_blocks_per_row, p.nb, out, redo, redo_count, lim_lo, lim_hi);                       \
     }
 #define PULSCAN_V2_REDO(E)                                                                                            \
-    norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.main_blocks_per_row, P, p.pitchP, redo, \
+    norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.nb, p.main_blocks_per_row, out, redo, \
                                                               redo_count);
     // key = threads per CTA · 64 + values per thread of the single-histogram kernel (B = their product)
     switch (p.norm_nt * 64 + p.B / p.norm_nt) {
@@ -534,11 +557,13 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
 
 // d_scratch: the redo list and its counter (inside the workspace for pulscan_search; a temporary for the stand-alone
 // pulscan_normalise_power, which has no workspace).  redo_count must be zero on entry.
-int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStream_t st, unsigned* d_redo,
+int enqueue_norm(pulscan_plan& p, const void* d_spectra, const NormOut& out, cudaStream_t st, unsigned* d_redo,
                  unsigned* d_redo_count) {
+    float* d_power = out.P;
     const float2* spec = reinterpret_cast<const float2*>(d_spectra);
     int rc = PULSCAN_OK;
     if (p.norm_mode == 1) {   // Alg. 1: one kernel for every chunk, the last one of a row included
+        if (!d_power) return fail(PULSCAN_EINVAL, "internal: the Alg. 1 kernel writes the per-bin power array");
         const long long grid = (long long)p.nb * p.batch;
         if (grid > 2147483647LL) return fail(PULSCAN_EINVAL, "too many normalisation blocks for one launch");
 #define PULSCAN_MOM_CASE(E, NT_)                                                                                      \
@@ -563,25 +588,29 @@ int enqueue_norm(pulscan_plan& p, const void* d_spectra, float* d_power, cudaStr
         const long long grid = (long long)p.main_blocks_per_row * p.batch;
         if (grid > 2147483647LL) return fail(PULSCAN_EINVAL, "too many normalisation blocks for one launch");
         if (p.use_fast && d_redo)
-            rc = launch_norm_fast(p, (int)grid, st, spec, d_power, d_redo, d_redo_count);
+            rc = launch_norm_fast(p, (int)grid, st, spec, out, d_redo, d_redo_count);
         else
             rc = (p.nt_main == 256)
-                     ? launch_norm<256>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP)
-                     : launch_norm<1024>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, d_power, p.pitchP);
+                     ? launch_norm<256>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, out)
+                     : launch_norm<1024>(p.ept_main, (int)grid, st, spec, p.pitch, p.n, p.B, p.nb, 0, p.main_blocks_per_row, out);
         if (rc) return rc;
     }
     if (p.has_tail) {
         rc = (p.nt_tail == 256)
-                 ? launch_norm<256>(p.ept_tail, p.batch, st, spec, p.pitch, p.n, p.B, p.nb, p.nb - 1, 1, d_power, p.pitchP)
-                 : launch_norm<1024>(p.ept_tail, p.batch, st, spec, p.pitch, p.n, p.B, p.nb, p.nb - 1, 1, d_power, p.pitchP);
+                 ? launch_norm<256>(p.ept_tail, p.batch, st, spec, p.pitch, p.n, p.B, p.nb, p.nb - 1, 1, out)
+                 : launch_norm<1024>(p.ept_tail, p.batch, st, spec, p.pitch, p.n, p.B, p.nb, p.nb - 1, 1, out);
     }
     return rc;
 }
 
 // Kernels (b) and (c) on a power (or harmonic-summed) spectrum that is ready in d_P; the plan's bitmap and counters must
 // have been zeroed on the stream.  Exactly one of d_candidates / d_hcandidates is non-null.
-int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candidates, pulscan_hcandidate* d_hcandidates,
-                        uint32_t* d_count, cudaStream_t st, cudaEvent_t* ev) {
+// d_in: what the sweep streams — the per-bin array (P or Y_H, pitchP) or, for a plan that does not keep one, the group sums G
+// (pitchG).  src: where the rare-path kernels read a bin's power (power_source.cuh).
+int enqueue_sweep_exact(pulscan_plan& p, const float* d_in, const PowerSource& src, pulscan_candidate* d_candidates,
+                        pulscan_hcandidate* d_hcandidates, uint32_t* d_count, cudaStream_t st, cudaEvent_t* ev) {
+    const bool from_g = !p.keep_P;
+    const long long pitch_in = from_g ? p.pitchG : p.pitchP;
     int rc = PULSCAN_OK;
     char* ws = static_cast<char*>(p.ws);
     unsigned* d_bitmap = reinterpret_cast<unsigned*>(ws + p.off_bitmap);
@@ -592,16 +621,17 @@ int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candid
     if (p.mode == 0) {
         if (!p.pruned_error.empty()) return fail(PULSCAN_EINVAL, "%s; use mode 1 (exhaustive)", p.pruned_error.c_str());
         SweepCell* d_cells = reinterpret_cast<SweepCell*>(ws + p.off_cells);
-        (p.sweep_fine ? boxcar_sweep_kernel<true> : boxcar_sweep_kernel<false>)<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, grid_b,
-                                                                              p.C, p.nblk, p.d_tau, d_cells, p.cell_cap,
-                                                                              d_bitmap, d_flagged, d_counters);
+        sweep_function(p)<<<p.sweep_grid, kSweepThreads, p.smem_sweep, st>>>(p.sp, d_in, pitch_in, p.n, p.tiles_per_row, grid_b, p.C,
+                                                                             p.nblk, p.d_tau, d_cells, p.cell_cap, d_bitmap, d_flagged,
+                                                                             d_counters);
         CUDA_TRY(cudaGetLastError());
         if ((rc = debug_sync("boxcar_sweep_kernel"))) return rc;
-        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, d_P, p.pitchP, p.n, p.tiles_per_row, p.C,
+        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, src, p.n, p.tiles_per_row, p.C,
                                                                                   p.nblk, p.d_tau, p.d_Tp, d_cells, p.cell_cap,
                                                                                   d_bitmap, d_flagged, d_counters);
     } else {
-        boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_P, p.pitchP,
+        if (from_g) return fail(PULSCAN_EINVAL, "internal: the exhaustive sweep needs the per-bin power array");
+        boxcar_exhaustive_kernel<<<(int)grid_b, kSweepThreads, p.smem_exh, st>>>(p.sp.tile, p.exh_len, p.zmax, d_in, p.pitchP,
                                                                                 p.n, p.tiles_per_row, p.C, p.nblk, p.d_Tp,
                                                                                 d_bitmap, d_flagged, d_counters);
     }
@@ -611,11 +641,33 @@ int enqueue_sweep_exact(pulscan_plan& p, float* d_P, pulscan_candidate* d_candid
 
     const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
     const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
-    block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(d_P, p.pitchP, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
-                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity,
+    block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(src, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
+                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.signif_mode, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity,
                                                                    d_flagged, d_counters, d_candidates, d_count);
     CUDA_TRY(cudaGetLastError());
     return PULSCAN_OK;
+}
+
+// What kernel (a) writes for this plan, what the sweep streams, and where the rare-path kernels read powers.
+NormOut norm_outputs(const pulscan_plan& p) {
+    char* ws = static_cast<char*>(p.ws);
+    if (p.keep_P) return NormOut{reinterpret_cast<float*>(ws + p.off_P), p.pitchP, nullptr, 0, nullptr};
+    return NormOut{nullptr, 0, reinterpret_cast<float*>(ws + p.off_G), p.pitchG, reinterpret_cast<float*>(ws + p.off_stats)};
+}
+const float* sweep_input(const pulscan_plan& p) {
+    char* ws = static_cast<char*>(p.ws);
+    return reinterpret_cast<const float*>(ws + (p.keep_P ? p.off_P : p.off_G));
+}
+PowerSource power_source(const pulscan_plan& p, const void* d_spectra) {
+    char* ws = static_cast<char*>(p.ws);
+    PowerSource s{};
+    s.P = p.keep_P ? reinterpret_cast<const float*>(ws + p.off_P) : nullptr;
+    s.pitchP = p.pitchP;
+    s.spectra = reinterpret_cast<const float2*>(d_spectra);
+    s.pitch = p.pitch;
+    s.stats = p.keep_P ? nullptr : reinterpret_cast<const float*>(ws + p.off_stats);
+    s.B = p.B; s.nb = p.nb;
+    return s;
 }
 
 // The search entry points only look at host state here: no CUDA call, no allocation.
@@ -681,6 +733,7 @@ int pulscan_plan_set_pitch(pulscan_plan* plan, int64_t pitch_bins) {
 int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode) {
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (mode != 0 && mode != 1) return fail(PULSCAN_EINVAL, "mode must be 0 (pruned) or 1 (exhaustive)");
+    if (plan->mode != mode) invalidate(*plan);   // the exhaustive sweep needs the per-bin power array in the workspace
     plan->mode = mode;
     return PULSCAN_OK;
 }
@@ -708,7 +761,16 @@ int pulscan_plan_set_normalisation(pulscan_plan* plan, int32_t mode) {
             return fail(PULSCAN_EINVAL, "median-of-medians normalisation needs norm_block = 256 … 16384, a power of two (it is %d)", B);
         if (plan->n < B) return fail(PULSCAN_EINVAL, "median-of-medians normalisation needs n_bins >= norm_block");
     }
+    if (plan->norm_mode != mode) invalidate(*plan);
     plan->norm_mode = mode;
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_significance(pulscan_plan* plan, int32_t mode) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    if (mode != 0 && mode != 1) return fail(PULSCAN_EINVAL, "mode must be 0 (exact chi-squared tail) or 1 (polynomial ln p, Alg. 3)");
+    plan->signif_mode = mode;
+    invalidate(*plan);       // the per-width power thresholds follow the significance function
     return PULSCAN_OK;
 }
 
@@ -792,9 +854,35 @@ int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_
         char* ws = static_cast<char*>(plan->ws);
         unsigned* d_counters = reinterpret_cast<unsigned*>(ws + plan->off_counters);
         CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
-        return enqueue_norm(*plan, d_spectra, d_power, st, reinterpret_cast<unsigned*>(ws + plan->off_redo), d_counters + 1);
+        return enqueue_norm(*plan, d_spectra, NormOut{d_power, plan->pitchP, nullptr, 0, nullptr}, st,
+                            reinterpret_cast<unsigned*>(ws + plan->off_redo), d_counters + 1);
     }
-    return enqueue_norm(*plan, d_spectra, d_power, st, nullptr, nullptr); // no workspace: general kernels only
+    return enqueue_norm(*plan, d_spectra, NormOut{d_power, plan->pitchP, nullptr, 0, nullptr}, st, nullptr, nullptr); // no workspace: general kernels only
+}
+
+int64_t pulscan_plan_group_pitch(const pulscan_plan* plan) {
+    if (!plan) { fail(PULSCAN_EINVAL, "null plan"); return -1; }
+    return (int64_t)align_up((size_t)((plan->n + 3) / 4), 4);
+}
+
+int pulscan_normalise_group_sums(pulscan_plan* plan, const void* d_spectra, float* d_group_sums, float* d_block_stats,
+                                 void* cuda_stream) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    int rc = derive(*plan);
+    if (rc) return rc;
+    if (!d_spectra || !d_group_sums || !d_block_stats) return fail(PULSCAN_EINVAL, "null pointer");
+    if (reinterpret_cast<uintptr_t>(d_spectra) & 7) return fail(PULSCAN_EINVAL, "d_spectra must be 8-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(d_group_sums) | reinterpret_cast<uintptr_t>(d_block_stats)) & 31)
+        return fail(PULSCAN_EINVAL, "d_group_sums / d_block_stats must be 32-byte aligned");
+    if (plan->B & 3) return fail(PULSCAN_EINVAL, "group sums need norm_block to be a multiple of 4 (it is %d)", plan->B);
+    if (plan->norm_mode == 1) return fail(PULSCAN_EINVAL, "group sums are written by the exact normalisation kernels only");
+    if (!plan->ws || !plan->finalized) return fail(PULSCAN_ENOWORKSPACE, "no workspace attached (pulscan_plan_set_workspace)");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char* ws = static_cast<char*>(plan->ws);
+    unsigned* d_counters = reinterpret_cast<unsigned*>(ws + plan->off_counters);
+    CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
+    return enqueue_norm(*plan, d_spectra, NormOut{nullptr, 0, d_group_sums, plan->pitchG, d_block_stats}, st,
+                        reinterpret_cast<unsigned*>(ws + plan->off_redo), d_counters + 1);
 }
 
 int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate* d_candidates, uint32_t* d_count,
@@ -808,9 +896,7 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     pulscan_plan& p = *plan;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     char* ws = static_cast<char*>(p.ws);
-    float* d_P = reinterpret_cast<float*>(ws + p.off_P);
     unsigned* d_bitmap = reinterpret_cast<unsigned*>(ws + p.off_bitmap);
-    unsigned* d_flagged = reinterpret_cast<unsigned*>(ws + p.off_flagged);
     unsigned* d_counters = reinterpret_cast<unsigned*>(ws + p.off_counters);
 
     cudaEvent_t* ev = nullptr;
@@ -824,11 +910,11 @@ int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate*
     CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
 
     if (ev) CUDA_TRY(cudaEventRecord(ev[1], st));
-    rc = enqueue_norm(p, d_spectra, d_P, st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1); // (a)
+    rc = enqueue_norm(p, d_spectra, norm_outputs(p), st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1); // (a)
     if (rc) return rc;
     if (ev) CUDA_TRY(cudaEventRecord(ev[2], st));
 
-    rc = enqueue_sweep_exact(p, d_P, d_candidates, nullptr, d_count, st, ev);
+    rc = enqueue_sweep_exact(p, sweep_input(p), power_source(p, d_spectra), d_candidates, nullptr, d_count, st, ev);
     if (rc) return rc;
     if (ev) CUDA_TRY(cudaEventRecord(ev[4], st));
     return debug_sync("block_exact_kernel");
@@ -867,9 +953,11 @@ int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_
     CUDA_TRY(cudaMemsetAsync(ws + p.off_bitmap, 0, p.bitmap_bytes, st));
     CUDA_TRY(cudaMemsetAsync(d_counters, 0, 256, st));
     CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
-    rc = enqueue_norm(p, d_spectra, d_P, st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1);      // (a)
+    rc = enqueue_norm(p, d_spectra, norm_outputs(p), st, reinterpret_cast<unsigned*>(ws + p.off_redo), d_counters + 1);   // (a)
     if (rc) return rc;
-    if ((rc = enqueue_sweep_exact(p, d_P, nullptr, d_hcandidates, d_count, st, nullptr))) return rc;           // Y_1 = P
+    if ((rc = enqueue_sweep_exact(p, sweep_input(p), power_source(p, d_spectra), nullptr, d_hcandidates, d_count, st, nullptr)))
+        return rc;                                                                                              // Y_1 = P
+    if (!p.harm.empty() && !p.keep_P) return fail(PULSCAN_EINVAL, "internal: the harmonic sum needs the per-bin power array");
     if (!p.harm.empty()) {                                                                                      // Y_2 … in one pass
         HarmonicOut ho{};
         for (size_t k = 0; k < p.harm.size(); ++k) {
@@ -893,7 +981,7 @@ int pulscan_search_harmonics(pulscan_plan* plan, const void* d_spectra, pulscan_
         char* cws = static_cast<char*>(c.ws);
         CUDA_TRY(cudaMemsetAsync(cws + c.off_bitmap, 0, c.bitmap_bytes, st));
         CUDA_TRY(cudaMemsetAsync(cws + c.off_counters, 0, 256, st));
-        if ((rc = enqueue_sweep_exact(c, reinterpret_cast<float*>(cws + c.off_P), nullptr, d_hcandidates, d_count, st, nullptr))) return rc;
+        if ((rc = enqueue_sweep_exact(c, sweep_input(c), power_source(c, nullptr), nullptr, d_hcandidates, d_count, st, nullptr))) return rc;
     }
     return PULSCAN_OK;
 }
@@ -941,10 +1029,10 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
              "pulscan plan: n_bins=%lld batch=%d zmax=%d block_width=%d norm_block=%d sigma_threshold=%g n_trials=%g pitch=%lld mode=%s\n",
              (long long)p.n, p.batch, p.zmax, p.C, p.B, p.sigma_thr, p.n_trials, (long long)p.pitch, p.mode ? "exhaustive" : "pruned");
     s += line;
-    snprintf(line, sizeof line, "options: widths searched = %s, location = %s, normalisation = %s, numharm = %d\n",
+    snprintf(line, sizeof line, "options: widths searched = %s, location = %s, normalisation = %s, significance = %s, numharm = %d\n",
              p.log_sampling ? "z = 0, 1, 2, 4, ... (L411)" : (p.z_step == 1 ? "every width" : "every z_step-th drift (L152)"),
              p.r_block ? "R-Block (L222-226)" : "exact bin", p.norm_mode ? "median of medians (Alg. 1)" : "exact median/MAD",
-             p.numharm);
+             p.signif_mode ? "polynomial ln p (Alg. 3)" : "exact chi-squared tail", p.numharm);
     s += line;
     snprintf(line, sizeof line, "norm: %d blocks/row, main %s<EPT=%d,NT=%d> x %d/row%s\n", p.nb, p.use_fast ? "single-histogram" : "general",
              p.use_fast ? p.B / p.norm_nt : p.ept_main, p.use_fast ? p.norm_nt : p.nt_main, p.main_blocks_per_row,
@@ -964,6 +1052,9 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
     snprintf(line, sizeof line,
              "sweep: tile=%d len=%d tiles/row=%d smem=%zu B, %.3f cover sums per bin (exhaustive: %d), p_flag=1e%g\n", p.sp.tile,
              p.sp.len, p.tiles_per_row, p.smem_sweep, evals, p.zmax, p.log10_p_flag);
+    s += line;
+    snprintf(line, sizeof line, "intermediate in HBM: %s\n",
+             p.keep_P ? "float32 power of every bin (4 B/bin)" : "sums of 4-bin groups (1 B/bin) + 32 B per normalisation block");
     s += line;
     snprintf(line, sizeof line, "exact: smem=%zu B; workspace=%zu B; T_1=%.4f T_zmax=%.4f\n", p.smem_exact, p.need_bytes, p.T.front(), p.T.back());
     s += line;

@@ -74,6 +74,38 @@ __host__ __device__ inline double sigma_from_lnp(double lnp) {
     return x;
 }
 
+// Algorithm 3 (§2.6 Eq. 10-12): the paper's GPU approximation of ln p, a degree-16 polynomial
+// in x = 1500·dof/pow fitted by regression, in the paper's units (pow = |X'|² summed over the window = 2S, dof = its χ²
+// degrees of freedom = 2·shape; R31).  Horner form in double: the printed coefficients span 1e-46 … 1e2 and x
+// reaches 1428, so neither the coefficients nor the powers of x fit float32.
+__host__ __device__ inline double power_to_logp(double pw, double dof) {
+    if (dof >= pw * 1.05) return 0.0;
+    const double x = 1500.0 * dof / pw;
+    double f = -4.4604059e-46;
+    f = f * x + 9.4927863e-42;
+    f = f * x - 9.1470451e-38;
+    f = f * x + 5.2810851e-34;
+    f = f * x - 2.0376166e-30;
+    f = f * x + 5.5480334e-27;
+    f = f * x - 1.0973877e-23;
+    f = f * x + 1.5991804e-20;
+    f = f * x - 1.7231488e-17;
+    f = f * x + 1.3660070e-14;
+    f = f * x - 7.8617952e-12;
+    f = f * x + 3.2136336e-9;
+    f = f * x - 9.0466418e-7;
+    f = f * x + 0.00016945948;
+    f = f * x - 0.021494231;
+    f = f * x + 2.9515954;
+    f = f * x - 755.24091;
+    return pw * f / 1500.0;
+}
+
+// ln p of a sum S of Gamma shape `shape` (mean-1 units): mode 0 the exact χ² tail, mode 1 Alg. 3.
+__host__ __device__ inline double lnp_of(int signif_mode, int shape, double S) {
+    return signif_mode ? power_to_logp(2.0 * S, 2.0 * (double)shape) : ln_q(shape, S);
+}
+
 // Host only: the power T at which ln Q(w, T) = lnp_target (bisection; ln Q is strictly decreasing in S).
 inline double power_threshold(int w, double lnp_target) {
     double lo = 0.0, hi = (double)w + 16.0;
@@ -83,6 +115,21 @@ inline double power_threshold(int w, double lnp_target) {
         if (ln_q(w, mid) > lnp_target) lo = mid; else hi = mid;
     }
     return 0.5 * (lo + hi);
+}
+
+// Host only: a lower bound of the smallest power S at which Alg. 3 reports ln p ≤ lnp_target for Gamma shape `shape`.  The
+// polynomial is not monotone in S (beyond x ≈ 1100 the printed coefficients do not determine it), so the first crossing is
+// found by a scan from the branch point S = shape/1.05 upwards and the last grid point before it is returned.
+inline double power_threshold_poly(int shape, double lnp_target) {
+    const double s0 = (double)shape / 1.05;
+    const double hi = 4.0 * power_threshold(shape, lnp_target) + 64.0;
+    const double step = 0.01 + 0.01 * std::sqrt((double)shape);
+    double prev = s0 * (1.0 - 1e-12);
+    for (double S = s0; S <= hi; S += step) {
+        if (power_to_logp(2.0 * S, 2.0 * (double)shape) <= lnp_target) return prev;
+        prev = S;
+    }
+    return hi;
 }
 
 } // namespace pulscan

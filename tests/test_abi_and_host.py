@@ -105,8 +105,10 @@ def test_sizes(binding):
     p = binding.Plan(4194305, 256, 200, 200, 6.0, norm_block=4096)
     assert p.max_candidates == 256 * 20972
     assert p.power_pitch == 4194308
-    ws = p.workspace_bytes
-    assert 256 * 4194308 * 4 <= ws <= 256 * 4194308 * 4 + 64e6
+    ws = p.workspace_bytes                     # group sums (1 float per 4 bins) + 32 bytes per normalisation block + lists
+    assert 256 * 1048580 * 4 <= ws <= 256 * 1048580 * 4 + 80e6
+    pe = binding.Plan(4194305, 256, 200, 200, 6.0, norm_block=4096, mode=1)    # exhaustive mode keeps the per-bin powers
+    assert 256 * 4194308 * 4 <= pe.workspace_bytes <= 256 * 4194308 * 4 + 64e6
     ph = binding.Plan(4194305, 256, 200, 200, 6.0, norm_block=4096, host_staging=True)
     assert ph.workspace_bytes >= ws + 256 * 4194305 * 8
     assert p.launches_per_search == 6      # (a) single-histogram + (a) redo + (a) last blocks + (b) sweep + (b) refine + (c)

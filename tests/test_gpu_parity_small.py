@@ -400,7 +400,10 @@ def test_setter_after_attach_needs_a_new_attach():
     assert e.value.code == binding.PULSCAN_ENOWORKSPACE
     plan.attach("cuda")
     plan.search(spec)
-    plan.set_mode(1)                                         # no derived state depends on the mode: no new attach needed
+    assert plan.lib.pulscan_plan_set_mode(plan.handle, 1) == 0   # the exhaustive sweep keeps the per-bin powers: new layout
+    with pytest.raises(binding.PulscanError):
+        plan.search(spec)
+    plan.set_mode(1)                                         # the binding attaches again
     plan.search(spec)
     torch.cuda.synchronize()
     plan.destroy()
@@ -425,3 +428,62 @@ def test_host_staging_with_per_width_emission(orc):
         keys = set(zip(ora["bin"].tolist(), ora["width"].tolist()))
         assert all(k in keys for k in zip(got["bin"].tolist(), got["width"].tolist())) and np.all(got["width"] >= 1)
         plan.destroy()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,batch,zmax,B,C,thr,numharm,log_sampling,mom", [
+    (20001, 2, 40, 2048, 100, 4.0, 1, False, False), (9001, 2, 64, 4096, 200, 5.0, 3, False, False),
+    (30011, 1, 129, 8192, 300, 6.0, 4, True, True),      # the paper's GPU-native configuration: Alg. 1 + Alg. 3 + log z + 4 harmonics
+    (12001, 1, 300, 4096, 400, 6.0, 1, False, False)])   # wide widths: x = 1500·dof/pow > 1100, where Alg. 3 diverges and floods
+def test_polynomial_logp_matches_oracle(orc, n, batch, zmax, B, C, thr, numharm, log_sampling, mom, mode):
+    """Fast mode (Alg. 3): every ln p from the printed polynomial, on the device and in the oracle; the
+    candidate lists (bins, widths exact; sigma = Φ_sf⁻¹(e^{ln p}) within 1e-3, i.e. ln p element by element) must agree."""
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(batch, n, seed=n + 17 * numharm)
+    bump(spec, 0, n // 3, 6, 3.0)
+    bump(spec, batch - 1, n // 2, min(zmax, 30), 1.8)
+    plan = binding.Plan(n, batch, zmax, C, thr, norm_block=B, mode=mode, numharm=numharm, log_sampling=log_sampling,
+                        median_of_medians=mom, poly_logp=True)
+    plan.attach("cuda")
+    plan.search_harmonics(spec)
+    gpu = plan.hcandidates()
+    plan.destroy()
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, numharm, log_sampling=log_sampling, median_of_medians=mom,
+                               poly_logp=True)
+    assert len(ora) > 0
+    _assert_same_hcandidates(gpu, ora, f"Alg. 3 n={n} zmax={zmax} numharm={numharm} mode={mode}")
+    exact = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, numharm, log_sampling=log_sampling, median_of_medians=mom)
+    if zmax <= 64:
+        assert len(ora) <= len(exact)        # usable region: Alg. 3 under-states significance, marginal candidates drop out
+    if zmax == 300:
+        assert len(ora) > 2 * len(exact)     # divergent region: wide widths pass on pure noise
+
+
+@pytest.mark.parametrize("n,B", [(4097, 1024), (12289, 4096), (8192, 4096), (16385, 8192), (2051, 512), (40000, 16384), (5003, 100),
+                                 (1 << 16, 2048)])
+def test_group_sums_and_block_statistics_rebuild_the_powers(orc, n, B):
+    """What the default search keeps in HBM instead of the per-bin powers: G[k] = (P[4k]+P[4k+1]) + (P[4k+2]+P[4k+3]) in
+    float32, bit for bit, and per-block (a, inv, k) from which every P is rebuilt bit for bit with the same FMAs."""
+    from paper_2406_15186_b200 import binding
+    spec = noise_spectra(3, n, seed=n + B)
+    spec[1] = spec[1] * 1e-3 + (5.0 - 2.0j)
+    plan = binding.Plan(n, 3, min(8, n - 1), 16, 6.0, norm_block=B)
+    plan.attach("cuda")
+    P = plan.normalise_power(spec)
+    G, st = plan.normalise_group_sums(spec, B)
+    plan.destroy()
+    Pp = torch.zeros((3, 4 * ((n + 3) // 4)), dtype=torch.float32, device="cuda")
+    Pp[:, :n] = P
+    q = Pp.view(3, -1, 4)
+    want = (q[:, :, 0] + q[:, :, 1]) + (q[:, :, 2] + q[:, :, 3])
+    assert torch.equal(G, want)
+    nb = max(1, n // B)
+    blk = torch.clamp(torch.arange(n, device="cuda") // B, max=nb - 1)
+    a0, i0, k0, a1, i1, k1 = (st[:, :, c][:, blk].double() for c in range(6))
+    x = (spec.real.float() - a0.float()).double() * i0 + k0         # fma = one rounding of the exact product-sum: emulate in double
+    y = (spec.imag.float() - a1.float()).double() * i1 + k1
+    x, y = x.float().double(), y.float().double()
+    rebuilt = (x * x + (y * y).float().double()).float()
+    assert torch.equal(rebuilt, P)
+    ref = orc.normalise_power(spec[0].cpu().numpy(), B)              # and the statistics are the paper's: median and κ·MAD
+    assert np.all(np.abs(P[0].cpu().numpy() - ref) <= 1e-5 * ref + 1e-6)
