@@ -22,10 +22,14 @@
 
 namespace pulscan {
 
-constexpr int kExactThreads = 512;
+constexpr int kExactThreads = 1024;
 
 struct ExactSmemHdr {
     double part[kExactThreads];   // per-thread chunk sums for the prefix scan
+    double list_s[kExactThreads]; // widths of the current round whose maximum reaches T_w: (maximum, width, arg-max)
+    int list_w[kExactThreads];
+    int list_i[kExactThreads];
+    unsigned nlist[2];
     double best_lnp[kExactThreads / 32];
     int best_w[kExactThreads / 32];
     int best_i[kExactThreads / 32];
@@ -52,19 +56,44 @@ __device__ __forceinline__ void emit_candidate(long long row, int32_t bin, int w
     }
 }
 
+// Partial result of one part of a block (see `parts` below): the best width among the rounds that part evaluated.
+struct alignas(8) ExactPartial {
+    double lnp, s;
+    int w, i;
+};
+
+// lg_split: the start bins of a block are cut into 2^lg_split chunks handled by adjacent lanes, so that zmax·2^lg_split
+// (width, chunk) pairs keep all 1024 threads busy when zmax is small and balance the rounds when it is large (host choice).
+// parts > 1 (large zmax): the rounds of widths of one block are dealt to `parts` CTAs (each rebuilds the block's prefix sum),
+// their partial arg-minima meet in `partial` and the CTA that arrives last (`done` counter) reduces and emits — a few
+// hundred marked blocks then occupy the whole GPU instead of one CTA each.  Only the first `split_slots` marked blocks are
+// split (the size of `partial` / `done`); the rest is evaluated by one CTA per block.
 __global__ void __launch_bounds__(kExactThreads)
 block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long long nblk,
                    const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int signif_mode, int numharm,
-                   pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity,
+                   pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity, int lg_split, int parts,
+                   unsigned split_slots, ExactPartial* __restrict__ partial, unsigned* __restrict__ done,
                    const unsigned* __restrict__ flagged, const unsigned* __restrict__ counters,
                    pulscan_candidate* __restrict__ out, unsigned* __restrict__ out_count) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     ExactSmemHdr& hdr = *reinterpret_cast<ExactSmemHdr*>(smem_raw);
     double* pre = reinterpret_cast<double*>(smem_raw + sizeof(ExactSmemHdr)); // [L + 1]
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
     const unsigned nflag = counters[0];
+    if (tid == 0) { hdr.nlist[0] = 0; hdr.nlist[1] = 0; }
+    __syncthreads();
+    const int nsplit = 1 << lg_split, piece = tid & (nsplit - 1), w_per_round = kExactThreads >> lg_split;
+    // start bins per chunk; for 4 or more chunks rounded up to ≡ 32/nsplit (mod 16) doubles, so that the nsplit segments a
+    // warp reads with one LDS.64 (32/nsplit consecutive widths each) fall on disjoint banks: 2 wavefronts instead of 4
+    int cs = (C + nsplit - 1) >> lg_split;
+    if (nsplit >= 4) cs += (((32 >> lg_split) - cs) & 15);
 
-    for (unsigned e = blockIdx.x; e < nflag; e += gridDim.x) {
+    const unsigned n_split = parts > 1 ? min(nflag, split_slots) : 0u;
+    const unsigned n_items = n_split * (unsigned)parts + (nflag - n_split);
+    for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const bool split = item < n_split * (unsigned)parts;
+        const unsigned e = split ? item / (unsigned)parts : n_split + (item - n_split * (unsigned)parts);
+        const int part = split ? (int)(item % (unsigned)parts) : 0, nparts = split ? parts : 1;
         const unsigned gid = flagged[e];
         const long long row = gid / nblk;
         const long long c = gid % nblk;
@@ -75,60 +104,86 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
         long long end = hi + zmax - 1;              // last bin any window of the block can touch, exclusive: hi−1+zmax
         if (end > n) end = n;
         const int L = (int)(end - lo);
-        PowerSource::Row src(src_pw, row);
 
-        // double-precision exclusive prefix sum: pre[j] = Σ_{t<j} P[lo+t]
-        const int chunk = (L + kExactThreads - 1) / kExactThreads;
-        const int a = tid * chunk;
-        const int b = min(a + chunk, L);
-        double s = 0.0;
-        for (int j = a; j < b; ++j) s += (double)src(lo + j);
-        hdr.part[tid] = s;
+        // double-precision prefix sum pre[j] = Σ_{t<j} P[lo+t]: coalesced loads (or rebuilds, power_source.cuh) into
+        // pre[j+1], each thread then scans its own chunk in place and the chunk totals are scanned by one warp
+        {
+            PowerSource::Row src(src_pw, row);
+            for (int j = tid; j < L; j += kExactThreads) pre[j + 1] = (double)src(lo + j);
+            if (tid == 0) pre[0] = 0.0;
+        }
         __syncthreads();
-        if (tid < 32) { // scan of the 512 chunk sums by one warp, 16 each
+        const int chunk = (L + kExactThreads - 1) / kExactThreads;
+        const int a = min(tid * chunk, L), b = min(a + chunk, L);
+        {
             double run = 0.0;
-            double loc[kExactThreads / 32];
-#pragma unroll
-            for (int q = 0; q < kExactThreads / 32; ++q) { loc[q] = run; run += hdr.part[tid * (kExactThreads / 32) + q]; }
+            for (int j = a; j < b; ++j) { run += pre[j + 1]; pre[j + 1] = run; }
+            hdr.part[tid] = run;
+        }
+        __syncthreads();
+        if (tid < 32) { // exclusive scan of the 1024 chunk sums by one warp, 32 each
+            double run = 0.0;
+            for (int q = 0; q < kExactThreads / 32; ++q) { const double v = hdr.part[tid * (kExactThreads / 32) + q]; hdr.part[tid * (kExactThreads / 32) + q] = run; run += v; }
             double inc = run;
 #pragma unroll
             for (int off = 1; off < 32; off <<= 1) {
-                double t = __shfl_up_sync(0xffffffffu, inc, off);
+                const double t = __shfl_up_sync(0xffffffffu, inc, off);
                 if (tid >= off) inc += t;
             }
             const double base = inc - run;
-#pragma unroll
-            for (int q = 0; q < kExactThreads / 32; ++q) hdr.part[tid * (kExactThreads / 32) + q] = base + loc[q];
+            for (int q = 0; q < kExactThreads / 32; ++q) hdr.part[tid * (kExactThreads / 32) + q] += base;
         }
         __syncthreads();
         {
-            double run = hdr.part[tid];
-            for (int j = a; j < b; ++j) { pre[j] = run; run += (double)src(lo + j); }
-            if (b == L && a < L) pre[L] = run;
-            if (L == 0 && tid == 0) pre[0] = 0.0;
+            const double base = hdr.part[tid];
+            for (int j = a; j < b; ++j) pre[j + 1] += base;
         }
         __syncthreads();
 
-        // one width per thread: maximum over the block's start bins, then ln p where it can matter
+        // (width, chunk of start bins) per thread: maximum and lowest arg-max over the chunk, combined over the chunks of a
+        // width by shuffles (adjacent lanes, increasing start bins: ties keep the lower bin, R14); then ln p where it can matter
         double my_lnp = INFINITY, my_s = 0.0;
         int my_w = 0, my_i = 0;
-        for (int w = tid + 1; w <= zmax; w += kExactThreads) {
-            const int imax = min(nstart, L - w + 1);   // starts i with i + w ≤ L
+        for (int w0 = part * w_per_round; w0 < zmax; w0 += nparts * w_per_round) {
+            const int w = w0 + (tid >> lg_split) + 1;
             double best = -1.0;
             int arg = -1;
-            for (int i = 0; i < imax; ++i) {
-                const double v = pre[i + w] - pre[i];
-                if (v > best) { best = v; arg = i; }
+            if (w <= zmax) {
+                const int imax = min(nstart, L - w + 1);   // starts i with i + w ≤ L
+                const int i1 = min((piece + 1) * cs, imax);
+                for (int i = piece * cs; i < i1; ++i) {
+                    const double v = pre[i + w] - pre[i];
+                    if (v > best) { best = v; arg = i; }
+                }
             }
-            if (arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
+            for (int off = 1; off < nsplit; off <<= 1) {       // lanes piece, piece^off: the lower piece holds the lower bins
+                const double ob = __shfl_xor_sync(0xffffffffu, best, off);
+                const int oa = __shfl_xor_sync(0xffffffffu, arg, off);
+                const bool other_lower = (piece & off) != 0;
+                if (ob > best || (ob == best && other_lower && oa >= 0)) { best = ob; arg = oa; }
+            }
+            // The widths whose maximum reaches T_w are collected and their ln p evaluated by all threads: the series of ln Q is
+            // a serial loop of up to w terms, and only one lane in 2^lg_split holds a width after the reduction above.
+            const int rnd = (w0 / w_per_round) & 1;
+            if (piece == 0 && w <= zmax && arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
+                const unsigned slot = atomicAdd(&hdr.nlist[rnd], 1u);
+                hdr.list_s[slot] = best; hdr.list_w[slot] = w; hdr.list_i[slot] = arg;
+            }
+            __syncthreads();
+            const int nl = (int)hdr.nlist[rnd];
+            if (tid == 0) hdr.nlist[rnd ^ 1] = 0;
+            for (int idx = tid; idx < nl; idx += kExactThreads) {
+                const int lw = hdr.list_w[idx], li = hdr.list_i[idx];
+                const double ls = hdr.list_s[idx];
                 // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220); signif_mode 1: Alg. 3's polynomial instead of the tail
-                double lnp = lnp_of(signif_mode, w * shape_mult, best) + ln_trials;
+                double lnp = lnp_of(signif_mode, lw * shape_mult, ls) + ln_trials;
                 if (lnp > 0.0) lnp = 0.0;
                 if (per_width) {   // the paper's GPU output: one candidate per (block, searched width) above the threshold (Alg. 4)
                     if (lnp <= lnp_thr)
-                        emit_candidate(row, r_block ? (int32_t)lo : (int32_t)(lo + arg), w, best, lnp, numharm, out, out_h, out_count, capacity);
-                } else if (lnp < my_lnp) { my_lnp = lnp; my_w = w; my_i = arg; my_s = best; } // ascending w: ties keep the smaller
+                        emit_candidate(row, r_block ? (int32_t)lo : (int32_t)(lo + li), lw, ls, lnp, numharm, out, out_h, out_count, capacity);
+                } else if (lnp < my_lnp || (lnp == my_lnp && lw < my_w)) { my_lnp = lnp; my_w = lw; my_i = li; my_s = ls; }   // ties keep the smaller width
             }
+            __syncthreads();
         }
         // block arg-min over (ln p, w)
 #pragma unroll
@@ -139,7 +194,7 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
             const double os = __shfl_xor_sync(0xffffffffu, my_s, off);
             if (ol < my_lnp || (ol == my_lnp && ow != 0 && (my_w == 0 || ow < my_w))) { my_lnp = ol; my_w = ow; my_i = oi; my_s = os; }
         }
-        if ((tid & 31) == 0) {
+        if (lane == 0) {
             hdr.best_lnp[tid >> 5] = my_lnp; hdr.best_w[tid >> 5] = my_w; hdr.best_i[tid >> 5] = my_i; hdr.best_s[tid >> 5] = my_s;
         }
         __syncthreads();
@@ -149,6 +204,23 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
                 const int ow = hdr.best_w[q];
                 if (ol < my_lnp || (ol == my_lnp && ow != 0 && (my_w == 0 || ow < my_w))) {
                     my_lnp = ol; my_w = ow; my_i = hdr.best_i[q]; my_s = hdr.best_s[q];
+                }
+            }
+            if (nparts > 1 && !per_width) {      // meet the other parts of this block; the last one to arrive finishes the job
+                ExactPartial* slot = partial + (size_t)e * parts;
+                slot[part] = ExactPartial{my_lnp, my_s, my_w, my_i};
+                __threadfence();
+                if (atomicAdd(done + e, 1u) != (unsigned)(parts - 1)) my_w = 0;
+                else {
+                    __threadfence();
+                    for (int q = 0; q < parts; ++q) {
+                        if (q == part) continue;
+                        const double ol = __ldcg(&slot[q].lnp);
+                        const int ow = __ldcg(&slot[q].w);
+                        if (ol < my_lnp || (ol == my_lnp && ow != 0 && (my_w == 0 || ow < my_w))) {
+                            my_lnp = ol; my_w = ow; my_i = __ldcg(&slot[q].i); my_s = __ldcg(&slot[q].s);
+                        }
+                    }
                 }
             }
             if (my_w > 0 && my_lnp <= lnp_thr)   // R-Block: block index × block width (L222-226)

@@ -78,10 +78,12 @@ struct SweepParams {
     int narr;        // decimated arrays: one per distinct group size
     int arr_lg[kMaxLevels];
     int arr_off[kMaxLevels];
+    int off_lg[8];   // offset of the array with group size 2^lg, lg = 0..7; −1 if no level uses it
     int npass;       // scan passes per tile = ceil(len / kScanPass)
     int z_floats;    // floats of ONE landing buffer: len + kScanPer zeros (len/4 + kScanPer/4 for group-sum input), rounded up to 4
     int smem_floats; // two landing buffers + decimated arrays
     int ref_span;    // longest span of bins a listed cell covers (sweep_refine_kernel's shared memory per warp)
+    int tp_monotone; // T'_w is finite and non-decreasing in w (every width searched, exact significance)
     SweepLevel lv[kMaxLevels];
 };
 
@@ -141,7 +143,7 @@ __device__ __forceinline__ void load_tile(float* sP, const float* __restrict__ P
 // TMA copy into this buffer).  Returns PP[len] in every thread.  Ends with a CTA barrier; the barrier inside a pass
 // also orders the previous tile's cover sums before this tile's writes to the arrays.
 struct ScanSmem {
-    alignas(16) float wtot[kSweepThreads / 32];
+    alignas(16) float wtot[kSweepThreads / 32 + 4];   // warp totals; [8] = the running total carried into the next pass
 };
 
 __device__ __forceinline__ float scan_sel5(const float (&s)[5], int q) {
@@ -151,6 +153,26 @@ __device__ __forceinline__ float scan_sel5(const float (&s)[5], int q) {
     v = (q == 1) ? s[1] : v;
     v = (q == 0) ? s[0] : v;
     return v;
+}
+
+// The entries of the decimated array PG_LG (PG[k] = PP[k << LG]) among a thread's five prefix values s[q] = PP[4(u + q)].
+template <int LG>
+__device__ __forceinline__ void scan_put(float* __restrict__ dst, int u, const float (&s)[5]) {
+    if (LG == 2) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) dst[u + q] = s[q];
+    } else if (LG == 3) {
+        const bool odd = u & 1;                                 // hits q = odd, odd+2 (and 4 when even)
+        float* d = dst + ((u + 1) >> 1);
+        d[0] = odd ? s[1] : s[0];
+        d[1] = odd ? s[3] : s[2];
+        if (!odd) d[2] = s[4];
+    } else {
+        constexpr int sh = LG - 2;
+        const int q0 = (-u) & ((1 << sh) - 1);
+        if (q0 < 5) dst[(u + q0) >> sh] = scan_sel5(s, q0);
+        if (LG == 4 && q0 == 0) dst[(u + 4) >> 2] = s[4];
+    }
 }
 
 // FINE = true additionally keeps the prefix inside each quad (x[3q+t] = the quad's first t+1 powers) and writes the arrays
@@ -200,22 +222,15 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
             const float t = __shfl_up_sync(0xffffffffu, incl, off);
             if (lane >= off) incl += t;
         }
-        float excl = __shfl_up_sync(0xffffffffu, incl, 1);
-        if (lane == 0) excl = 0.f;
+        const float excl = incl - s[4];
         if (lane == 31) ss.wtot[warp] = incl;
         __syncthreads();
         if (pass == sp.npass - 1) after_loads();
-        // exclusive prefix of the 8 warp totals: lane w < 8 holds total w, three shuffle steps, broadcast
-        float wt = (lane < kSweepThreads / 32) ? ss.wtot[lane] : 0.f;
-        const float mine = (lane < warp) ? wt : 0.f;
-        float wbase = mine, total = wt;
+        // sum of the totals of the warps below this one: lane w < 8 holds total w, masked, three butterfly steps
+        float wbase = (lane < warp) ? ss.wtot[lane & (kSweepThreads / 32 - 1)] : 0.f;
 #pragma unroll
-        for (int off = 4; off > 0; off >>= 1) {
-            wbase += __shfl_xor_sync(0xffffffffu, wbase, off);
-            total += __shfl_xor_sync(0xffffffffu, total, off);
-        }
+        for (int off = 4; off > 0; off >>= 1) wbase += __shfl_xor_sync(0xffffffffu, wbase, off);
         wbase = __shfl_sync(0xffffffffu, wbase, 0);
-        total = __shfl_sync(0xffffffffu, total, 0);
         if (act) {
             const float off = carry + (wbase + excl);
 #pragma unroll
@@ -227,37 +242,33 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
                     const float oq = q ? s[q - 1] : off;
                     x[3 * q] += oq; x[3 * q + 1] += oq; x[3 * q + 2] += oq;
                 }
-            }
-            for (int a = 0; a < sp.narr; ++a) {
-                const int lg = sp.arr_lg[a];
-                float* dst = sG + sp.arr_off[a];
-                if (FINE && lg == 0) {                          // PG0[i] = PP[i]: entries i0+1 … i0+20 (the pad holds 16)
+                if (sp.off_lg[0] >= 0) {                        // PG0[i] = PP[i]: entries i0+1 … i0+20 (the pad holds 16)
+                    float* dst = sG + sp.off_lg[0];
 #pragma unroll
                     for (int q = 0; q < 5; ++q) {
                         float* d = dst + i0 + 4 * q + 1;
                         if (i0 + 4 * q + 4 <= len + kPadG) { d[0] = x[3 * q]; d[1] = x[3 * q + 1]; d[2] = x[3 * q + 2]; d[3] = s[q]; }
                     }
-                } else if (FINE && lg == 1) {                   // PG1[k] = PP[2k]: entries i0/2+1 … i0/2+10
+                }
+                if (sp.off_lg[1] >= 0) {                        // PG1[k] = PP[2k]: entries i0/2+1 … i0/2+10
+                    float* dst = sG + sp.off_lg[1];
 #pragma unroll
                     for (int q = 0; q < 5; ++q) { dst[(i0 >> 1) + 2 * q + 1] = x[3 * q + 1]; dst[(i0 >> 1) + 2 * q + 2] = s[q]; }
-                } else if (lg == 2) {
-#pragma unroll
-                    for (int q = 0; q < 5; ++q) dst[u + q] = s[q];
-                } else if (lg == 3) {
-                    const bool odd = u & 1;                     // hits q = odd, odd+2 (and 4 when even)
-                    float* d = dst + ((u + 1) >> 1);
-                    d[0] = odd ? s[1] : s[0];
-                    d[1] = odd ? s[3] : s[2];
-                    if (!odd) d[2] = s[4];
-                } else {
-                    const int sh = lg - 2, q0 = (-u) & ((1 << sh) - 1);
-                    if (q0 < 5) dst[(u + q0) >> sh] = scan_sel5(s, q0);
-                    if (lg == 4 && q0 == 0) dst[(u + 4) >> 2] = s[4];
                 }
             }
+            // one store sequence per group size, the group size a compile-time constant in each (the branches are uniform)
+            if (sp.off_lg[2] >= 0) scan_put<2>(sG + sp.off_lg[2], u, s);
+            if (sp.off_lg[3] >= 0) scan_put<3>(sG + sp.off_lg[3], u, s);
+            if (sp.off_lg[4] >= 0) scan_put<4>(sG + sp.off_lg[4], u, s);
+            if (sp.off_lg[5] >= 0) scan_put<5>(sG + sp.off_lg[5], u, s);
+            if (sp.off_lg[6] >= 0) scan_put<6>(sG + sp.off_lg[6], u, s);
+            if (sp.off_lg[7] >= 0) scan_put<7>(sG + sp.off_lg[7], u, s);
         }
-        carry += total;
+        // PP at the end of this pass = the last thread's running total: the carry of the next pass and, after the last pass,
+        // PP[len] (the bound of every entry, which the caller's slack is scaled by)
+        if (tid == kSweepThreads - 1) ss.wtot[kSweepThreads / 32] = act ? s[4] : carry + (wbase + excl);
         __syncthreads();
+        carry = ss.wtot[kSweepThreads / 32];
     }
     return carry;
 }
@@ -567,6 +578,30 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const PowerSource sr
                 const unsigned long long gb = (unsigned long long)(row * nblk + min(base + i0 + g - 1, n - 1) / C);
                 const unsigned wa = __ldcg(bitmap + (ga >> 5)), wb = __ldcg(bitmap + (gb >> 5));
                 if ((wa >> (ga & 31) & 1u) && (wb >> (gb & 31) & 1u)) continue;
+            }
+            if (lg >= 4 && sp.tp_monotone) {
+                // Wide groups: cut the cover's g × g (start, end) pairs into 4 × 4 sub-covers of h = g/4 starts and ends.  The
+                // sum from a sub-cover's first start to its last end bounds all its windows, and (T'_w non-decreasing in w)
+                // the threshold of its narrowest searched width bounds theirs from below: only sub-covers that pass that test
+                // (a few in noise) have their h² windows summed.
+                const int lh = lg - 2, h = 1 << lh, sa = lane & 3, sb = (lane >> 2) & 3;
+                const int fs = i0 + (sa << lh), le = min(e0 + ((sb + 1) << lh) - 1, valid - 1);   // first start, last (valid) end
+                const int w_lo = max((e0 + (sb << lh)) - (fs + h - 1) + 1, max(lv.wlo, 1)), w_hi = min(le - fs + 1, lv.whi);
+                const bool sub_live = lane < 16 && w_lo <= w_hi && pp[le + 1] - pp[fs] >= (double)__ldg(Tp_g + (w_lo - 1));
+                unsigned subs = __ballot_sync(0xffffffffu, sub_live);
+                while (subs) {
+                    const int sl = __ffs(subs) - 1;
+                    subs &= subs - 1;
+                    const int is = i0 + ((sl & 3) << lh), es = e0 + (((sl >> 2) & 3) << lh);
+                    for (int idx = lane; idx < h * h; idx += 32) {
+                        const int i = is + (idx >> lh), ee = es + (idx & (h - 1));
+                        const int w = ee - i + 1;
+                        if (w < 1 || w < lv.wlo || w > lv.whi || ee >= valid) continue;
+                        if (pp[ee + 1] - pp[i] >= (double)__ldg(Tp_g + (w - 1)))
+                            mark_block((unsigned long long)(row * nblk + (base + i) / C), bitmap, flagged, counters);
+                    }
+                }
+                continue;
             }
             for (int idx = lane; idx < g * g; idx += 32) {
                 const int i = i0 + (idx >> lg), ee = e0 + (idx & (g - 1));

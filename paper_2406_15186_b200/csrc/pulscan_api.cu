@@ -103,6 +103,10 @@ struct pulscan_plan {
     unsigned cell_cap_user = 0;
     unsigned cell_cap = 0;     // capacity of the flagged-cell list between the sweep and its refine kernel
     int exh_len = 0;
+    int exact_lg_split = 0;    // kernel (c): 2^lg lanes share the start bins of a width
+    int exact_parts = 1;       // kernel (c): CTAs that share the widths of one marked block
+    unsigned exact_slots = 0;  // marked blocks that can be split (size of the partial-result scratch)
+    size_t off_partial = 0, off_done = 0;
     // normalisation launch shapes
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
     bool has_tail = false;
@@ -179,7 +183,10 @@ int derive(pulscan_plan& p) {
     }
 
     // ---- sweep tile
-    int tile = p.tile_user ? p.tile_user : (p.zmax <= 512 ? 4096 : 8192);
+    // the group-sum input needs a quarter of the landing space: 8192-bin tiles halve the barriers per bin and balance the
+    // warp-tasks better (measured at cfg 3: sweep 1.55 -> 1.43 ms; cfg 5: 2.42 -> 2.22 ms)
+    const bool likely_from_g = !p.is_child && p.mode == 0 && p.numharm == 1 && p.norm_mode == 0 && (p.B & 3) == 0;
+    int tile = p.tile_user ? p.tile_user : ((p.zmax <= 512 && !likely_from_g) ? 4096 : 8192);
     // ---- group size per width: the largest g = 2^lg whose worst cover (w + 2g − 2 bins) of pure noise passes the
     //      width's threshold with probability ≤ p_flag; made non-decreasing in w by a suffix minimum.
     //      Levels with g < 4 (narrow widths of harmonic-summed spectra, very low σ thresholds) make the sweep use its
@@ -303,6 +310,8 @@ int derive(pulscan_plan& p) {
         sp.lv[l] = lv;
     }
     sp.ntasks = task;
+    for (int lg = 0; lg < 8; ++lg) sp.off_lg[lg] = -1;
+    for (int a = 0; a < sp.narr; ++a) sp.off_lg[sp.arr_lg[a]] = sp.arr_off[a];
     p.sweep_fine = false;
     for (int a = 0; a < sp.narr; ++a) p.sweep_fine = p.sweep_fine || sp.arr_lg[a] < 2;
     // Does the float32 power of every bin have to exist in HBM?  Not on the default path: kernel (a) then leaves only the sums
@@ -320,6 +329,9 @@ int derive(pulscan_plan& p) {
     p.tiles_per_row = (int)((p.n + tile - 1) / tile);
     const size_t flag_bytes = align_up((size_t)(tile / p.C + 3), 16);
     sp.zmax = p.zmax;
+    sp.tp_monotone = 1;
+    for (int w = 1; w <= p.zmax; ++w)
+        if (!std::isfinite(p.Tp[w - 1]) || (w > 1 && p.Tp[w - 1] < p.Tp[w - 2])) sp.tp_monotone = 0;
     sp.ref_span = 0;
     for (int l = 0; l < sp.nlevels; ++l)
         sp.ref_span = std::max(sp.ref_span, (sp.lv[l].m_start + 4 * sp.lv[l].nsteps + 6) << sp.lv[l].lg);
@@ -330,6 +342,17 @@ int derive(pulscan_plan& p) {
     p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
     p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
+    {   // kernel (c): split the start bins of a block over 2^lg adjacent lanes so that rounds × starts per chunk is smallest
+        long long best = -1;
+        for (int lg = 0; lg <= 5; ++lg) {
+            const long long rounds = ((long long)p.zmax * (1 << lg) + kExactThreads - 1) / kExactThreads;
+            const long long cost = rounds * (((p.C + (1 << lg) - 1) >> lg) + (lg >= 2 ? 8 : 0)) + 2 * lg;
+            if (best < 0 || cost < best) { best = cost; p.exact_lg_split = lg; }
+        }
+        const int rounds = (int)(((long long)p.zmax * (1 << p.exact_lg_split) + kExactThreads - 1) / kExactThreads);
+        p.exact_parts = std::min(rounds, 8);
+        p.exact_slots = p.exact_parts > 1 ? (unsigned)std::min<long long>((long long)p.batch * p.nblk, 16384) : 0u;
+    }
 
     // ---- normalisation launch shapes (a child plan searches a spectrum that its parent has normalised and summed)
     if (p.is_child) { p.main_blocks_per_row = 0; p.has_tail = false; p.use_fast = false; }
@@ -371,6 +394,8 @@ int derive(pulscan_plan& p) {
     p.cell_cap = (unsigned)std::min<unsigned long long>(1ull << 28, std::max<unsigned long long>(65536, (unsigned long long)p.batch * p.n / 256));
     if (p.cell_cap_user) p.cell_cap = p.cell_cap_user;
     p.off_cells = o; o += align_up((size_t)p.cell_cap * sizeof(SweepCell), 256);
+    p.off_partial = o; o += align_up((size_t)p.exact_slots * p.exact_parts * sizeof(ExactPartial), 256);
+    p.off_done = o; o += align_up((size_t)p.exact_slots * sizeof(unsigned), 256);
     p.off_tables = o;
     o += align_up(p.T.size() * sizeof(double), 256) + align_up(p.Tp.size() * sizeof(float), 256) +
          align_up(std::max<size_t>(1, p.tau.size()) * sizeof(float), 256);
@@ -640,9 +665,12 @@ int enqueue_sweep_exact(pulscan_plan& p, const float* d_in, const PowerSource& s
     if (ev) CUDA_TRY(cudaEventRecord(ev[3], st));
 
     const long long total_blocks = (long long)p.batch * p.nblk;                    // (c)
-    const int grid_c = (int)std::min<long long>(total_blocks, (long long)p.sm_count * 4);
+    const int grid_c = (int)std::min<long long>(total_blocks * p.exact_parts, (long long)p.sm_count * 4);
+    if (p.exact_slots) CUDA_TRY(cudaMemsetAsync(ws + p.off_done, 0, (size_t)p.exact_slots * sizeof(unsigned), st));
     block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(src, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
-                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.signif_mode, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity,
+                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.signif_mode, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity, p.exact_lg_split, p.exact_parts,
+                                                                   p.exact_slots, reinterpret_cast<ExactPartial*>(ws + p.off_partial),
+                                                                   reinterpret_cast<unsigned*>(ws + p.off_done),
                                                                    d_flagged, d_counters, d_candidates, d_count);
     CUDA_TRY(cudaGetLastError());
     return PULSCAN_OK;

@@ -18,11 +18,18 @@ __host__ __device__ inline double ln_q(int w, double S) {
     int ks = (S >= (double)(w - 1)) ? (w - 1) : (int)floor(S);
     double sum = 1.0, t = 1.0;
     const double inv_s = 1.0 / S;
-    for (int k = ks; k >= 1; --k) {
-        t *= (double)k * inv_s;
-        sum += t;
-        if (t < 1e-18 * sum) break;
+    // terms ks−1 … 0: t_{j+1} = t_j · k/S with k = ks, ks−1, …; the ratio is carried as a double (no conversion per term) and
+    // the stopping test runs every fourth term
+    double kd = (double)ks;
+    int k = ks;
+    for (; k >= 4; k -= 4) {
+        t *= kd * inv_s; sum += t; kd -= 1.0;
+        t *= kd * inv_s; sum += t; kd -= 1.0;
+        t *= kd * inv_s; sum += t; kd -= 1.0;
+        t *= kd * inv_s; sum += t; kd -= 1.0;
+        if (t < 1e-18 * sum) { k = 0; break; }
     }
+    for (; k >= 1; --k) { t *= kd * inv_s; sum += t; kd -= 1.0; }
     t = 1.0;
     for (int k = ks + 1; k <= w - 1; ++k) {
         t *= S / (double)k;

@@ -453,7 +453,7 @@ def test_polynomial_logp_matches_oracle(orc, n, batch, zmax, B, C, thr, numharm,
     assert len(ora) > 0
     _assert_same_hcandidates(gpu, ora, f"Alg. 3 n={n} zmax={zmax} numharm={numharm} mode={mode}")
     exact = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, numharm, log_sampling=log_sampling, median_of_medians=mom)
-    if zmax <= 64:
+    if zmax <= 64 and numharm == 1:
         assert len(ora) <= len(exact)        # usable region: Alg. 3 under-states significance, marginal candidates drop out
     if zmax == 300:
         assert len(ora) > 2 * len(exact)     # divergent region: wide widths pass on pure noise
