@@ -104,6 +104,7 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
         long long end = hi + zmax - 1;              // last bin any window of the block can touch, exclusive: hi−1+zmax
         if (end > n) end = n;
         const int L = (int)(end - lo);
+        if (tid == 0) { hdr.nlist[0] = 0; hdr.nlist[1] = 0; }   // (barriers of the prefix build separate this from the first use)
 
         // double-precision prefix sum pre[j] = Σ_{t<j} P[lo+t]: coalesced loads (or rebuilds, power_source.cuh) into
         // pre[j+1], each thread then scans its own chunk in place and the chunk totals are scanned by one warp
@@ -144,7 +145,8 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
         // width by shuffles (adjacent lanes, increasing start bins: ties keep the lower bin, R14); then ln p where it can matter
         double my_lnp = INFINITY, my_s = 0.0;
         int my_w = 0, my_i = 0;
-        for (int w0 = part * w_per_round; w0 < zmax; w0 += nparts * w_per_round) {
+        int rnd = 0;                                        // which of the two list counters this round uses
+        for (int w0 = part * w_per_round; w0 < zmax; w0 += nparts * w_per_round, rnd ^= 1) {
             const int w = w0 + (tid >> lg_split) + 1;
             double best = -1.0;
             int arg = -1;
@@ -164,7 +166,6 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
             }
             // The widths whose maximum reaches T_w are collected and their ln p evaluated by all threads: the series of ln Q is
             // a serial loop of up to w terms, and only one lane in 2^lg_split holds a width after the reduction above.
-            const int rnd = (w0 / w_per_round) & 1;
             if (piece == 0 && w <= zmax && arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
                 const unsigned slot = atomicAdd(&hdr.nlist[rnd], 1u);
                 hdr.list_s[slot] = best; hdr.list_w[slot] = w; hdr.list_i[slot] = arg;

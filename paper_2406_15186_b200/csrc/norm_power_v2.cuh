@@ -392,7 +392,7 @@ template <int EPT, int NT, bool STAGED>
 __global__ void __launch_bounds__(NT, STAGED ? ((EPT * NT <= 4096) ? 4 : 2) : (NT == 128 ? (EPT <= 16 ? PULSCAN_NORM_OCC128_SMALL : PULSCAN_NORM_OCC128) : (EPT * NT <= 4096) ? 6 : 4))
 norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int blocks_per_row, int nb, NormOut out,
                      unsigned* __restrict__ redo, unsigned* __restrict__ redo_count,
-                     const char* __restrict__ lim_lo, const char* __restrict__ lim_hi) {
+                     const char* __restrict__ lim_lo, const char* __restrict__ lim_hi, unsigned l2_ahead) {
     static_assert(EPT % 2 == 0 && EPT <= 32, "bucket indices are packed in pairs; hit mask has 16 + 16 bits");
     static_assert(NT % 32 == 0 && (EPT * NT) % 128 == 0, "sample stride");
     constexpr int B = EPT * NT;
@@ -412,6 +412,18 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     const unsigned nbytes = (unsigned)B * 8u + (shift ? 16u : 0u);
     const bool use_tma = STAGED && csrc >= lim_lo && csrc + nbytes <= lim_hi;
     const float2* sdat = STAGED ? reinterpret_cast<const float2*>(stage + shift) : src;
+    // L2 look-ahead: ask for the block that the CTA `l2_ahead` launches behind this one will work on (about one wave of
+    // resident CTAs later) to be brought into L2 now, with one bulk prefetch that occupies no register and no LSU slot.
+    // That CTA's three passes then find their 8·B bytes in L2: the HBM stream is decoupled from the latency-bound phases.
+    if (!STAGED && l2_ahead && tid == 0 && blockIdx.x + l2_ahead < gridDim.x) {
+        const unsigned nxt = blockIdx.x + l2_ahead;
+        const unsigned nrow = nxt / (unsigned)blocks_per_row;
+        const char* a = reinterpret_cast<const char*>(spectra + (long long)nrow * pitch_in + (long long)(nxt - nrow * (unsigned)blocks_per_row) * B);
+        const char* a16 = a - (reinterpret_cast<uintptr_t>(a) & 15);
+        const unsigned nb16 = (unsigned)B * 8u + 16u;
+        if (a16 >= lim_lo && a16 + nb16 <= lim_hi)
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a16), "r"(nb16) : "memory");
+    }
     if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(v2_smem(&ctl.mbar)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");

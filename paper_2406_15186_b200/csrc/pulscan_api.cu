@@ -111,6 +111,7 @@ struct pulscan_plan {
     int ept_main = 0, nt_main = 0, ept_tail = 0, nt_tail = 0, main_blocks_per_row = 0;
     bool has_tail = false;
     int norm_nt = 256;         // threads per CTA of the single-histogram kernel
+    unsigned norm_l2_ahead = 0; // single-histogram kernel: bulk-prefetch into L2 the block of the CTA this many launches ahead
     bool norm_staged = false;  // single-histogram kernel variant: block staged in shared memory by TMA, or read from global
     bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_v2_kernel + redo list
     // workspace (device, caller-owned)
@@ -478,6 +479,10 @@ int finalize_device(pulscan_plan& p) {
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_refine_kernel, kRefineThreads, p.smem_refine));
     if (occ < 1) return fail(PULSCAN_ECUDA, "sweep_refine_kernel does not fit an SM with %zu bytes of shared memory", p.smem_refine);
     p.refine_grid = p.sm_count * std::min(occ, 16);
+    {   // about one wave of resident CTAs of the single-histogram kernel (8-10 per SM); PULSCAN_NORM_L2_AHEAD overrides (0 = off)
+        const char* e = std::getenv("PULSCAN_NORM_L2_AHEAD");
+        p.norm_l2_ahead = e ? (unsigned)std::strtoul(e, nullptr, 10) : (unsigned)p.sm_count * 8u;
+    }
     p.finalized = true;
     return PULSCAN_OK;
 }
@@ -548,7 +553,7 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
 #define PULSCAN_V2_LAUNCH(E, NT_, ST)                                                                                 \
     {                                                                                                                 \
         norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                              \
-            spec, p.pitch, p.main_blocks_per_row, p.nb, out, redo, redo_count, lim_lo, lim_hi);                       \
+            spec, p.pitch, p.main_blocks_per_row, p.nb, out, redo, redo_count, lim_lo, lim_hi, p.norm_l2_ahead);      \
     }
 #define PULSCAN_V2_REDO(E)                                                                                            \
     norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.nb, p.main_blocks_per_row, out, redo, \
