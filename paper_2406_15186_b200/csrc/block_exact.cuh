@@ -24,9 +24,9 @@ namespace pulscan {
 
 constexpr int kExactThreads = 1024;
 
-struct ExactSmemHdr {
+struct alignas(16) ExactSmemHdr {   // the prefix array behind it is read with 16-byte loads
     double part[kExactThreads];   // per-thread chunk sums for the prefix scan
-    double list_s[kExactThreads]; // widths of the current round whose maximum reaches T_w: (maximum, width, arg-max)
+    double list_s[kExactThreads]; // widths of the current step whose maximum reaches T_w: (maximum, width, arg-max)
     int list_w[kExactThreads];
     int list_i[kExactThreads];
     unsigned nlist[2];
@@ -83,10 +83,10 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
     if (tid == 0) { hdr.nlist[0] = 0; hdr.nlist[1] = 0; }
     __syncthreads();
     const int nsplit = 1 << lg_split, piece = tid & (nsplit - 1), w_per_round = kExactThreads >> lg_split;
-    // start bins per chunk; for 4 or more chunks rounded up to ≡ 32/nsplit (mod 16) doubles, so that the nsplit segments a
-    // warp reads with one LDS.64 (32/nsplit consecutive widths each) fall on disjoint banks: 2 wavefronts instead of 4
+    // start bins per chunk: even (16-byte loads of pairs of doubles), and ≡ 2 (mod 4) when there are several chunks, so that
+    // the chunks' 16-byte loads of a warp (lanes of a chunk 32 bytes apart) interleave on the banks: 4 wavefronts per 512 bytes
     int cs = (C + nsplit - 1) >> lg_split;
-    if (nsplit >= 4) cs += (((32 >> lg_split) - cs) & 15);
+    if (nsplit >= 2) cs += (2 - cs) & 3;
 
     const unsigned n_split = parts > 1 ? min(nflag, split_slots) : 0u;
     const unsigned n_items = n_split * (unsigned)parts + (nflag - n_split);
@@ -141,50 +141,79 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
         }
         __syncthreads();
 
-        // (width, chunk of start bins) per thread: maximum and lowest arg-max over the chunk, combined over the chunks of a
-        // width by shuffles (adjacent lanes, increasing start bins: ties keep the lower bin, R14); then ln p where it can matter
+        // (four consecutive widths, chunk of start bins) per thread.  A 4 × 4 register tile — starts i..i+3, widths W4..W4+3 —
+        // needs pre[i..i+3] and pre[i+W4 .. i+W4+6]: 6 shared-memory loads for 16 window sums instead of 32 (the kernel is
+        // bound by the rate of LDS instructions).  Per width the maximum and its lowest arg-max (strict >, ascending starts:
+        // R14), combined over the chunks of a width by shuffles (adjacent lanes, the lower chunk holds the lower bins).
         double my_lnp = INFINITY, my_s = 0.0;
         int my_w = 0, my_i = 0;
         int rnd = 0;                                        // which of the two list counters this round uses
-        for (int w0 = part * w_per_round; w0 < zmax; w0 += nparts * w_per_round, rnd ^= 1) {
-            const int w = w0 + (tid >> lg_split) + 1;
-            double best = -1.0;
-            int arg = -1;
-            if (w <= zmax) {
-                const int imax = min(nstart, L - w + 1);   // starts i with i + w ≤ L
-                const int i1 = min((piece + 1) * cs, imax);
-                for (int i = piece * cs; i < i1; ++i) {
-                    const double v = pre[i + w] - pre[i];
-                    if (v > best) { best = v; arg = i; }
+        const int nquads = zmax / 4 + 1;                    // width quads {4q, …, 4q+3}; width 0 does not exist
+        for (int q0 = part * w_per_round; q0 < nquads; q0 += nparts * w_per_round) {
+            const int W4 = 4 * (q0 + (tid >> lg_split));
+            double best[4] = {-1.0, -1.0, -1.0, -1.0};
+            int arg[4] = {-1, -1, -1, -1};
+            if (W4 <= zmax) {
+                const int lo_i = piece * cs, hi_i = lo_i + cs;
+                const int full_end = min(hi_i, min(nstart, L - (W4 + 3) + 1));   // all four widths exist for starts below this
+                int i = lo_i;
+                for (; i + 4 <= full_end; i += 4) {
+                    const double2 p01 = *reinterpret_cast<const double2*>(pre + i), p23 = *reinterpret_cast<const double2*>(pre + i + 2);
+                    const double* pj = pre + i + W4;
+                    const double2 j01 = *reinterpret_cast<const double2*>(pj), j23 = *reinterpret_cast<const double2*>(pj + 2),
+                                  j45 = *reinterpret_cast<const double2*>(pj + 4);
+                    const double pi[4] = {p01.x, p01.y, p23.x, p23.y};
+                    const double jv[7] = {j01.x, j01.y, j23.x, j23.y, j45.x, j45.y, pj[6]};
+#pragma unroll
+                    for (int a4 = 0; a4 < 4; ++a4)
+#pragma unroll
+                        for (int b4 = 0; b4 < 4; ++b4) {
+                            const double v = jv[a4 + b4] - pi[a4];
+                            if (v > best[b4]) { best[b4] = v; arg[b4] = i + a4; }
+                        }
+                }
+#pragma unroll
+                for (int b4 = 0; b4 < 4; ++b4) {            // the starts that only some of the four widths have
+                    const int w = W4 + b4;
+                    const int i1 = min(hi_i, min(nstart, L - w + 1));
+                    for (int t = i; t < i1; ++t) {
+                        const double v = pre[t + w] - pre[t];
+                        if (v > best[b4]) { best[b4] = v; arg[b4] = t; }
+                    }
+                    if (w < 1 || w > zmax) { best[b4] = -1.0; arg[b4] = -1; }
                 }
             }
-            for (int off = 1; off < nsplit; off <<= 1) {       // lanes piece, piece^off: the lower piece holds the lower bins
-                const double ob = __shfl_xor_sync(0xffffffffu, best, off);
-                const int oa = __shfl_xor_sync(0xffffffffu, arg, off);
-                const bool other_lower = (piece & off) != 0;
-                if (ob > best || (ob == best && other_lower && oa >= 0)) { best = ob; arg = oa; }
+#pragma unroll
+            for (int b4 = 0; b4 < 4; ++b4, rnd ^= 1) {         // one of the thread's four widths per step (the list holds 1024)
+                for (int off = 1; off < nsplit; off <<= 1) {   // lanes piece, piece^off: the lower piece holds the lower bins
+                    const double ob = __shfl_xor_sync(0xffffffffu, best[b4], off);
+                    const int oa = __shfl_xor_sync(0xffffffffu, arg[b4], off);
+                    const bool other_lower = (piece & off) != 0;
+                    if (ob > best[b4] || (ob == best[b4] && other_lower && oa >= 0)) { best[b4] = ob; arg[b4] = oa; }
+                }
+                // The widths whose maximum reaches T_w are collected and their ln p evaluated by all threads: the series of
+                // ln Q is a serial loop of up to w terms, and only one lane in 2^lg_split holds a width after the reduction.
+                const int w = W4 + b4;
+                if (piece == 0 && arg[b4] >= 0 && best[b4] >= T_g[w - 1] * (1.0 - 1e-9)) {
+                    const unsigned slot = atomicAdd(&hdr.nlist[rnd], 1u);
+                    hdr.list_s[slot] = best[b4]; hdr.list_w[slot] = w; hdr.list_i[slot] = arg[b4];
+                }
+                __syncthreads();
+                const int nl = (int)hdr.nlist[rnd];
+                if (tid == 0) hdr.nlist[rnd ^ 1] = 0;
+                for (int idx = tid; idx < nl; idx += kExactThreads) {
+                    const int lw = hdr.list_w[idx], li = hdr.list_i[idx];
+                    const double ls = hdr.list_s[idx];
+                    // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220); signif_mode 1: Alg. 3's polynomial instead of the tail
+                    double lnp = lnp_of(signif_mode, lw * shape_mult, ls) + ln_trials;
+                    if (lnp > 0.0) lnp = 0.0;
+                    if (per_width) {   // the paper's GPU output: one candidate per (block, searched width) above the threshold (Alg. 4)
+                        if (lnp <= lnp_thr)
+                            emit_candidate(row, r_block ? (int32_t)lo : (int32_t)(lo + li), lw, ls, lnp, numharm, out, out_h, out_count, capacity);
+                    } else if (lnp < my_lnp || (lnp == my_lnp && lw < my_w)) { my_lnp = lnp; my_w = lw; my_i = li; my_s = ls; }   // ties keep the smaller width
+                }
+                __syncthreads();
             }
-            // The widths whose maximum reaches T_w are collected and their ln p evaluated by all threads: the series of ln Q is
-            // a serial loop of up to w terms, and only one lane in 2^lg_split holds a width after the reduction above.
-            if (piece == 0 && w <= zmax && arg >= 0 && best >= T_g[w - 1] * (1.0 - 1e-9)) {
-                const unsigned slot = atomicAdd(&hdr.nlist[rnd], 1u);
-                hdr.list_s[slot] = best; hdr.list_w[slot] = w; hdr.list_i[slot] = arg;
-            }
-            __syncthreads();
-            const int nl = (int)hdr.nlist[rnd];
-            if (tid == 0) hdr.nlist[rnd ^ 1] = 0;
-            for (int idx = tid; idx < nl; idx += kExactThreads) {
-                const int lw = hdr.list_w[idx], li = hdr.list_i[idx];
-                const double ls = hdr.list_s[idx];
-                // harmonic-summed spectra: χ² with H(H+1)·w d.o.f. (L220); signif_mode 1: Alg. 3's polynomial instead of the tail
-                double lnp = lnp_of(signif_mode, lw * shape_mult, ls) + ln_trials;
-                if (lnp > 0.0) lnp = 0.0;
-                if (per_width) {   // the paper's GPU output: one candidate per (block, searched width) above the threshold (Alg. 4)
-                    if (lnp <= lnp_thr)
-                        emit_candidate(row, r_block ? (int32_t)lo : (int32_t)(lo + li), lw, ls, lnp, numharm, out, out_h, out_count, capacity);
-                } else if (lnp < my_lnp || (lnp == my_lnp && lw < my_w)) { my_lnp = lnp; my_w = lw; my_i = li; my_s = ls; }   // ties keep the smaller width
-            }
-            __syncthreads();
         }
         // block arg-min over (ln p, w)
 #pragma unroll

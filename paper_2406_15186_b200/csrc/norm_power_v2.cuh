@@ -376,6 +376,12 @@ __device__ __forceinline__ void v2_mbar_wait(unsigned long long* mbar, unsigned 
     }
 }
 
+// Which instantiations use the L2 look-ahead (see the kernel): measured on a B200 it pays for short blocks only, where the
+// first touch of a block is a larger share of its time (cfg 5, B = 2048: 8.25 -> 7.61 ms with a look-ahead of 592 CTAs;
+// cfg 3, B = 4096: 3.18 -> 3.25 ms; cfg 4, B = 8192: 0.905 -> 0.96 ms), so it is compiled out of the others.
+template <int EPT, int NT, bool STAGED>
+constexpr bool kV2L2Ahead() { return !STAGED && EPT * NT <= 2048; }
+
 // Dynamic shared memory of norm_power_v2_kernel<EPT, NT>: [stage: 8·B + 16 bytes][hist: 2·NB·4][V2Ctl].
 template <int EPT, int NT, bool STAGED>
 constexpr size_t v2_smem_bytes() {
@@ -415,7 +421,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     // L2 look-ahead: ask for the block that the CTA `l2_ahead` launches behind this one will work on (about one wave of
     // resident CTAs later) to be brought into L2 now, with one bulk prefetch that occupies no register and no LSU slot.
     // That CTA's three passes then find their 8·B bytes in L2: the HBM stream is decoupled from the latency-bound phases.
-    if (!STAGED && l2_ahead && tid == 0 && blockIdx.x + l2_ahead < gridDim.x) {
+    if (kV2L2Ahead<EPT, NT, STAGED>() && l2_ahead && tid == 0 && blockIdx.x + l2_ahead < gridDim.x) {
         const unsigned nxt = blockIdx.x + l2_ahead;
         const unsigned nrow = nxt / (unsigned)blocks_per_row;
         const char* a = reinterpret_cast<const char*>(spectra + (long long)nrow * pitch_in + (long long)(nxt - nrow * (unsigned)blocks_per_row) * B);

@@ -343,15 +343,21 @@ int derive(pulscan_plan& p) {
     p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
     p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
-    {   // kernel (c): split the start bins of a block over 2^lg adjacent lanes so that rounds × starts per chunk is smallest
+    {   // kernel (c): a thread owns four consecutive widths; the start bins of a block are split over 2^lg adjacent lanes.  One
+        // block costs zmax·C window sums on ONE SM (the kernel is issue-bound: double-precision compare and select): when that
+        // is large (cfg 4: 1.44 M) the widths of a block are dealt to several CTAs, so lg is chosen to give at least that
+        // many rounds of 1024 threads; otherwise the lg with the fewest iterations per thread.
+        const long long nquads = p.zmax / 4 + 1;
+        const long long want_parts = std::min<long long>(8, std::max<long long>(1, ((long long)p.zmax * p.C + 75000) / 150000));
         long long best = -1;
         for (int lg = 0; lg <= 5; ++lg) {
-            const long long rounds = ((long long)p.zmax * (1 << lg) + kExactThreads - 1) / kExactThreads;
-            const long long cost = rounds * (((p.C + (1 << lg) - 1) >> lg) + (lg >= 2 ? 8 : 0)) + 2 * lg;
+            const long long rounds = (nquads * (1 << lg) + kExactThreads - 1) / kExactThreads;
+            long long cost = ((rounds + want_parts - 1) / want_parts) * ((((p.C + (1 << lg) - 1) >> lg) + 3) / 4 + 8) + lg;
+            if (rounds < want_parts) cost += 1000000;          // cannot be split that far
             if (best < 0 || cost < best) { best = cost; p.exact_lg_split = lg; }
         }
-        const int rounds = (int)(((long long)p.zmax * (1 << p.exact_lg_split) + kExactThreads - 1) / kExactThreads);
-        p.exact_parts = std::min(rounds, 8);
+        const int rounds = (int)((nquads * (1 << p.exact_lg_split) + kExactThreads - 1) / kExactThreads);
+        p.exact_parts = (int)std::min<long long>(rounds, want_parts);
         p.exact_slots = p.exact_parts > 1 ? (unsigned)std::min<long long>((long long)p.batch * p.nblk, 16384) : 0u;
     }
 
@@ -479,9 +485,10 @@ int finalize_device(pulscan_plan& p) {
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, sweep_refine_kernel, kRefineThreads, p.smem_refine));
     if (occ < 1) return fail(PULSCAN_ECUDA, "sweep_refine_kernel does not fit an SM with %zu bytes of shared memory", p.smem_refine);
     p.refine_grid = p.sm_count * std::min(occ, 16);
-    {   // about one wave of resident CTAs of the single-histogram kernel (8-10 per SM); PULSCAN_NORM_L2_AHEAD overrides (0 = off)
+    {   // look-ahead of the single-histogram kernel's L2 prefetch in CTAs (short blocks only, see kV2L2Ahead): half a wave of
+        // resident CTAs measured best (592 and 1184: 7.61 ms at cfg 5; 2368: 8.0; off: 8.25); PULSCAN_NORM_L2_AHEAD overrides
         const char* e = std::getenv("PULSCAN_NORM_L2_AHEAD");
-        p.norm_l2_ahead = e ? (unsigned)std::strtoul(e, nullptr, 10) : (unsigned)p.sm_count * 8u;
+        p.norm_l2_ahead = e ? (unsigned)std::strtoul(e, nullptr, 10) : (unsigned)p.sm_count * 4u;
     }
     p.finalized = true;
     return PULSCAN_OK;
@@ -1088,6 +1095,9 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
     s += line;
     snprintf(line, sizeof line, "intermediate in HBM: %s\n",
              p.keep_P ? "float32 power of every bin (4 B/bin)" : "sums of 4-bin groups (1 B/bin) + 32 B per normalisation block");
+    s += line;
+    snprintf(line, sizeof line, "exact: 4 widths per thread, start bins split over %d lanes, widths of a block dealt to %d CTA(s)\n",
+             1 << p.exact_lg_split, p.exact_parts);
     s += line;
     snprintf(line, sizeof line, "exact: smem=%zu B; workspace=%zu B; T_1=%.4f T_zmax=%.4f\n", p.smem_exact, p.need_bytes, p.T.front(), p.T.back());
     s += line;
