@@ -18,9 +18,19 @@
  * so at most one candidate per (spectrum, candidate block).
  *
  * Conventions.  All `d_` pointers are DEVICE pointers, all `h_` pointers are HOST pointers; the library never
- * takes ownership of either.  Every function returns PULSCAN_OK (0) or a negative error code and never throws;
+ * takes ownership of either and owns no device memory of its own (its small threshold tables live in the caller's
+ * workspace).  Every function returns PULSCAN_OK (0) or a negative error code and never throws;
  * pulscan_last_error() describes the last failure on the calling thread.  There is no CPU fallback: without a
- * CUDA device of compute capability 10.x the search functions return PULSCAN_ECUDA / PULSCAN_EARCH.
+ * CUDA device of compute capability 10.x pulscan_plan_set_workspace returns PULSCAN_ECUDA / PULSCAN_EARCH.
+ *
+ * Life of a plan.  (1) configure: pulscan_plan_create and the pulscan_plan_set_* calls are host-only and touch no CUDA
+ * device.  (2) finalise: pulscan_plan_set_workspace checks the device, uploads the tables into the workspace (synchronous
+ * copies), sets the kernels' shared-memory attributes on the CURRENT device and fixes the launch shapes — the only place
+ * besides the launches that calls the CUDA runtime.  (3) search: pulscan_search / pulscan_search_harmonics allocate
+ * nothing and never synchronise, from their first call on (the first search of a fresh plan can be captured into a CUDA
+ * graph).  A setter that changes derived state or the workspace layout (every setter except _set_r_block, and
+ * _set_emission without host staging) returns the plan to step (1): searches then fail with PULSCAN_ENOWORKSPACE until
+ * pulscan_plan_set_workspace is called again (pulscan_plan_workspace_bytes may have changed).
  */
 #ifndef PULSCAN_H
 #define PULSCAN_H
@@ -87,7 +97,8 @@ int pulscan_plan_set_trials(pulscan_plan* plan, double n_trials);
 int pulscan_plan_set_pitch(pulscan_plan* plan, int64_t pitch_bins);
 
 /* Search mode: 0 = pruned sweep (default; exact — cover-sum upper bounds only discard windows that cannot reach
- * their width's power threshold), 1 = exhaustive sweep (every (bin, width) evaluated; the cross-check). */
+ * their width's power threshold), 1 = exhaustive sweep (every (bin, width) evaluated; the cross-check; it keeps the
+ * float32 power of every bin in the workspace, so the workspace grows and must be attached again). */
 int pulscan_plan_set_mode(pulscan_plan* plan, int32_t mode);
 
 /* Which boxcar widths are SEARCHED for candidates; all widths are still summed (L152 "the user can select the step size to
@@ -152,17 +163,22 @@ int pulscan_plan_set_cell_capacity(pulscan_plan* plan, int64_t cells);
 /* Capacity the caller must give d_candidates: batch · ceil(n_bins / block_width) records. */
 int64_t pulscan_plan_max_candidates(const pulscan_plan* plan);
 
-/* Scratch the caller must provide (device memory, 256-byte aligned): the float32 power intermediate
- * [batch][power_pitch], the flagged-block list and counters.  With host staging enabled it also holds a device
- * copy of the input for pulscan_search_host. */
+/* Scratch the caller must provide (device memory, 256-byte aligned): the sums of 4-bin groups of the power spectrum
+ * [batch][group_pitch] and 32 bytes per normalisation block (or, in exhaustive mode / with levels finer than 4 bins / for
+ * the harmonic search / with the Alg. 1 normalisation, the float32 power of every bin [batch][power_pitch]), the
+ * flagged-cell and flagged-block lists, counters and the threshold tables.  With host staging enabled it also holds a
+ * device copy of the input for pulscan_search_host.  pulscan_plan_set_workspace FINALISES the plan (see "Life of a plan"):
+ * it is synchronous, must be called with the target device current, and again after any setter that changes the plan. */
 size_t pulscan_plan_workspace_bytes(const pulscan_plan* plan);
 int pulscan_plan_enable_host_staging(pulscan_plan* plan, int32_t enable);
 int pulscan_plan_set_workspace(pulscan_plan* plan, void* d_workspace, size_t bytes);
 
 /* Run the whole path on the device.  d_spectra: complex64 [batch][pitch] (interleaved re, im float32; 8-byte
- * aligned; read-only).  d_candidates: pulscan_plan_max_candidates() records.  d_count: one uint32, zeroed by the
- * call, then the number of candidates.  Enqueues kernels on `cuda_stream` (a cudaStream_t; NULL = default
- * stream), allocates nothing and does not synchronise; the order of the records is unspecified (R19). */
+ * aligned; read-only; it must stay valid until the search has finished: flagged spans are rebuilt from it).
+ * d_candidates: pulscan_plan_max_candidates() records.  d_count: one uint32, zeroed by the call, then the number of
+ * candidates.  Enqueues memsets and kernels on `cuda_stream` (a cudaStream_t; NULL = default stream) and nothing else:
+ * no allocation, no synchronisation, no other runtime call — on every call, the first included (CUDA-graph capturable);
+ * the order of the records is unspecified (R19).  PULSCAN_ENOWORKSPACE if the plan is not finalised. */
 int pulscan_search(pulscan_plan* plan, const void* d_spectra, pulscan_candidate* d_candidates, uint32_t* d_count,
                    void* cuda_stream);
 
@@ -202,7 +218,7 @@ int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_str
 /* Kernels one pulscan_search() enqueues for this plan (memsets not counted). */
 int32_t pulscan_plan_launches_per_search(const pulscan_plan* plan);
 
-/* Per-kernel timing.  set_profiling(n_slots > 0) makes every pulscan_search record CUDA events on its stream
+/* Per-kernel timing.  set_profiling(n_slots > 0) creates 5·n_slots CUDA events (needs a current device) and makes every pulscan_search record them on its stream
  * around its stages into slot (search index mod n_slots); get_profile waits for that search and returns
  * h_ms[0..3] = milliseconds of {workspace memsets, kernel (a) normalise+power, kernel (b) sweep, kernel (c) exact
  * evaluation + significance + compaction}.  n_slots = 0 (default) records nothing. */

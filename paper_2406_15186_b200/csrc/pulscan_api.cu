@@ -344,15 +344,17 @@ int derive(pulscan_plan& p) {
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
     p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
     {   // kernel (c): a thread owns four consecutive widths; the start bins of a block are split over 2^lg adjacent lanes.  One
-        // block costs zmax·C window sums on ONE SM (the kernel is issue-bound: double-precision compare and select): when that
-        // is large (cfg 4: 1.44 M) the widths of a block are dealt to several CTAs, so lg is chosen to give at least that
-        // many rounds of 1024 threads; otherwise the lg with the fewest iterations per thread.
+        // block costs zmax·C window sums on ONE SM (issue-bound: double-precision compare and select) plus ≈ 45 µs of
+        // barrier-separated set-up per CTA (prefix sum rebuilt from the spectrum, ln p of the passing widths): only when the
+        // window sums are several times that (measured at cfg 4, 1.44 M sums per block: 1 CTA 0.245 ms, 8 CTAs 0.387 ms) are
+        // the widths of a block dealt to several CTAs; lg is then chosen to give that many rounds of 1024 threads.
         const long long nquads = p.zmax / 4 + 1;
-        const long long want_parts = std::min<long long>(8, std::max<long long>(1, ((long long)p.zmax * p.C + 75000) / 150000));
+        const long long want_parts = std::min<long long>(8, std::max<long long>(1, (long long)p.zmax * p.C / 3000000));
         long long best = -1;
         for (int lg = 0; lg <= 5; ++lg) {
             const long long rounds = (nquads * (1 << lg) + kExactThreads - 1) / kExactThreads;
-            long long cost = ((rounds + want_parts - 1) / want_parts) * ((((p.C + (1 << lg) - 1) >> lg) + 3) / 4 + 8) + lg;
+            // a round costs its 4 x 4 tiles plus eight barriers and the ln p evaluations (worth ~48 tiles)
+            long long cost = ((rounds + want_parts - 1) / want_parts) * ((((p.C + (1 << lg) - 1) >> lg) + 3) / 4 + 48) + lg;
             if (rounds < want_parts) cost += 1000000;          // cannot be split that far
             if (best < 0 || cost < best) { best = cost; p.exact_lg_split = lg; }
         }

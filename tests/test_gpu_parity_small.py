@@ -87,6 +87,8 @@ CASES = [
     (5000, 4, 7, 512, 1, 3.5),
     (777, 2, 100, 256, 5000, 3.0),
     (2100, 1, 2000, 1024, 50, 3.5),
+    (30011, 1, 4096, 8192, 2000, 4.0),     # zmax·C = 8.2 M window sums per block: kernel (c) deals a block's widths to 2 CTAs
+    (40001, 2, 3000, 4096, 3100, 4.5),     # … to 3 CTAs
 ]
 
 
