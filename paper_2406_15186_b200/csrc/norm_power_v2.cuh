@@ -29,6 +29,9 @@
 
 #include "norm_power.cuh"
 
+#ifndef PULSCAN_V2_SAMPLE_AHEAD
+#define PULSCAN_V2_SAMPLE_AHEAD 0
+#endif
 #ifndef PULSCAN_NORM_OCC128_SMALL
 #define PULSCAN_NORM_OCC128_SMALL 10   /* EPT <= 16 fits 48 registers without spills: cfg 5 kernel (a) 8.85 -> 8.61 ms */
 #endif
@@ -430,6 +433,20 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         if (a16 >= lim_lo && a16 + nb16 <= lim_hi)
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a16), "r"(nb16) : "memory");
     }
+#if PULSCAN_V2_SAMPLE_AHEAD
+    // Longer blocks: only the four runs of 32 bins that the later CTA's sample estimate reads (its first, latency-bound step)
+    if (!STAGED && !kV2L2Ahead<EPT, NT, STAGED>() && l2_ahead && tid == 0 && blockIdx.x + l2_ahead < gridDim.x) {
+        const unsigned nxt = blockIdx.x + l2_ahead;
+        const unsigned nrow = nxt / (unsigned)blocks_per_row;
+        const char* a = reinterpret_cast<const char*>(spectra + (long long)nrow * pitch_in + (long long)(nxt - nrow * (unsigned)blocks_per_row) * B);
+        const char* a16 = a - (reinterpret_cast<uintptr_t>(a) & 15);
+        if (a16 >= lim_lo && a16 + (unsigned)B * 8u + 16u <= lim_hi) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(a16 + (size_t)k * (B / 4) * 8), "r"(272u) : "memory");
+        }
+    }
+#endif
     if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(v2_smem(&ctl.mbar)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
