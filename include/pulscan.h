@@ -151,7 +151,7 @@ int pulscan_plan_set_significance(pulscan_plan* plan, int32_t mode);
 int pulscan_plan_set_emission(pulscan_plan* plan, int32_t per_width, int64_t capacity);
 
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
- * probability in noise as log10 (−2 … −9; 0 = default).  Affects speed only, never results. */
+ * probability in noise as log10 (−1 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);
 
 /* Capacity (in cells, 8 bytes each) of the list that carries flagged cover cells from the sweep to its refine kernel;

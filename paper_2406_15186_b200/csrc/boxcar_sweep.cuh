@@ -66,6 +66,10 @@ struct SweepLevel {
     int nk;        // group starts per tile = tile / g
     int wt_off;    // first warp-task of this level; a warp-task is 32 lanes × 8 group starts
     int nwt;       // warp-tasks of this level
+    // second look at a flagged cell with groups of half the size (sweep_refine_kernel, from the group sums); nmh = 0: none
+    int tauh_off;  // offset of τ_h[mh − mh_start] in the τ table: thresholds of covers made of mh half-groups of g/2 bins
+    int mh_start;  // first half-cover length in that table (= 2·m_start − 2, clamped at 0)
+    int nmh;       // entries of that table
 };
 
 struct SweepParams {
@@ -501,8 +505,8 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
 // are summed and compared with T'_w.  A window that passes marks the candidate block of its start bin.
 // Dynamic shared memory: (kRefineThreads/32) × (ref_span + 1) doubles.
 __global__ void __launch_bounds__(kRefineThreads)
-sweep_refine_kernel(const __grid_constant__ SweepParams sp, const PowerSource src_pw, long long n,
-                    int tiles_per_row, int C, long long nblk, const float* __restrict__ tau_g,
+sweep_refine_kernel(const __grid_constant__ SweepParams sp, const PowerSource src_pw, const float* __restrict__ G,
+                    long long pitchG, long long n, int tiles_per_row, int C, long long nblk, const float* __restrict__ tau_g,
                     const float* __restrict__ Tp_g, const SweepCell* __restrict__ cells, unsigned cell_cap,
                     unsigned* __restrict__ bitmap, unsigned* __restrict__ flagged, unsigned* __restrict__ counters) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -533,6 +537,51 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const PowerSource sr
                 }
                 if (__all_sync(0xffffffffu, marked)) continue;
             }
+        }
+        // ---- Second look, from the group sums (1 B/bin, no rebuild).  A cover of m groups of g bins is 2g − 2 bins longer than
+        // the narrowest window it answers for, and most noise flags live off that slack.  The same window is also covered by
+        // half-groups of g/2 bins — starts in half a of the first group, ends in half b of the last, mh = 2m − 1 + b − a
+        // half-groups — and that cover is only g − 2 bins longer than its narrowest window: the four half-covers of every
+        // passing cover are tested against their own thresholds τ_h[mh] (the lowest T'_w among the level's searched widths
+        // (mh − 2)·g/2 + 2 … mh·g/2, rounded down like τ).  A window that reaches its T_w passes its half-cover for the same
+        // reason it passes its cover (P ≥ 0; the group sums are float32 sums of four powers, 2·2⁻²⁴ relative, inside τ_h's
+        // margin), so a cell without a passing half-cover holds nothing.  Needs g ≥ 8 (half-groups are whole group sums).
+        if (G != nullptr && lg >= 3 && lv.nmh > 0) {
+            const float* gsrc = G + row * pitchG + (base >> 2);
+            const int nq = span >> 2, vq = (valid + 3) >> 2;
+            for (int j = lane; j < nq; j += 32) pp[j + 1] = (j < vq) ? (double)__ldg(gsrc + j) : 0.0;
+            if (lane == 0) pp[0] = 0.0;
+            __syncwarp();
+            {
+                const int Lq = (nq + 31) >> 5;
+                const int q0 = min(lane * Lq, nq), q1 = min(q0 + Lq, nq);
+                double run = 0.0;
+                for (int j = q0; j < q1; ++j) { run += pp[j + 1]; pp[j + 1] = run; }
+                double incl = run;
+#pragma unroll
+                for (int off = 1; off < 32; off <<= 1) {
+                    const double t = __shfl_up_sync(0xffffffffu, incl, off);
+                    if (lane >= off) incl += t;
+                }
+                const double excl = incl - run;
+                for (int j = q0; j < q1; ++j) pp[j + 1] += excl;
+            }
+            __syncwarp();
+            const int r = lane & 7, m = m4 + (lane >> 3), lq = lg - 2, lhq = lg - 3;   // group / half-group size in quads: 2^lq, 2^lhq
+            bool confirmed = false;
+            if (pp[(r + m) << lq] - pp[r << lq] >= (double)__ldg(tau_g + lv.tau_off + 4 * step + (lane >> 3)) * (1.0 - 1e-6)) {
+#pragma unroll
+                for (int ab = 0; ab < 4; ++ab) {
+                    const int ha = ab & 1, hb = ab >> 1;
+                    const int mh = 2 * m - 1 + hb - ha, t = mh - lv.mh_start;
+                    if (mh < 1 || t < 0 || t >= lv.nmh) continue;
+                    const int h0 = 2 * r + ha;
+                    if (pp[(h0 + mh) << lhq] - pp[h0 << lhq] >= (double)__ldg(tau_g + lv.tauh_off + t) * (1.0 - 1e-6)) confirmed = true;
+                }
+            }
+            const bool any = __any_sync(0xffffffffu, confirmed);
+            __syncwarp();
+            if (!any) continue;
         }
         PowerSource::Row src(src_pw, row);
         // ---- prefix sum in double: stage the span (coalesced loads, several in flight), then each lane scans its own

@@ -313,6 +313,23 @@ int derive(pulscan_plan& p) {
     sp.ntasks = task;
     for (int lg = 0; lg < 8; ++lg) sp.off_lg[lg] = -1;
     for (int a = 0; a < sp.narr; ++a) sp.off_lg[sp.arr_lg[a]] = sp.arr_off[a];
+    // τ_h tables: thresholds of covers of mh half-groups (g/2 bins), per level with g ≥ 8: the refine kernel's second look
+    for (int l = 0; l < sp.nlevels; ++l) {
+        SweepLevel& lv = sp.lv[l];
+        lv.tauh_off = 0; lv.mh_start = 0; lv.nmh = 0;
+        if (lv.lg < 3 || lv.nsteps == 0 || std::getenv("PULSCAN_NO_CONFIRM") != nullptr) continue;
+        const int gh = 1 << (lv.lg - 1);
+        lv.mh_start = std::max(0, 2 * lv.m_start - 2);
+        const int mh_end = 2 * (lv.m_start + 4 * lv.nsteps - 1);
+        lv.nmh = mh_end - lv.mh_start + 1;
+        lv.tauh_off = (int)p.tau.size();
+        for (int mh = lv.mh_start; mh <= mh_end; ++mh) {
+            const int wmin = (mh <= 1) ? 1 : (mh - 2) * gh + 2, wtop = std::min(lv.whi, mh * gh);
+            double tmin = INFINITY;
+            for (int wq = std::max(lv.wlo, wmin); wq <= wtop; ++wq) tmin = std::min(tmin, p.T[wq - 1]);
+            p.tau.push_back(std::isfinite(tmin) && mh >= 1 ? conservative_threshold(tmin, mh * gh) : INFINITY);
+        }
+    }
     p.sweep_fine = false;
     for (int a = 0; a < sp.narr; ++a) p.sweep_fine = p.sweep_fine || sp.arr_lg[a] < 2;
     // Does the float32 power of every bin have to exist in HBM?  Not on the default path: kernel (a) then leaves only the sums
@@ -665,7 +682,7 @@ int enqueue_sweep_exact(pulscan_plan& p, const float* d_in, const PowerSource& s
                                                                              d_counters);
         CUDA_TRY(cudaGetLastError());
         if ((rc = debug_sync("boxcar_sweep_kernel"))) return rc;
-        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, src, p.n, p.tiles_per_row, p.C,
+        sweep_refine_kernel<<<p.refine_grid, kRefineThreads, p.smem_refine, st>>>(p.sp, src, from_g ? d_in : nullptr, p.pitchG, p.n, p.tiles_per_row, p.C,
                                                                                   p.nblk, p.d_tau, p.d_Tp, d_cells, p.cell_cap,
                                                                                   d_bitmap, d_flagged, d_counters);
     } else {
@@ -831,8 +848,8 @@ int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_
     if (!plan) return fail(PULSCAN_EINVAL, "null plan");
     if (tile_bins != 0 && (tile_bins < 1024 || tile_bins > 16384 || tile_bins % 512 != 0))
         return fail(PULSCAN_EINVAL, "tile_bins must be 0 or a multiple of 512 in [1024, 16384]");
-    if (log10_p_flag != 0.0 && !(log10_p_flag <= -2.0 && log10_p_flag >= -9.0))
-        return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -2]");
+    if (log10_p_flag != 0.0 && !(log10_p_flag <= -1.0 && log10_p_flag >= -9.0))
+        return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -1]");
     plan->tile_user = tile_bins;
     plan->log10_p_flag = (log10_p_flag == 0.0) ? -3.0 : log10_p_flag;
     invalidate(*plan);

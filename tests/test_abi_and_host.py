@@ -66,7 +66,7 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_pitch(p.handle, 9999) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_mode(p.handle, 7) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_tuning(p.handle, 1000, 0.0) == binding.PULSCAN_EINVAL
-    assert lib.pulscan_plan_set_tuning(p.handle, 2048, -1.0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_tuning(p.handle, 2048, -0.5) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_width_sampling(p.handle, 0, 0) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_normalisation(p.handle, 2) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_norm_block(p.handle, 3000) == binding.PULSCAN_OK
