@@ -335,7 +335,7 @@ def run_ours(args):
             "data": "synthetic", "config": config_dict(wl, world, args), "bin_widths_per_sec": value * wl.zmax,
             "latency_us_per_search": ms_step * 1e3 if n_copies > 1 else None,
             "candidates_per_step": n_cand, "blocks_flagged_by_sweep": flagged,
-            "sweep_cells_refined": int(stats[2]), "norm_blocks_redone": int(stats[1]), "clocks": clk.summary(),
+            "sweep_cells_refined": int(stats[2]), "sweep_cells_flagged": int(stats[9]), "norm_blocks_redone": int(stats[1]), "clocks": clk.summary(),
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
         }
         print(json.dumps(out), flush=True)

@@ -209,9 +209,11 @@ int64_t pulscan_plan_group_pitch(const pulscan_plan* plan);
  * (zmax doubles).  describe: a human-readable dump of the plan (levels of the pruned sweep, sizes); returns the
  * number of bytes needed including the terminator.  stats: after the stream has been synchronised, h_stats[0] =
  * candidate blocks flagged by the sweep in the last search, h_stats[1] = normalisation blocks the fast kernel handed
- * to the general path, h_stats[2] = cover cells the sweep flagged for its refine kernel, h_stats[3] = cells dropped because the list was full (their tiles' blocks are all marked),
+ * to the general path, h_stats[2] = cover cells the sweep listed for its refine kernel (after its own second look),
+ * h_stats[3] = cells dropped because the list was full (their tiles' blocks are all marked),
  * h_stats[4..8] = why blocks were handed over (geometry, search window, list capacity, verification,
- * degenerate sample), h_stats[9..15] reserved.  h_stats must hold 16 values. */
+ * degenerate sample), h_stats[9] = cover cells flagged by the sweep's cover sums before its second look,
+ * h_stats[10..15] reserved.  h_stats must hold 16 values. */
 int pulscan_plan_get_thresholds(const pulscan_plan* plan, double* h_T);
 int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf_bytes);
 int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_stream);

@@ -40,8 +40,8 @@ namespace pulscan {
 constexpr int kMaxLevels = 8;
 constexpr int kSweepThreads = 256;
 constexpr int kSweepR = 8;                 // consecutive group starts per thread
-constexpr int kScanPer = 20;               // floats per thread per scan pass: 80-byte lane stride is bank-conflict-free
-constexpr int kScanPass = kScanPer * kSweepThreads;
+constexpr int kScanTail = 48;              // zeros kept after a landing buffer's len powers (12 after its len/4 group sums): the
+                                           // last scanning thread's run of ≤ 11 quads may start before len and end after it
 #ifndef PULSCAN_SWEEP_BUFS
 #define PULSCAN_SWEEP_BUFS 2
 #endif
@@ -59,8 +59,9 @@ struct SweepLevel {
     int wlo, whi;  // widths this level answers for
     int m_lo;      // smallest number of groups a cover of a width-wlo window has
     int m_hi;      // largest number of groups a cover of a width-whi window has
-    int m_start;   // m_lo rounded down to a multiple of 4 (16-byte alignment of the sliding window's vector loads)
-    int nsteps;    // 4-wide steps over m: m_start + 4·nsteps > m_hi; ≤ 33; τ = +inf below m_lo and above m_hi
+    int m_start;   // first cover length of the first step: ≡ 0 or 1 (mod 4), ≤ m_lo (the sliding window's vector loads start at
+                   // m_start rounded down to a multiple of 4, and its 12 entries reach one length further, see sweep_step)
+    int nsteps;    // 4-wide steps over m: m_start + 4·nsteps > m_hi; ≤ 32; τ = +inf below m_lo and above m_hi
     int tau_off;   // offset of τ[m_start ..] in the τ table (4·nsteps entries)
     int pg_off;    // offset (floats) of this level's decimated prefix array PG[k] = PP[k·g] in shared memory
     int nk;        // group starts per tile = tile / g
@@ -83,8 +84,9 @@ struct SweepParams {
     int arr_lg[kMaxLevels];
     int arr_off[kMaxLevels];
     int off_lg[8];   // offset of the array with group size 2^lg, lg = 0..7; −1 if no level uses it
-    int npass;       // scan passes per tile = ceil(len / kScanPass)
-    int z_floats;    // floats of ONE landing buffer: len + kScanPer zeros (len/4 + kScanPer/4 for group-sum input), rounded up to 4
+    int scan_nq;     // quads per thread per scan pass (5, 9 or 11: the kernel's NQ); a pass covers 4·NQ·256 bins
+    int npass;       // scan passes per tile = ceil(len / (4·NQ·256)): 1 when NQ = 9 or 11
+    int z_floats;    // floats of ONE landing buffer: len + kScanTail zeros (len/4 + kScanTail/4 for group-sum input)
     int smem_floats; // two landing buffers + decimated arrays
     int ref_span;    // longest span of bins a listed cell covers (sweep_refine_kernel's shared memory per warp)
     int tp_monotone; // T'_w is finite and non-decreasing in w (every width searched, exact significance)
@@ -137,45 +139,40 @@ __device__ __forceinline__ void load_tile(float* sP, const float* __restrict__ P
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Quad-sum scan.  raw[i] = P[t0+i] for i < len and 0 for len ≤ i < len + kScanPer.  Each thread owns kScanPer = 20
-// consecutive powers (80-byte lane stride: conflict-free 16-byte loads) = 5 quads, so PP at the multiples of 4 it owns,
-// PP[4(u+q)] with u = i0/4 + 1, q = 0..4, are its running quad sums plus the scanned offset, and the multiples of g
-// among them follow a fixed pattern: the decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg], lg ≥ 2, are
-// written straight from registers.  Entries past len >> lg (written by the thread that straddles len, inside the kPadG
-// pad) equal PP[len] because of the zeros after len; the other pad entries only ever meet τ = +inf and are zeroed once
-// per kernel.  After the first barrier of the last pass nobody reads `raw` any more (`after_loads` runs there: the next
-// TMA copy into this buffer).  Returns PP[len] in every thread.  Ends with a CTA barrier; the barrier inside a pass
-// also orders the previous tile's cover sums before this tile's writes to the arrays.
+// Quad-sum scan.  raw[i] = P[t0+i] for i < len and 0 for len ≤ i < len + kScanTail.  Each thread owns NQ consecutive quads
+// (4·NQ powers; NQ odd: 16·NQ-byte lane stride = conflict-free 16-byte loads, 4·NQ bytes for group sums), so PP at the
+// multiples of 4 it owns, PP[4(u+q)] with u = i0/4 + 1, q = 0..NQ−1, are its running quad sums plus the scanned offset,
+// and the multiples of g among them follow a fixed pattern: the decimated arrays PG_lg[k] = PP[k << lg], k ∈ [0, len >> lg],
+// lg ≥ 2, are written straight from registers.  NQ = 9 or 11 scans a whole tile + halo in ONE pass (≤ 9216 / 11264 bins:
+// two CTA barriers per tile instead of four and no half-idle second pass); NQ = 5 takes as many passes as the tile needs.
+// Entries past len >> lg (written by the thread that straddles len, inside the kPadG pad) equal PP[len] because of the
+// zeros after len; the other pad entries only ever meet τ = +inf and are zeroed once per kernel.  After the first barrier
+// of the last pass nobody reads `raw` any more (`after_loads` runs there: the next TMA copy into this buffer).  Returns
+// PP[len] in every thread.  Ends with a CTA barrier; the barrier inside a pass also orders the previous tile's cover sums
+// before this tile's writes to the arrays.
 struct ScanSmem {
     alignas(16) float wtot[kSweepThreads / 32 + 4];   // warp totals; [8] = the running total carried into the next pass
 };
 
-__device__ __forceinline__ float scan_sel5(const float (&s)[5], int q) {
-    float v = s[4];
-    v = (q == 3) ? s[3] : v;
-    v = (q == 2) ? s[2] : v;
-    v = (q == 1) ? s[1] : v;
-    v = (q == 0) ? s[0] : v;
-    return v;
-}
-
-// The entries of the decimated array PG_LG (PG[k] = PP[k << LG]) among a thread's five prefix values s[q] = PP[4(u + q)].
-template <int LG>
-__device__ __forceinline__ void scan_put(float* __restrict__ dst, int u, const float (&s)[5]) {
-    if (LG == 2) {
+// The entries of the decimated array PG_LG (PG[k] = PP[k << LG]) among a thread's prefix values s[q] = PP[4(u + q)]: those
+// with u + q ≡ 0 (mod 2^(LG−2)), i.e. q = q0, q0 + M, … with q0 = −u mod M; each is picked from its M candidates by selects.
+template <int LG, int NQ>
+__device__ __forceinline__ void scan_put(float* __restrict__ dst, int u, const float (&s)[NQ]) {
+    if constexpr (LG == 2) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) dst[u + q] = s[q];
-    } else if (LG == 3) {
-        const bool odd = u & 1;                                 // hits q = odd, odd+2 (and 4 when even)
-        float* d = dst + ((u + 1) >> 1);
-        d[0] = odd ? s[1] : s[0];
-        d[1] = odd ? s[3] : s[2];
-        if (!odd) d[2] = s[4];
+        for (int q = 0; q < NQ; ++q) dst[u + q] = s[q];
     } else {
-        constexpr int sh = LG - 2;
-        const int q0 = (-u) & ((1 << sh) - 1);
-        if (q0 < 5) dst[(u + q0) >> sh] = scan_sel5(s, q0);
-        if (LG == 4 && q0 == 0) dst[(u + 4) >> 2] = s[4];
+        constexpr int sh = LG - 2, M = 1 << sh;
+        const int q0 = (-u) & (M - 1);
+        float* d = dst + ((u + q0) >> sh);
+#pragma unroll
+        for (int j = 0; j * M < NQ; ++j) {
+            float v = s[j * M];
+#pragma unroll
+            for (int t = 1; t < M && j * M + t < NQ; ++t) v = (q0 == t) ? s[j * M + t] : v;
+            if (j * M + M - 1 < NQ) d[j] = v;                    // every q0 lands inside the thread's run
+            else if (j * M + q0 < NQ) d[j] = v;
+        }
     }
 }
 
@@ -183,29 +180,31 @@ __device__ __forceinline__ void scan_put(float* __restrict__ dst, int u, const f
 // with g = 1 and g = 2 (PG0 = PP itself, PG1): needed when a level's covers must be finer than 4 bins — harmonic-summed
 // spectra, whose noise level per bin is H(H+1)/2, and very low σ thresholds.
 // FROMG = true: `raw` holds the tile's group sums G[k] = P[4k] + … + P[4k+3] (written by kernel (a), norm_power.cuh)
-// instead of the powers: a thread's five quad sums are five loads (20-byte lane stride: conflict-free).
-template <bool FINE, bool FROMG, class AfterLoads>
+// instead of the powers: a thread's NQ quad sums are NQ loads.
+template <bool FINE, bool FROMG, int NQ, class AfterLoads>
 __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* raw, float* sG, ScanSmem& ss,
                                            AfterLoads after_loads) {
     static_assert(!(FINE && FROMG), "levels finer than four bins need the powers themselves");
+    static_assert(NQ % 2 == 1 && NQ <= kScanTail / 4, "odd lane stride; zeros after the landing buffer");
+    constexpr int kPer = 4 * NQ, kPass = kPer * kSweepThreads;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int len = sp.len;
     float carry = 0.f;
     for (int pass = 0; pass < sp.npass; ++pass) {
-        const int i0 = pass * kScanPass + kScanPer * tid;
+        const int i0 = pass * kPass + kPer * tid;
         const bool act = i0 < len;
-        float s[5];
-        float x[FINE ? 15 : 1];
+        float s[NQ];
+        float x[FINE ? 3 * NQ : 1];
         if (act && FROMG) {
             const float* gq = raw + (i0 >> 2);
 #pragma unroll
-            for (int q = 0; q < 5; ++q) s[q] = gq[q];
+            for (int q = 0; q < NQ; ++q) s[q] = gq[q];
 #pragma unroll
-            for (int q = 1; q < 5; ++q) s[q] += s[q - 1];
+            for (int q = 1; q < NQ; ++q) s[q] += s[q - 1];
         } else if (act) {
             const float4* zq = reinterpret_cast<const float4*>(raw) + (i0 >> 2);
 #pragma unroll
-            for (int q = 0; q < 5; ++q) {
+            for (int q = 0; q < NQ; ++q) {
                 const float4 v = zq[q];
                 if (FINE) {
                     x[3 * q] = v.x; x[3 * q + 1] = v.x + v.y; x[3 * q + 2] = x[3 * q + 1] + v.z;
@@ -215,18 +214,18 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
                 }
             }
 #pragma unroll
-            for (int q = 1; q < 5; ++q) s[q] += s[q - 1];
+            for (int q = 1; q < NQ; ++q) s[q] += s[q - 1];
         } else {
 #pragma unroll
-            for (int q = 0; q < 5; ++q) s[q] = 0.f;
+            for (int q = 0; q < NQ; ++q) s[q] = 0.f;
         }
-        float incl = s[4];
+        float incl = s[NQ - 1];
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
             const float t = __shfl_up_sync(0xffffffffu, incl, off);
             if (lane >= off) incl += t;
         }
-        const float excl = incl - s[4];
+        const float excl = incl - s[NQ - 1];
         if (lane == 31) ss.wtot[warp] = incl;
         __syncthreads();
         if (pass == sp.npass - 1) after_loads();
@@ -238,48 +237,51 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
         if (act) {
             const float off = carry + (wbase + excl);
 #pragma unroll
-            for (int q = 0; q < 5; ++q) s[q] += off;            // s[q] = PP[4(u+q)]
+            for (int q = 0; q < NQ; ++q) s[q] += off;           // s[q] = PP[4(u+q)]
             const int u = (i0 >> 2) + 1;
             if (FINE) {                                         // x[3q+t] = PP[i0 + 4q + t + 1], t = 0..2
 #pragma unroll
-                for (int q = 0; q < 5; ++q) {
+                for (int q = 0; q < NQ; ++q) {
                     const float oq = q ? s[q - 1] : off;
                     x[3 * q] += oq; x[3 * q + 1] += oq; x[3 * q + 2] += oq;
                 }
-                if (sp.off_lg[0] >= 0) {                        // PG0[i] = PP[i]: entries i0+1 … i0+20 (the pad holds 16)
+                if (sp.off_lg[0] >= 0) {                        // PG0[i] = PP[i]: entries i0+1 … i0+4·NQ (the pad holds 16)
                     float* dst = sG + sp.off_lg[0];
 #pragma unroll
-                    for (int q = 0; q < 5; ++q) {
+                    for (int q = 0; q < NQ; ++q) {
                         float* d = dst + i0 + 4 * q + 1;
                         if (i0 + 4 * q + 4 <= len + kPadG) { d[0] = x[3 * q]; d[1] = x[3 * q + 1]; d[2] = x[3 * q + 2]; d[3] = s[q]; }
                     }
                 }
-                if (sp.off_lg[1] >= 0) {                        // PG1[k] = PP[2k]: entries i0/2+1 … i0/2+10
+                if (sp.off_lg[1] >= 0) {                        // PG1[k] = PP[2k]: entries i0/2+1 … i0/2+2·NQ
                     float* dst = sG + sp.off_lg[1];
 #pragma unroll
-                    for (int q = 0; q < 5; ++q) { dst[(i0 >> 1) + 2 * q + 1] = x[3 * q + 1]; dst[(i0 >> 1) + 2 * q + 2] = s[q]; }
+                    for (int q = 0; q < NQ; ++q) { dst[(i0 >> 1) + 2 * q + 1] = x[3 * q + 1]; dst[(i0 >> 1) + 2 * q + 2] = s[q]; }
                 }
             }
             // one store sequence per group size, the group size a compile-time constant in each (the branches are uniform)
-            if (sp.off_lg[2] >= 0) scan_put<2>(sG + sp.off_lg[2], u, s);
-            if (sp.off_lg[3] >= 0) scan_put<3>(sG + sp.off_lg[3], u, s);
-            if (sp.off_lg[4] >= 0) scan_put<4>(sG + sp.off_lg[4], u, s);
-            if (sp.off_lg[5] >= 0) scan_put<5>(sG + sp.off_lg[5], u, s);
-            if (sp.off_lg[6] >= 0) scan_put<6>(sG + sp.off_lg[6], u, s);
-            if (sp.off_lg[7] >= 0) scan_put<7>(sG + sp.off_lg[7], u, s);
+            if (sp.off_lg[2] >= 0) scan_put<2, NQ>(sG + sp.off_lg[2], u, s);
+            if (sp.off_lg[3] >= 0) scan_put<3, NQ>(sG + sp.off_lg[3], u, s);
+            if (sp.off_lg[4] >= 0) scan_put<4, NQ>(sG + sp.off_lg[4], u, s);
+            if (sp.off_lg[5] >= 0) scan_put<5, NQ>(sG + sp.off_lg[5], u, s);
+            if (sp.off_lg[6] >= 0) scan_put<6, NQ>(sG + sp.off_lg[6], u, s);
+            if (sp.off_lg[7] >= 0) scan_put<7, NQ>(sG + sp.off_lg[7], u, s);
         }
         // PP at the end of this pass = the last thread's running total: the carry of the next pass and, after the last pass,
         // PP[len] (the bound of every entry, which the caller's slack is scaled by)
-        if (tid == kSweepThreads - 1) ss.wtot[kSweepThreads / 32] = act ? s[4] : carry + (wbase + excl);
+        if (tid == kSweepThreads - 1) ss.wtot[kSweepThreads / 32] = act ? s[NQ - 1] : carry + (wbase + excl);
         __syncthreads();
         carry = ss.wtot[kSweepThreads / 32];
     }
     return carry;
 }
 
-// One 4-wide step over m for 8 group starts.  O is the rotation of the 12-entry window W (compile time, so that the
-// window never moves between registers): W[(O + j) % 12] = PG[k0b + m + j], j = 0..11 after the load below.
-template <int O>
+// One 4-wide step over m for 8 group starts.  O is the rotation of the 12-entry window W (compile time, so that the window
+// never moves between registers): W[(O + j) % 12] = PG[k0b + m_base + 4·step + j], j = 0..11 after the load below, where
+// m_base = m_start − D is a multiple of 4 (16-byte alignment of the vector loads) and D ∈ {0, 1}: the step's cover lengths
+// are m_start + 4·step + q, q = 0..3, whose ends are the entries D + q + r ≤ 11.  D = 1 lets a level start at m ≡ 1 (mod 4)
+// without a dead cover length: the levels with 4-bin groups start at m = 1 and are the most expensive per step.
+template <int O, int D>
 __device__ __forceinline__ bool sweep_step(const float (&A)[kSweepR], float (&W)[12], const float* __restrict__ pg_next,
                                            const float* __restrict__ tau4) {
     const float4 nw = *reinterpret_cast<const float4*>(pg_next);
@@ -291,7 +293,7 @@ __device__ __forceinline__ bool sweep_step(const float (&A)[kSweepR], float (&W)
     for (int q = 0; q < 4; ++q) {
         float u[kSweepR];
 #pragma unroll
-        for (int r = 0; r < kSweepR; ++r) u[r] = W[(O + q + r) % 12] - A[r];
+        for (int r = 0; r < kSweepR; ++r) u[r] = W[(O + D + q + r) % 12] - A[r];
         const float m0 = fmaxf(fmaxf(u[0], u[1]), u[2]);
         const float m1 = fmaxf(fmaxf(u[3], u[4]), u[5]);
         const float m2 = fmaxf(fmaxf(u[6], u[7]), m0);
@@ -302,29 +304,66 @@ __device__ __forceinline__ bool sweep_step(const float (&A)[kSweepR], float (&W)
 
 // All covers of one level for 8 consecutive group starts k0b..k0b+7: returns the bit mask of the 4-wide m steps in
 // which some cover reached its threshold (slack already folded into A).
-__device__ __forceinline__ unsigned sweep_task(const float* __restrict__ PG, int k0b, int m_start, int nsteps,
-                                               const float* __restrict__ tau, float slack) {
+template <int D>
+__device__ __forceinline__ unsigned sweep_task_d(const float* __restrict__ PG, int k0b, int m_base, int nsteps,
+                                                 const float* __restrict__ tau, float slack) {
     float A[kSweepR], W[12];
     {
         const float4 a0 = *reinterpret_cast<const float4*>(PG + k0b);
         const float4 a1 = *reinterpret_cast<const float4*>(PG + k0b + 4);
         A[0] = a0.x - slack; A[1] = a0.y - slack; A[2] = a0.z - slack; A[3] = a0.w - slack;
         A[4] = a1.x - slack; A[5] = a1.y - slack; A[6] = a1.z - slack; A[7] = a1.w - slack;
-        const float* p = PG + k0b + m_start;
+        const float* p = PG + k0b + m_base;
         const float4 w0 = *reinterpret_cast<const float4*>(p);
         const float4 w1 = *reinterpret_cast<const float4*>(p + 4);
         W[0] = w0.x; W[1] = w0.y; W[2] = w0.z; W[3] = w0.w; W[4] = w1.x; W[5] = w1.y; W[6] = w1.z; W[7] = w1.w;
         W[8] = W[9] = W[10] = W[11] = 0.f;
     }
     unsigned mask = 0;
-    const float* p = PG + k0b + m_start + 8;
+    const float* p = PG + k0b + m_base + 8;
     for (int s = 0; s < nsteps; s += 3) {
-        if (sweep_step<0>(A, W, p, tau)) mask |= 1u << s;
-        if (s + 1 < nsteps && sweep_step<4>(A, W, p + 4, tau + 4)) mask |= 2u << s;
-        if (s + 2 < nsteps && sweep_step<8>(A, W, p + 8, tau + 8)) mask |= 4u << s;
+        if (sweep_step<0, D>(A, W, p, tau)) mask |= 1u << s;
+        if (s + 1 < nsteps && sweep_step<4, D>(A, W, p + 4, tau + 4)) mask |= 2u << s;
+        if (s + 2 < nsteps && sweep_step<8, D>(A, W, p + 8, tau + 8)) mask |= 4u << s;
         p += 12; tau += 12;
     }
     return mask;
+}
+
+__device__ __forceinline__ unsigned sweep_task(const float* __restrict__ PG, int k0b, int m_start, int nsteps,
+                                               const float* __restrict__ tau, float slack) {
+    return (m_start & 1) ? sweep_task_d<1>(PG, k0b, m_start - 1, nsteps, tau, slack)     // warp-uniform
+                         : sweep_task_d<0>(PG, k0b, m_start, nsteps, tau, slack);
+}
+
+// Second look at a flagged cell before it is listed, by the whole warp (lane = 8·q + r looks at cover length m4 + q from group
+// start k0b + r: the refine kernel's layout, and the same test as its look from the group sums, here on the tile's float32
+// prefix arrays with the slack on the keeping side).  A window that reaches its T_w is covered by m groups of g bins and by
+// mh = 2m − 1 + b − a half-groups of g/2 bins (start in half a of the first group, end in half b of the last); the half-cover
+// is only g − 2 bins longer than its narrowest window, so its threshold τ_h[mh] rejects most of the noise flags that live off
+// the 2g − 2 bins of slack of the full cover (cfg 3: 9 of 10 cells).  Needs the array PG_{lg−1} in shared memory (a level of
+// that group size exists) and the level's τ_h table; otherwise the cell is kept.  Returns the same value in every lane.
+__device__ __forceinline__ bool sweep_confirm_cell(const SweepParams& sp, const SweepLevel& lv, const float* __restrict__ sG,
+                                                   const float* __restrict__ sTau, int k0b, int st, float slack) {
+    if (lv.lg < 3 || lv.nmh <= 0) return true;
+    const int offh = sp.off_lg[lv.lg - 1];
+    if (offh < 0) return true;
+    const int lane = threadIdx.x & 31;
+    const float* PG = sG + lv.pg_off;
+    const float* PH = sG + offh;
+    const int q = lane >> 3, k = k0b + (lane & 7), m = lv.m_start + 4 * st + q;
+    bool ok = false;
+    if (PG[k + m] - (PG[k] - slack) >= sTau[lv.tau_off + 4 * st + q]) {
+#pragma unroll
+        for (int ab = 0; ab < 4; ++ab) {
+            const int ha = ab & 1, hb = ab >> 1;
+            const int mh = 2 * m - 1 + hb - ha, tt = mh - lv.mh_start;
+            if (mh < 1 || tt < 0 || tt >= lv.nmh) continue;
+            const int h0 = 2 * k + ha;
+            if (PH[h0 + mh] - (PH[h0] - slack) >= sTau[lv.tauh_off + tt]) ok = true;
+        }
+    }
+    return __any_sync(0xffffffffu, ok);
 }
 
 // Append the tile's marked candidate blocks to the global list, once each (bitmap test-and-set).
@@ -405,11 +444,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
 // Streaming filter, persistent: gridDim.x CTAs (a multiple of the SM count) stride over the n_items = tiles_per_row ·
 // batch tiles.  Two landing buffers: a tile's copy is issued as soon as the previous user of its buffer has read its
 // powers into registers, i.e. a whole tile ahead.  Two CTA barriers per tile (both inside the scan).
-// counters[2] = cells appended (the refine kernel's work count), counters[3] = cells dropped because the list was full
+// counters[2] = cells appended (the refine kernel's work count), counters[9] = cells flagged before the second look
+// (sweep_confirm_cell), counters[3] = cells dropped because the list was full
 // (their tile's blocks are all marked instead, which is always allowed: kernel (c) decides).
 // Dynamic shared memory: [kSweepBufs × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
 // FROMG = true: P / pitchP are the group-sum array G and its pitch (see scan_tile).
-template <bool FINE, bool FROMG>
+template <bool FINE, bool FROMG, int NQ>
 __global__ void __launch_bounds__(kSweepThreads, PULSCAN_SWEEP_OCC)
 boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restrict__ P, long long pitchP, long long n,
                     int tiles_per_row, long long n_items, int C, long long nblk, const float* __restrict__ tau_g,
@@ -426,9 +466,9 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
     // ---- once per CTA: τ table, zeros after len and in the arrays (PG[0] = 0, pads), task list, the first two copies
     for (int i = tid; i < sp.ntau; i += kSweepThreads) sTau[i] = tau_g[i];
     for (int i = tid; i < sp.smem_floats - kSweepBufs * sp.z_floats; i += kSweepThreads) sG[i] = 0.f;
-    if (tid < kSweepBufs * kScanPer) {   // zeros after the copied elements (a thread's five quads may start before and end after them)
-        const int pos = (FROMG ? (sp.len >> 2) : sp.len) + tid % kScanPer;
-        if (pos < sp.z_floats) raw0[(tid / kScanPer) * sp.z_floats + pos] = 0.f;
+    {   // zeros after the copied elements (a thread's run of quads may start before and end after them)
+        const int first = FROMG ? (sp.len >> 2) : sp.len, ntail = sp.z_floats - first;
+        for (int i = tid; i < kSweepBufs * ntail; i += kSweepThreads) raw0[(i / ntail) * sp.z_floats + first + i % ntail] = 0.f;
     }
     for (int q = tid; q < sp.ntasks; q += kSweepThreads) {
         int L = 0;
@@ -466,7 +506,7 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             for (int i = first + tid; i < end; i += kSweepThreads) raw[i] = 0.f;
             __syncthreads();
         }
-        const float pp_max = scan_tile<FINE, FROMG>(sp, raw, sG, ctl.scan, [&] {
+        const float pp_max = scan_tile<FINE, FROMG, NQ>(sp, raw, sG, ctl.scan, [&] {
             const long long nxt = item + kSweepBufs * stride;
             if (tid == 0 && nxt < n_items) sweep_issue_tile<FROMG>(sp, nxt, P, pitchP, tiles_per_row, raw, &ctl.mbar[b]);
         });
@@ -477,19 +517,28 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             const int4 ta = *reinterpret_cast<const int4*>(&ctl.task[q]);            // pg_off, tau_off, m_start, nsteps
             const int4 tb = *reinterpret_cast<const int4*>(&ctl.task[q].level);      // level, kbase, nk
             const int k0b = tb.y + lane * kSweepR;
-            if (k0b < tb.z) {
-                unsigned mask = sweep_task(sG + ta.x, k0b, ta.z, ta.w, sTau + ta.y, slack);
-                while (mask) {
-                    const int st = __ffs(mask) - 1;
-                    mask &= mask - 1;
-                    const unsigned pos = atomicAdd(counters + 2, 1u);
-                    if (pos < cell_cap) {
-                        cells[pos] = SweepCell{(unsigned)item, ((unsigned)tb.x << 28) | ((unsigned)st << 20) | (unsigned)(k0b >> 3)};
-                    } else {                                     // list full: mark every block the tile's start bins touch
-                        atomicAdd(counters + 3, 1u);
-                        const long long t0 = (long long)tix * sp.tile;
-                        const long long last = min(t0 + sp.tile - 1, n - 1);
-                        for (long long c = t0 / C; c <= last / C; ++c) mark_block((unsigned long long)(row * nblk + c), bitmap, flagged, counters);
+            const unsigned mask = (k0b < tb.z) ? sweep_task(sG + ta.x, k0b, ta.z, ta.w, sTau + ta.y, slack) : 0u;
+            unsigned lanes = __ballot_sync(0xffffffffu, mask != 0u);     // rare: 1.3 cells per tile in noise
+            while (lanes) {
+                const int src = __ffs(lanes) - 1;
+                lanes &= lanes - 1;
+                unsigned ms = __shfl_sync(0xffffffffu, mask, src);
+                const int kc = tb.y + src * kSweepR;
+                while (ms) {
+                    const int st = __ffs(ms) - 1;
+                    ms &= ms - 1;
+                    const bool keep = sweep_confirm_cell(sp, sp.lv[tb.x], sG, sTau, kc, st, slack);
+                    if (lane == 0) {
+                        atomicAdd(counters + 9, 1u);             // cells flagged by the cover sums, before the second look
+                        const unsigned pos = keep ? atomicAdd(counters + 2, 1u) : 0u;
+                        if (keep && pos < cell_cap) {
+                            cells[pos] = SweepCell{(unsigned)item, ((unsigned)tb.x << 28) | ((unsigned)st << 20) | (unsigned)(kc >> 3)};
+                        } else if (keep) {                       // list full: mark every block the tile's start bins touch
+                            atomicAdd(counters + 3, 1u);
+                            const long long t0 = (long long)tix * sp.tile;
+                            const long long last = min(t0 + sp.tile - 1, n - 1);
+                            for (long long c = t0 / C; c <= last / C; ++c) mark_block((unsigned long long)(row * nblk + c), bitmap, flagged, counters);
+                        }
                     }
                 }
             }

@@ -41,6 +41,13 @@
 
 namespace pulscan {
 
+#ifdef PULSCAN_V2_TIMING
+__device__ unsigned long long g_v2_t[16];
+#define V2_TICK(k) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_v2_t[k], (unsigned long long)(now_ - tick_)); tick_ = now_; } } while (0)
+#else
+#define V2_TICK(k) do { } while (0)
+#endif
+
 constexpr int kV2NB = 2048;            // buckets per component
 constexpr int kV2KPT = 16;             // buckets per chunk
 constexpr int kV2NCH = kV2NB / kV2KPT; // chunks per component (128)
@@ -415,6 +422,9 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     const long long lo_bin = (long long)jblk * B;
     const float2* src = spectra + (long long)row * pitch_in + lo_bin;
 
+#ifdef PULSCAN_V2_TIMING
+    long long tick_ = clock64();
+#endif
     // ---- stage the block; zero the histograms meanwhile; warp 0 derives the bucket map from a sample
     const unsigned shift = (unsigned)(reinterpret_cast<uintptr_t>(src) & 15);          // 0 or 8
     const char* csrc = reinterpret_cast<const char*>(src) - shift;
@@ -470,6 +480,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         v2_estimate<B>(sdat, ctl);
     }
     __syncthreads();                                                                     // S1
+    V2_TICK(0);
     if (use_tma) v2_mbar_wait(&ctl.mbar, 0);           // already complete: makes the copied bytes visible to this thread
     bool bad = ctl.fail != 0;
 
@@ -490,6 +501,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
     }
     __syncthreads();                                                                     // S2
+    V2_TICK(1);
     // ---- chunk totals (16 buckets each), rotated 16-byte reads so that a quarter-warp touches all bank groups
     if (!bad) {
         for (int id = tid; id < 2 * kV2NCH; id += NT) {
@@ -505,8 +517,10 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
     }
     __syncthreads();                                                                     // S3
+    V2_TICK(2);
     if (!bad && warp < 2) v2_locate<B>(ctl, hist + warp * kV2NB, warp);
     __syncthreads();                                                                     // S4
+    V2_TICK(3);
     bad = bad || ctl.fail != 0;
     // ---- gather: z = ||4·(idx − ⌊c2/2⌋)| − K| − K, member ⇔ |z| ≤ HW', on fp16 pairs (exact small-integer arithmetic)
     if (!bad) {
@@ -537,8 +551,10 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
     }
     __syncthreads();                                                                     // S5
+    V2_TICK(4);
     if (!bad && warp < 2) v2_resolve<B>(ctl, warp);
     __syncthreads();                                                                     // S6
+    V2_TICK(5);
     bad = bad || ctl.fail != 0;
     if (!bad) {
         // x' = ((v − a) − h)·inv evaluated as fma(v − a, inv, −h·inv), as in the general path (norm_power.cuh)
@@ -572,6 +588,10 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
                 st[0] = a0; st[1] = i0; st[2] = k0; st[3] = a1; st[4] = i1; st[5] = k1;
             }
         }
+#ifdef PULSCAN_V2_TIMING
+        __syncthreads();
+        V2_TICK(6);
+#endif
     } else if (tid == 0) {
         redo[atomicAdd(redo_count, 1u)] = blockIdx.x;   // the general path will do this block
         atomicAdd(redo_count + 2 + min(max(ctl.fail, 1), 5), 1u);   // counters[4..8]: why (see V2Ctl::fail)

@@ -58,6 +58,11 @@ inline int pow2_ceil(int x) { int p = 1; while (p < x) p <<= 1; return p; }
 
 } // namespace
 
+// Per-cover false-flag probability of the pruned sweep in noise, log10.  Measured on a B200 with the sweep's own second look
+// in place (sweep + refine, ms): cfg 3 -3: 1.156, -3.25: 1.128, -3.5: 1.111, -3.75: 1.112, -4: 2.20 (levels finer than 4 bins);
+// cfg 4: 0.510 / 0.520 / 0.526 / 0.544 / 1.34; cfg 5: 1.876 / 1.816 / 1.771 / 1.735 / 1.780.
+constexpr double kDefaultLog10PFlag = -3.25;
+
 struct pulscan_plan {
     // user parameters
     int64_t n = 0;
@@ -80,7 +85,7 @@ struct pulscan_plan {
     int32_t r_block = 0;                     // report the candidate block's first bin instead of the exact bin (L222-226)
     int32_t z_step = 1, log_sampling = 0;   // which widths are searched (all are summed): Alg. 4
     int32_t tile_user = 0;
-    double log10_p_flag = -3.0;
+    double log10_p_flag = kDefaultLog10PFlag;
     bool host_staging = false;
     // derived (host)
     bool dirty = true;         // derived tables need (re)building
@@ -159,6 +164,9 @@ void attach_children(pulscan_plan& p) {
     }
 }
 
+// First cover length of a level's first step: the largest m ≤ m_lo with m ≡ 0 or 1 (mod 4), see sweep_step.
+int sweep_m_start(int m_lo) { return (m_lo & 3) >= 1 ? (m_lo & ~3) + 1 : m_lo; }
+
 int derive(pulscan_plan& p) {
     if (!p.dirty) return PULSCAN_OK;
     p.nblk = (p.n + p.C - 1) / p.C;
@@ -221,16 +229,16 @@ int derive(pulscan_plan& p) {
                 else { m_lo = (w + g - 1) / g; m_hi = (w2 >= 2) ? (w2 - 2) / g + 2 : 1; }
             };
             int w2 = w, m_lo = 0, m_hi = 0;
-            while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lg) {   // extend the run while the m range fits 32 steps of 4, counted
-                m_range(w2 + 1, m_lo, m_hi);                  // from m_lo rounded down to 4 (sweep_task's hit mask has 32 bits)
-                if ((m_hi - (m_lo & ~3) + 4) / 4 > 32) break;
+            while (w2 + 1 <= p.zmax && lgw[w2 + 1] == lg) {   // extend the run while the m range fits 32 steps of 4
+                m_range(w2 + 1, m_lo, m_hi);                  // (sweep_task's hit mask has 32 bits)
+                if ((m_hi - sweep_m_start(m_lo) + 4) / 4 > 32) break;
                 ++w2;
             }
             m_range(w2, m_lo, m_hi);
             if ((int)lvls.size() >= kMaxLevels) { fits = false; break; }
             SweepLevel lv{};
             lv.lg = lg; lv.wlo = w; lv.whi = w2; lv.m_lo = m_lo; lv.m_hi = m_hi;
-            lv.m_start = m_lo & ~3;
+            lv.m_start = sweep_m_start(m_lo);
             lv.nsteps = (m_hi - lv.m_start + 4) / 4;
             lv.nk = tile >> lg;
             lv.nwt = (lv.nk + 32 * kSweepR - 1) / (32 * kSweepR);
@@ -243,7 +251,7 @@ int derive(pulscan_plan& p) {
         if (fits && ntasks_all > kMaxWarpTasks) fits = false;   // too many fine levels for one tile: coarser groups
         if (fits) {   // shared memory of the two tile buffers + one decimated array per distinct group size
             const int len = tile + (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
-            size_t fl = kSweepBufs * ((size_t)len + kScanPer + 4);
+            size_t fl = kSweepBufs * ((size_t)len + kScanTail + 4);
             std::vector<int> seen;
             for (const SweepLevel& lv : lvls)
                 if (std::find(seen.begin(), seen.end(), lv.lg) == seen.end()) {
@@ -269,7 +277,6 @@ int derive(pulscan_plan& p) {
     sp.tile = tile;
     const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
     sp.len = tile + halo;
-    sp.npass = (sp.len + kScanPass - 1) / kScanPass;
     int off = 0, task = 0;
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = lvls[l];
@@ -340,7 +347,15 @@ int derive(pulscan_plan& p) {
     // normalisation blocks that are not a multiple of four bins.  PULSCAN_KEEP_P forces it (comparison runs).
     p.keep_P = p.is_child || p.mode == 1 || p.sweep_fine || p.numharm > 1 || p.norm_mode == 1 || (p.B & 3) != 0 ||
                std::getenv("PULSCAN_KEEP_P") != nullptr;
-    sp.z_floats = p.keep_P ? (int)align_up((size_t)(sp.len + kScanPer), 4) : (int)align_up((size_t)(sp.len / 4 + 8), 4);
+    sp.z_floats = p.keep_P ? (int)align_up((size_t)(sp.len + kScanTail), 4) : (int)align_up((size_t)(sp.len / 4 + kScanTail / 4), 4);
+    // quads per thread per scan pass: a whole tile + halo in one pass where it fits 9 or 11 quads per thread (the
+    // full-resolution scan keeps three more values per quad in registers and stays at 5)
+    sp.scan_nq = p.sweep_fine ? 5 : (sp.len <= 36 * kSweepThreads ? 9 : (sp.len <= 44 * kSweepThreads && !p.keep_P ? 11 : 5));
+    {
+        const char* e = std::getenv("PULSCAN_SCAN_NQ");
+        if (e && std::atoi(e) == 5) sp.scan_nq = 5;
+    }
+    sp.npass = (sp.len + 4 * sp.scan_nq * kSweepThreads - 1) / (4 * sp.scan_nq * kSweepThreads);
     if (task > kMaxWarpTasks) return fail(PULSCAN_EINVAL, "sweep tile of %d bins needs %d warp-tasks (limit %d)", tile, task, kMaxWarpTasks);
     sp.ntau = (int)p.tau.size();
     sp.smem_floats = kSweepBufs * sp.z_floats + off;
@@ -468,8 +483,10 @@ int set_kernel_attributes(const pulscan_plan& p);
 using SweepFn = void (*)(const SweepParams, const float*, long long, long long, int, long long, int, long long, const float*,
                          SweepCell*, unsigned, unsigned*, unsigned*, unsigned*);
 SweepFn sweep_function(const pulscan_plan& p) {
-    if (!p.keep_P) return boxcar_sweep_kernel<false, true>;
-    return p.sweep_fine ? boxcar_sweep_kernel<true, false> : boxcar_sweep_kernel<false, false>;
+    const int nq = p.sp.scan_nq;
+    if (!p.keep_P) return nq == 9 ? boxcar_sweep_kernel<false, true, 9> : nq == 11 ? boxcar_sweep_kernel<false, true, 11> : boxcar_sweep_kernel<false, true, 5>;
+    if (p.sweep_fine) return boxcar_sweep_kernel<true, false, 5>;
+    return nq == 9 ? boxcar_sweep_kernel<false, false, 9> : boxcar_sweep_kernel<false, false, 5>;
 }
 
 int finalize_device(pulscan_plan& p) {
@@ -533,9 +550,12 @@ void invalidate(pulscan_plan& p) {
 int set_kernel_attributes(const pulscan_plan& p) {
     (void)p;
     constexpr int kMaxDynSmem = 227 * 1024;
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, false, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, false, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<true, false, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, true, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, true, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
+    CUDA_TRY(cudaFuncSetAttribute(boxcar_sweep_kernel<false, true, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
@@ -851,7 +871,7 @@ int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_
     if (log10_p_flag != 0.0 && !(log10_p_flag <= -1.0 && log10_p_flag >= -9.0))
         return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -1]");
     plan->tile_user = tile_bins;
-    plan->log10_p_flag = (log10_p_flag == 0.0) ? -3.0 : log10_p_flag;
+    plan->log10_p_flag = (log10_p_flag == 0.0) ? kDefaultLog10PFlag : log10_p_flag;
     invalidate(*plan);
     return PULSCAN_OK;
 }
@@ -1186,3 +1206,11 @@ const char* pulscan_last_error(void) { return g_last_error.c_str(); }
 const char* pulscan_version(void) { return "pulscan-b200 0.1.0 (sm_100a)"; }
 
 } // extern "C"
+
+#ifdef PULSCAN_V2_TIMING
+extern "C" int pulscan_debug_v2_timing(unsigned long long* out, int reset) {
+    if (out) cudaMemcpyFromSymbol(out, pulscan::g_v2_t, sizeof(unsigned long long) * 16);
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(pulscan::g_v2_t, z, sizeof z); }
+    return 0;
+}
+#endif
