@@ -44,8 +44,10 @@ namespace pulscan {
 #ifdef PULSCAN_V2_TIMING
 __device__ unsigned long long g_v2_t[16];
 #define V2_TICK(k) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_v2_t[k], (unsigned long long)(now_ - tick_)); tick_ = now_; } } while (0)
+#define V2_RTICK(k) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_v2_t[k], (unsigned long long)(now_ - rt_)); rt_ = now_; } } while (0)
 #else
 #define V2_TICK(k) do { } while (0)
+#define V2_RTICK(k) do { } while (0)
 #endif
 
 constexpr int kV2NB = 2048;            // buckets per component
@@ -61,7 +63,7 @@ constexpr float kV2IdxScale = 2047.0f * 2.384185791015625e-07f;  // 2047·2⁻²
 
 struct alignas(16) V2Ctl {
     unsigned long long mbar;
-    unsigned list_n[2];
+    unsigned cls_n[2][2];             // members gathered so far: [component][0: median net, 1: shells]
     int fail;                         // 0 = ok; 1 degenerate geometry, 2 search window, 3 list capacity, 4 verification, 5 sample
     float scale[2], off[2];           // bucket map of each component
     int c2[2];                        // 2·jm + e: twice the (half-integer) bucket of the median
@@ -72,8 +74,7 @@ struct alignas(16) V2Ctl {
     float a[2], h[2], inv[2];         // median = a + h (a = lower central value, h = half the gap); 1/(√2·κ·MAD)
     alignas(16) unsigned chunk_tot[2][kV2NCH];
     alignas(16) unsigned CE[2][kV2NCH + 4];   // exclusive prefix of chunk_tot; CE[NCH] = B
-    float list[2][kV2ListCap];
-    float cls[2][2][kV2ClsCap + 4];   // [component][0: median net, 1: shell deviations], +inf padded to a multiple of 4
+    float cls[2][2][kV2ClsCap + 4];   // [component][0: median net, 1: shells (values, then deviations)], +inf padded to a multiple of 4
 };
 
 __device__ __forceinline__ unsigned v2_smem(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -301,24 +302,14 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     constexpr int kk = (B - 1) >> 1;
     constexpr bool kEven = (B & 1) == 0;
     const int lane = threadIdx.x & 31;
-    const int n = (int)ctl.list_n[c];
-    if (n > kV2ListCap) { if (lane == 0) ctl.fail = 3; return; }
-    const float scale = ctl.scale[c], off = ctl.off[c];
-    const int c2 = ctl.c2[c], t0 = ctl.t0[c], tE = ctl.tE[c], tm = ctl.tm[c];
+#ifdef PULSCAN_V2_TIMING
+    long long rt_ = clock64();
+#endif
     float* med = ctl.cls[c][0];
     float* shl = ctl.cls[c][1];
-    int nm = 0, ns = 0;
-    for (int j0 = 0; j0 < n; j0 += 32) {
-        const int j = j0 + lane;
-        const float x = j < n ? ctl.list[c][j] : 0.f;
-        const int tt = abs(2 * (int)(v2_bucket_bits(x, scale, off) & 0xFFFFu) - c2);
-        const bool is_med = j < n && tt <= tm, is_shl = j < n && tt >= t0 && tt <= tE;
-        const unsigned bm = __ballot_sync(0xffffffffu, is_med), bs = __ballot_sync(0xffffffffu, is_shl);
-        const unsigned lt = (1u << lane) - 1u;
-        if (is_med) { const int p = nm + __popc(bm & lt); if (p < kV2ClsCap) med[p] = x; }
-        if (is_shl) { const int p = ns + __popc(bs & lt); if (p < kV2ClsCap) shl[p] = x; }
-        nm += __popc(bm); ns += __popc(bs);
-    }
+    const int nm = (int)ctl.cls_n[c][0], ns = (int)ctl.cls_n[c][1];   // the gather has split the members already
+    const float scale = ctl.scale[c], off = ctl.off[c];
+    const int c2 = ctl.c2[c], t0 = ctl.t0[c], tE = ctl.tE[c];
     const int tmr = kk - (int)ctl.excl_med[c], tsr = kk - (int)ctl.n_in[c];
     if (nm != (int)ctl.n_med[c] || ns != (int)ctl.n_shl[c] ||      // the gather must deliver exactly what the histogram counted
         tmr < 0 || tsr < 0 || tmr + (kEven ? 1 : 0) >= nm || tsr + (kEven ? 1 : 0) >= ns) {
@@ -327,8 +318,10 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     }
     if (lane < 4) { med[nm + lane] = INFINITY; shl[ns + lane] = INFINITY; }
     __syncwarp();
+    V2_RTICK(8);
     float a, b;
     v2_rank_pair(med, nm, tmr, a, b);
+    V2_RTICK(9);
     if (!kEven) b = a;
     const float h = 0.5f * __fsub_rn(b, a);
     // deviations of the shell members, same arithmetic as the general path
@@ -338,6 +331,7 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     float da, db;
     v2_rank_pair(shl, ns, tsr, da, db);
     if (!kEven) db = da;
+    V2_RTICK(10);
     // ---- verification.  vb(k) = value at the boundary between buckets k−1 and k.  Every value whose bucket lies
     // strictly inside the shells deviates by at most din, every value beyond them by at least dout; the margin of
     // 0.05 bucket covers the float rounding of the map and of its inverse (|off| ≤ 64).
@@ -361,6 +355,7 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
         ctl.a[c] = a; ctl.h[c] = h;
         ctl.inv[c] = (s > 0.0 && isfinite(s)) ? (float)(0.70710678118654752440 / s) : 0.f;
     }
+    V2_RTICK(11);
 }
 
 // Stage `bytes` (multiple of 16) global → shared with one TMA bulk copy; thread 0 only.  The mbarrier must have been
@@ -461,7 +456,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(v2_smem(&ctl.mbar)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         if (use_tma) v2_tma_issue(stage, csrc, nbytes, &ctl.mbar);
-        ctl.fail = 0; ctl.list_n[0] = 0; ctl.list_n[1] = 0;
+        ctl.fail = 0; ctl.cls_n[0][0] = 0; ctl.cls_n[0][1] = 0; ctl.cls_n[1][0] = 0; ctl.cls_n[1][1] = 0;
     }
     {
         uint4* hz = reinterpret_cast<uint4*>(hist);
@@ -522,32 +517,50 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     __syncthreads();                                                                     // S4
     V2_TICK(3);
     bad = bad || ctl.fail != 0;
-    // ---- gather: z = ||4·(idx − ⌊c2/2⌋)| − K| − K, member ⇔ |z| ≤ HW', on fp16 pairs (exact small-integer arithmetic)
+    // ---- gather: z = ||4·(idx − ⌊c2/2⌋)| − K| − K, member ⇔ |z| ≤ HW', on fp16 pairs (exact small-integer arithmetic).
+    // The few hits (≈ 30 of 2·B values) are re-read, classified exactly (shell t = |2·bucket − c2|: median net t ≤ tm, MAD
+    // shells t0 ≤ t ≤ tE; for odd c2 the test above is one shell too wide and the extra hits are dropped here) and appended
+    // to their list, so that the ranking warps start from split lists.  The masks of both components are formed first and
+    // their hits are read in pairs: a thread's re-reads (L2 hits at best) overlap instead of following one another.
     if (!bad) {
         const __half2 four = __float2half2_rn(4.0f);
+        unsigned hm[2];
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             const unsigned u0 = ctl.hc2[c], u1 = ctl.hK[c], u2 = ctl.hHW[c];
             const __half2 hc2 = *reinterpret_cast<const __half2*>(&u0), Kh = *reinterpret_cast<const __half2*>(&u1),
                           HWh = *reinterpret_cast<const __half2*>(&u2);
-            unsigned hm = 0;
+            unsigned m = 0;
 #pragma unroll
             for (int q = 0; q < EPT / 2; ++q) {
                 const __half2 ih = *reinterpret_cast<const __half2*>(&idxp[c][q]);
                 const __half2 d4 = __hfma2(ih, four, hc2);
                 const __half2 u = __hsub2(__habs2(d4), Kh);
                 const __half2 z = __hsub2(__habs2(u), Kh);
-                const unsigned m = __hle2_mask(__habs2(z), HWh);
-                hm |= m & ((1u << q) | (1u << (16 + q)));
+                const unsigned mm = __hle2_mask(__habs2(z), HWh);
+                m |= mm & ((1u << q) | (1u << (16 + q)));
             }
-            while (hm) {
-                const int b = __ffs(hm) - 1;
-                hm &= hm - 1;
-                const int r = 2 * (b & 15) + (b >> 4);
-                const float val = reinterpret_cast<const float*>(sdat + tid + r * NT)[c];
-                const unsigned slot = atomicAdd(&ctl.list_n[c], 1u);
-                if (slot < (unsigned)kV2ListCap) ctl.list[c][slot] = val;
+            hm[c] = m;
+        }
+        auto hit_addr = [&](unsigned m, int c) {
+            const int b = __ffs(m) - 1;
+            return reinterpret_cast<const float*>(sdat + tid + (2 * (b & 15) + (b >> 4)) * NT) + c;
+        };
+        auto put = [&](float val, int c) {
+            const int tt = abs(2 * (int)(v2_bucket_bits(val, ctl.scale[c], ctl.off[c]) & 0xFFFFu) - ctl.c2[c]);
+            const int k = tt <= ctl.tm[c] ? 0 : (tt >= ctl.t0[c] && tt <= ctl.tE[c]) ? 1 : -1;
+            if (k >= 0) {
+                const unsigned slot = atomicAdd(&ctl.cls_n[c][k], 1u);
+                if (slot < (unsigned)kV2ClsCap) ctl.cls[c][k][slot] = val;
             }
+        };
+        while (hm[0] | hm[1]) {
+            const bool h0 = hm[0] != 0, h1 = hm[1] != 0;
+            float v0 = 0.f, v1 = 0.f;
+            if (h0) v0 = *hit_addr(hm[0], 0);
+            if (h1) v1 = *hit_addr(hm[1], 1);
+            if (h0) { put(v0, 0); hm[0] &= hm[0] - 1; }
+            if (h1) { put(v1, 1); hm[1] &= hm[1] - 1; }
         }
     }
     __syncthreads();                                                                     // S5
