@@ -628,9 +628,29 @@ sweep_refine_kernel(const __grid_constant__ SweepParams sp, const PowerSource sr
                     if (pp[(h0 + mh) << lhq] - pp[h0 << lhq] >= (double)__ldg(tau_g + lv.tauh_off + t) * (1.0 - 1e-6)) confirmed = true;
                 }
             }
-            const bool any = __any_sync(0xffffffffu, confirmed);
+            unsigned live = __ballot_sync(0xffffffffu, confirmed);
+            // Third look, wide groups only: the 4 × 4 sub-covers (g/4 starts × g/4 ends, whole group sums for g ≥ 16) of every cover
+            // that passed, against the threshold of their narrowest searched width — the test the rebuilt span would meet
+            // further down, taken here from the group sums so that a cell of noise is dropped before ≈ (m + 10)·g bins of
+            // the input spectrum are read and normalised for it.
+            if (live && lg >= 4 && sp.tp_monotone) {
+                const int lh = lg - 2, h = 1 << lh, sa = lane & 3, sb = (lane >> 2) & 3;
+                unsigned todo = live;
+                live = 0u;
+                while (todo) {
+                    const int srcl = __ffs(todo) - 1;
+                    todo &= todo - 1;
+                    const int rr = srcl & 7, mm = m4 + (srcl >> 3);
+                    const int i0 = rr << lg, e0 = (rr + mm - 1) << lg;
+                    const int fs = i0 + (sa << lh), le1 = min(e0 + ((sb + 1) << lh), valid);          // first start, one past the last end
+                    const int w_lo = max((e0 + (sb << lh)) - (fs + h - 1) + 1, max(lv.wlo, 1)), w_hi = min(le1 - fs, lv.whi);
+                    const bool sub = lane < 16 && w_lo <= w_hi &&
+                                     pp[(le1 + 3) >> 2] - pp[fs >> 2] >= (double)__ldg(Tp_g + (w_lo - 1)) * (1.0 - 1e-6);
+                    if (__any_sync(0xffffffffu, sub)) { live = 1u; break; }
+                }
+            }
             __syncwarp();
-            if (!any) continue;
+            if (!live) continue;
         }
         PowerSource::Row src(src_pw, row);
         // ---- prefix sum in double: stage the span (coalesced loads, several in flight), then each lane scans its own

@@ -399,8 +399,20 @@ constexpr size_t v2_smem_bytes() {
 // STAGED = false: nothing is staged; the histogram pass, the (rare) gather hits and the output pass read the block from
 // global memory (the second and third time out of L1/L2, where a block read microseconds earlier still is), which
 // leaves 19 KB of shared memory per CTA so that more blocks are in flight per SM to cover the warp-serial phases.
-template <int EPT, int NT, bool STAGED>
-__global__ void __launch_bounds__(NT, STAGED ? ((EPT * NT <= 4096) ? 4 : 2) : (NT == 128 ? (EPT <= 16 ? PULSCAN_NORM_OCC128_SMALL : PULSCAN_NORM_OCC128) : (EPT * NT <= 4096) ? 6 : 4))
+// KEEPIDX = false: the bucket indices are not kept in registers between the histogram pass and the gather; the gather re-reads
+// the block (L2, partly L1) and recomputes them.  More instructions and one more read pass, but the kernel fits 40 registers
+// and the SM holds 11-12 blocks instead of 8: the kernel is bound by the latency of its phases, not by their issue slots.
+#ifndef PULSCAN_NORM_OCC128_NOIDX
+#define PULSCAN_NORM_OCC128_NOIDX 11
+#endif
+template <int EPT, int NT, bool STAGED, bool KEEPIDX>
+constexpr int v2_min_ctas() {
+    if (STAGED) return (EPT * NT <= 4096) ? 4 : 2;
+    if (!KEEPIDX) return NT == 128 ? PULSCAN_NORM_OCC128_NOIDX : 6;
+    return NT == 128 ? (EPT <= 16 ? PULSCAN_NORM_OCC128_SMALL : PULSCAN_NORM_OCC128) : (EPT * NT <= 4096) ? 6 : 4;
+}
+template <int EPT, int NT, bool STAGED, bool KEEPIDX = true>
+__global__ void __launch_bounds__(NT, v2_min_ctas<EPT, NT, STAGED, KEEPIDX>())
 norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int blocks_per_row, int nb, NormOut out,
                      unsigned* __restrict__ redo, unsigned* __restrict__ redo_count,
                      const char* __restrict__ lim_lo, const char* __restrict__ lim_hi, unsigned l2_ahead) {
@@ -480,7 +492,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     bool bad = ctl.fail != 0;
 
     // ---- histogram pass: both components, bucket indices kept packed in pairs
-    unsigned idxp[2][EPT / 2];
+    unsigned idxp[2][KEEPIDX ? EPT / 2 : 1];
     if (!bad) {
         const float sc0 = ctl.scale[0], sc1 = ctl.scale[1], of0 = ctl.off[0], of1 = ctl.off[1];
         const unsigned hb0 = v2_smem(hist), hb1 = v2_smem(hist + kV2NB);
@@ -491,8 +503,10 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
             const unsigned b10 = v2_bucket_bits(z0.y, sc1, of1), b11 = v2_bucket_bits(z1.y, sc1, of1);
             v2_red_inc(hb0 + (b00 << 2)); v2_red_inc(hb0 + (b01 << 2));
             v2_red_inc(hb1 + (b10 << 2)); v2_red_inc(hb1 + (b11 << 2));
-            idxp[0][q] = __byte_perm(b00, b01, 0x5410);
-            idxp[1][q] = __byte_perm(b10, b11, 0x5410);
+            if (KEEPIDX) {
+                idxp[0][q] = __byte_perm(b00, b01, 0x5410);
+                idxp[1][q] = __byte_perm(b10, b11, 0x5410);
+            }
         }
     }
     __syncthreads();                                                                     // S2
@@ -524,23 +538,30 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     // their hits are read in pairs: a thread's re-reads (L2 hits at best) overlap instead of following one another.
     if (!bad) {
         const __half2 four = __float2half2_rn(4.0f);
-        unsigned hm[2];
+        unsigned hm[2] = {0u, 0u};
+        const unsigned u00 = ctl.hc2[0], u01 = ctl.hK[0], u02 = ctl.hHW[0], u10 = ctl.hc2[1], u11 = ctl.hK[1], u12 = ctl.hHW[1];
+        const __half2 hc2[2] = {*reinterpret_cast<const __half2*>(&u00), *reinterpret_cast<const __half2*>(&u10)};
+        const __half2 Kh[2] = {*reinterpret_cast<const __half2*>(&u01), *reinterpret_cast<const __half2*>(&u11)};
+        const __half2 HWh[2] = {*reinterpret_cast<const __half2*>(&u02), *reinterpret_cast<const __half2*>(&u12)};
+        const float sc0 = ctl.scale[0], sc1 = ctl.scale[1], of0 = ctl.off[0], of1 = ctl.off[1];
 #pragma unroll
-        for (int c = 0; c < 2; ++c) {
-            const unsigned u0 = ctl.hc2[c], u1 = ctl.hK[c], u2 = ctl.hHW[c];
-            const __half2 hc2 = *reinterpret_cast<const __half2*>(&u0), Kh = *reinterpret_cast<const __half2*>(&u1),
-                          HWh = *reinterpret_cast<const __half2*>(&u2);
-            unsigned m = 0;
-#pragma unroll
-            for (int q = 0; q < EPT / 2; ++q) {
-                const __half2 ih = *reinterpret_cast<const __half2*>(&idxp[c][q]);
-                const __half2 d4 = __hfma2(ih, four, hc2);
-                const __half2 u = __hsub2(__habs2(d4), Kh);
-                const __half2 z = __hsub2(__habs2(u), Kh);
-                const unsigned mm = __hle2_mask(__habs2(z), HWh);
-                m |= mm & ((1u << q) | (1u << (16 + q)));
+        for (int q = 0; q < EPT / 2; ++q) {
+            unsigned ip[2];
+            if (KEEPIDX) { ip[0] = idxp[0][q]; ip[1] = idxp[1][q]; }
+            else {
+                const float2 z0 = sdat[tid + (2 * q) * NT], z1 = sdat[tid + (2 * q + 1) * NT];
+                ip[0] = __byte_perm(v2_bucket_bits(z0.x, sc0, of0), v2_bucket_bits(z1.x, sc0, of0), 0x5410);
+                ip[1] = __byte_perm(v2_bucket_bits(z0.y, sc1, of1), v2_bucket_bits(z1.y, sc1, of1), 0x5410);
             }
-            hm[c] = m;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                const __half2 ih = *reinterpret_cast<const __half2*>(&ip[c]);
+                const __half2 d4 = __hfma2(ih, four, hc2[c]);
+                const __half2 u = __hsub2(__habs2(d4), Kh[c]);
+                const __half2 z = __hsub2(__habs2(u), Kh[c]);
+                const unsigned mm = __hle2_mask(__habs2(z), HWh[c]);
+                hm[c] |= mm & ((1u << q) | (1u << (16 + q)));
+            }
         }
         auto hit_addr = [&](unsigned m, int c) {
             const int b = __ffs(m) - 1;

@@ -118,6 +118,7 @@ struct pulscan_plan {
     int norm_nt = 256;         // threads per CTA of the single-histogram kernel
     unsigned norm_l2_ahead = 0; // single-histogram kernel: bulk-prefetch into L2 the block of the CTA this many launches ahead
     bool norm_staged = false;  // single-histogram kernel variant: block staged in shared memory by TMA, or read from global
+    bool norm_keepidx = true;  // single-histogram kernel keeps the bucket indices in registers for its gather (else: re-reads the block)
     bool use_fast = false;     // full blocks of exactly ept_main·256 bins go through norm_power_v2_kernel + redo list
     // workspace (device, caller-owned)
     void* ws = nullptr;
@@ -412,6 +413,14 @@ int derive(pulscan_plan& p) {
     }
 
     p.norm_staged = std::getenv("PULSCAN_NORM_STAGED") != nullptr;
+    // Bucket indices kept in registers between the histogram pass and the gather, or recomputed from a re-read of the block
+    // (40 instead of 64 registers: more blocks per SM, one more read pass).  Measured (kernel (a), ms; kept / recomputed):
+    // cfg 3 (B 4096, 128 threads, 8 -> 10 CTAs) 3.05 / 3.58; cfg 5 (B 2048) 7.53 / 8.05; cfg 4 (B 8192, 256 threads,
+    // 4 -> 6 CTAs) 0.864 / 0.830 — recomputed for blocks of 8192 bins only.  PULSCAN_NORM_NOIDX=0/1 overrides.
+    {
+        const char* e = std::getenv("PULSCAN_NORM_NOIDX");
+        p.norm_keepidx = e ? std::atoi(e) == 0 : p.B < 8192;
+    }
     // Fewer warps per CTA: the warp-serial phases keep two warps busy and idle the rest.  Measured: cfg 3 (B = 4096)
     // 256 threads 3.71 ms, 128 threads 3.41 ms; cfg 5 (B = 2048) 128 threads 9.06 ms, 64 threads 10.5 ms.
     // PULSCAN_NORM_NT256 / PULSCAN_NORM_STAGED select the earlier variants for comparison.
@@ -598,8 +607,12 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
     const char* lim_hi = lim_lo + ((size_t)(p.batch - 1) * p.pitch + p.n) * 8;
 #define PULSCAN_V2_LAUNCH(E, NT_, ST)                                                                                 \
     {                                                                                                                 \
-        norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                              \
-            spec, p.pitch, p.main_blocks_per_row, p.nb, out, redo, redo_count, lim_lo, lim_hi, p.norm_l2_ahead);      \
+        if (!ST && !p.norm_keepidx && (E) >= 16)                                                                       \
+            norm_power_v2_kernel<E, NT_, false, false><<<grid, NT_, v2_smem_bytes<E, NT_, false>(), st>>>(            \
+                spec, p.pitch, p.main_blocks_per_row, p.nb, out, redo, redo_count, lim_lo, lim_hi, p.norm_l2_ahead);  \
+        else                                                                                                          \
+            norm_power_v2_kernel<E, NT_, ST><<<grid, NT_, v2_smem_bytes<E, NT_, ST>(), st>>>(                          \
+                spec, p.pitch, p.main_blocks_per_row, p.nb, out, redo, redo_count, lim_lo, lim_hi, p.norm_l2_ahead);  \
     }
 #define PULSCAN_V2_REDO(E)                                                                                            \
     norm_power_redo_kernel<E, 256><<<kRedoGrid, 256, 0, st>>>(spec, p.pitch, p.B, p.nb, p.main_blocks_per_row, out, redo, \
