@@ -351,7 +351,7 @@ int derive(pulscan_plan& p) {
     sp.z_floats = p.keep_P ? (int)align_up((size_t)(sp.len + kScanTail), 4) : (int)align_up((size_t)(sp.len / 4 + kScanTail / 4), 4);
     // quads per thread per scan pass: a whole tile + halo in one pass where it fits 9 or 11 quads per thread (the
     // full-resolution scan keeps three more values per quad in registers and stays at 5)
-    sp.scan_nq = p.sweep_fine ? 5 : (sp.len <= 36 * kSweepThreads ? 9 : (sp.len <= 44 * kSweepThreads && !p.keep_P ? 11 : 5));
+    sp.scan_nq = (p.sweep_fine || sp.len <= 20 * kSweepThreads) ? 5 : (sp.len <= 36 * kSweepThreads ? 9 : (sp.len <= 44 * kSweepThreads && !p.keep_P ? 11 : 5));
     {
         const char* e = std::getenv("PULSCAN_SCAN_NQ");
         if (e && std::atoi(e) == 5) sp.scan_nq = 5;
@@ -468,7 +468,10 @@ int derive(pulscan_plan& p) {
         if (!c) return PULSCAN_EINVAL;
         c->is_child = true; c->shape_mult = H * (H + 1) / 2; c->numharm_tag = H; c->sigma_thr = p.sigma_thr; c->n_trials = p.n_trials;
         c->signif_mode = p.signif_mode;
-        c->z_step = p.z_step; c->log_sampling = p.log_sampling; c->tile_user = p.tile_user; c->log10_p_flag = p.log10_p_flag;
+        c->z_step = p.z_step; c->log_sampling = p.log_sampling; c->tile_user = p.tile_user;
+        // a harmonic-summed spectrum has H(H+1)/2 of noise in every bin of a cover's slack: coarser groups at a higher flag rate
+        // pay there (numharm 4, log-spaced widths, cfg 3: 8.92 ms at -3.25, 8.25 at -2.5, 8.35 at -2)
+        c->log10_p_flag = (p.log10_p_flag == kDefaultLog10PFlag) ? -2.5 : p.log10_p_flag;
         c->cell_cap_user = p.cell_cap_user; c->B = p.B;
         p.harm.push_back(c);
         const int rc = derive(*c);
@@ -1131,20 +1134,29 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
              p.has_tail ? "" : " (no tail launch)");
     s += line;
     if (p.has_tail) { snprintf(line, sizeof line, "norm tail: <EPT=%d,NT=%d> x 1/row\n", p.ept_tail, p.nt_tail); s += line; }
-    double evals = 0;
-    for (int l = 0; l < p.sp.nlevels; ++l) {
-        const SweepLevel& lv = p.sp.lv[l];
-        const double ev = 4.0 * lv.nsteps / (double)(1 << lv.lg);
-        evals += ev;
+    auto sweep_lines = [&](const pulscan_plan& q, const char* tag) {
+        double evals = 0;
+        for (int l = 0; l < q.sp.nlevels; ++l) {
+            const SweepLevel& lv = q.sp.lv[l];
+            const double ev = 4.0 * lv.nsteps / (double)(1 << lv.lg);
+            evals += ev;
+            snprintf(line, sizeof line,
+                     "sweep%s level %d: g=%d widths [%d,%d] covers m=[%d,%d] steps=%d warp-tasks/tile=%d  (%.3f cover sums per bin)\n", tag, l,
+                     1 << lv.lg, lv.wlo, lv.whi, lv.m_lo, lv.m_hi, lv.nsteps, lv.nwt, ev);
+            s += line;
+        }
         snprintf(line, sizeof line,
-                 "sweep level %d: g=%d widths [%d,%d] covers m=[%d,%d] steps=%d warp-tasks/tile=%d  (%.3f cover sums per bin)\n", l,
-                 1 << lv.lg, lv.wlo, lv.whi, lv.m_lo, lv.m_hi, lv.nsteps, lv.nwt, ev);
+                 "sweep%s: tile=%d len=%d tiles/row=%d smem=%zu B, %.3f cover sums per bin (exhaustive: %d), p_flag=1e%g, scan: %d quads per thread x %d pass(es)%s\n",
+                 tag, q.sp.tile, q.sp.len, q.tiles_per_row, q.smem_sweep, evals, q.zmax, q.log10_p_flag, q.sp.scan_nq, q.sp.npass,
+                 q.sweep_fine ? ", full resolution" : "");
         s += line;
+    };
+    sweep_lines(p, "");
+    for (size_t h = 0; h < p.harm.size(); ++h) {
+        char tag[16];
+        snprintf(tag, sizeof tag, " Y_%d", (int)h + 2);
+        if (!derive(*p.harm[h])) sweep_lines(*p.harm[h], tag);
     }
-    snprintf(line, sizeof line,
-             "sweep: tile=%d len=%d tiles/row=%d smem=%zu B, %.3f cover sums per bin (exhaustive: %d), p_flag=1e%g\n", p.sp.tile,
-             p.sp.len, p.tiles_per_row, p.smem_sweep, evals, p.zmax, p.log10_p_flag);
-    s += line;
     snprintf(line, sizeof line, "intermediate in HBM: %s\n",
              p.keep_P ? "float32 power of every bin (4 B/bin)" : "sums of 4-bin groups (1 B/bin) + 32 B per normalisation block");
     s += line;
