@@ -16,7 +16,8 @@
 //    register and read as fp16 pairs (bucket indices ≤ 2047 sit in fp16's denormal + first binade, where the
 //    encoding is linear, so HFMA2/HADD2 do exact integer arithmetic on them):
 //        z = ||4·(idx − ⌊c2/2⌋)| − K| − K,   member ⇔ |z| ≤ HW   (2t ∈ [0, HW] ∪ [2K − HW, 2K + HW])
-//    five half2 instructions per two values; hits (≈ 30 of 4096) are appended to a list;
+//    five half2 instructions per two values; the hits (≈ 30 of 4096) are re-read, classified exactly (median net or MAD
+//    shells) and appended to the list of their class, the re-reads of both components in flight together;
 //  * one warp per component ranks the ≤ 64 median-net members and the ≤ 64 shell members exactly, and VERIFIES that
 //    no value outside the shells can lie between the two central deviations (bucket boundaries mapped back to values
 //    in double, with a margin).  Anything unusual (degenerate sample, lists too long, verification failed) sends the
@@ -295,8 +296,8 @@ __device__ __forceinline__ void v2_rank_pair(const float* __restrict__ arr, int 
     vt1 = v2_key_float(__reduce_max_sync(0xffffffffu, kb));
 }
 
-// One warp, one component: split the gathered members into the median net and the shells, rank both exactly, verify
-// that the shells really hold the MAD, publish a, h, inv.
+// One warp, one component: rank the gathered members of the median net and of the shells exactly, verify that the
+// shells really hold the MAD, publish a, h, inv.
 template <int B>
 __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     constexpr int kk = (B - 1) >> 1;

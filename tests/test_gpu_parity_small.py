@@ -489,3 +489,26 @@ def test_group_sums_and_block_statistics_rebuild_the_powers(orc, n, B):
     assert torch.equal(rebuilt, P)
     ref = orc.normalise_power(spec[0].cpu().numpy(), B)              # and the statistics are the paper's: median and κ·MAD
     assert np.all(np.abs(P[0].cpu().numpy() - ref) <= 1e-5 * ref + 1e-6)
+
+
+@pytest.mark.parametrize("n,zmax,B,C,thr,tile", [
+    (200001, 200, 4096, 200, 5.0, 0),        # 8448-bin tiles: one scan pass of 9 quads per thread, group-sum input
+    (200001, 1200, 8192, 1200, 5.0, 0),      # 9472-bin tiles: one pass of 11 quads per thread
+    (200001, 3000, 8192, 1024, 5.0, 16384),  # 16384-bin tiles + halo: several passes of 5 quads per thread
+    (60001, 100, 2048, 100, 5.0, 2048),      # small tiles: one pass of 5
+])
+def test_sweep_second_look_and_scan_variants(orc, monkeypatch, n, zmax, B, C, thr, tile):
+    """The sweep's own second look at a flagged cell (half-group covers, boxcar_sweep.cuh sweep_confirm_cell) only removes
+    cells that cannot hold a window above threshold: the candidates equal those of a plan built without it (and the oracle's),
+    while fewer cells reach the refine kernel; run for every quads-per-thread variant of the tile scan."""
+    spec = noise_spectra(2, n, seed=n + zmax)
+    bump(spec, 0, n // 3, min(zmax, 150), 1.5)
+    bump(spec, 1, n // 2, 9, 2.5)
+    got, stats = gpu_search(spec, zmax, B, C, thr, tile=tile)
+    assert stats[9] >= stats[2] > 0 and stats[3] == 0        # flagged ≥ listed after the second look; nothing dropped
+    monkeypatch.setenv("PULSCAN_NO_CONFIRM", "1")
+    ref, rstats = gpu_search(spec, zmax, B, C, thr, tile=tile)
+    monkeypatch.delenv("PULSCAN_NO_CONFIRM")
+    assert np.array_equal(got, ref) and len(got) > 0
+    assert rstats[2] == rstats[9] >= stats[2]                 # without the τ_h tables every flagged cell is listed
+    assert_same_candidates(got, oracle_search(orc, spec, zmax, B, C, thr), f"zmax={zmax} tile={tile}")
