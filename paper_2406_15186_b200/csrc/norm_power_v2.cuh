@@ -425,6 +425,9 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     unsigned* hist = reinterpret_cast<unsigned*>(v2_raw + (STAGED ? (size_t)B * 8 + 16 : 0));
     V2Ctl& ctl = *reinterpret_cast<V2Ctl*>(hist + 2 * kV2NB);
     const int tid = threadIdx.x, warp = tid >> 5;
+    // Bin of thread tid in round r: wb + 32·r.  Each warp owns a contiguous run of 32·EPT bins: four rounds of a warp are 128
+    // consecutive bins = 32 consecutive group sums, which the output pass writes as one 128-byte line per store.
+    const int wb = warp * (EPT * 32) + (tid & 31);
     const unsigned row = blockIdx.x / (unsigned)blocks_per_row;
     const unsigned jblk = blockIdx.x - row * (unsigned)blocks_per_row;
     const long long lo_bin = (long long)jblk * B;
@@ -479,7 +482,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     if (STAGED && !use_tma) {
         float2* sw = reinterpret_cast<float2*>(stage + shift);
 #pragma unroll 4
-        for (int r = 0; r < EPT; ++r) sw[tid + r * NT] = __ldg(src + tid + r * NT);
+        for (int r = 0; r < EPT; ++r) sw[wb + r * 32] = __ldg(src + wb + r * 32);
         __syncthreads();
     }
     if (warp == 0) {
@@ -499,7 +502,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         const unsigned hb0 = v2_smem(hist), hb1 = v2_smem(hist + kV2NB);
 #pragma unroll
         for (int q = 0; q < EPT / 2; ++q) {
-            const float2 z0 = sdat[tid + (2 * q) * NT], z1 = sdat[tid + (2 * q + 1) * NT];
+            const float2 z0 = sdat[wb + (2 * q) * 32], z1 = sdat[wb + (2 * q + 1) * 32];
             const unsigned b00 = v2_bucket_bits(z0.x, sc0, of0), b01 = v2_bucket_bits(z1.x, sc0, of0);
             const unsigned b10 = v2_bucket_bits(z0.y, sc1, of1), b11 = v2_bucket_bits(z1.y, sc1, of1);
             v2_red_inc(hb0 + (b00 << 2)); v2_red_inc(hb0 + (b01 << 2));
@@ -550,7 +553,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
             unsigned ip[2];
             if (KEEPIDX) { ip[0] = idxp[0][q]; ip[1] = idxp[1][q]; }
             else {
-                const float2 z0 = sdat[tid + (2 * q) * NT], z1 = sdat[tid + (2 * q + 1) * NT];
+                const float2 z0 = sdat[wb + (2 * q) * 32], z1 = sdat[wb + (2 * q + 1) * 32];
                 ip[0] = __byte_perm(v2_bucket_bits(z0.x, sc0, of0), v2_bucket_bits(z1.x, sc0, of0), 0x5410);
                 ip[1] = __byte_perm(v2_bucket_bits(z0.y, sc1, of1), v2_bucket_bits(z1.y, sc1, of1), 0x5410);
             }
@@ -566,7 +569,7 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
         auto hit_addr = [&](unsigned m, int c) {
             const int b = __ffs(m) - 1;
-            return reinterpret_cast<const float*>(sdat + tid + (2 * (b & 15) + (b >> 4)) * NT) + c;
+            return reinterpret_cast<const float*>(sdat + wb + (2 * (b & 15) + (b >> 4)) * 32) + c;
         };
         auto put = [&](float val, int c) {
             const int tt = abs(2 * (int)(v2_bucket_bits(val, ctl.scale[c], ctl.off[c]) & 0xFFFFu) - ctl.c2[c]);
@@ -598,24 +601,24 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         if (out.P) {
             float* dst = out.P + (long long)row * out.pitchP + lo_bin;
 #pragma unroll
-            for (int r = 0; r < EPT; ++r) dst[tid + r * NT] = norm_power_value(sdat[tid + r * NT], a0, i0, k0, a1, i1, k1);
+            for (int r = 0; r < EPT; ++r) dst[wb + r * 32] = norm_power_value(sdat[wb + r * 32], a0, i0, k0, a1, i1, k1);
         }
         if (out.G) {   // sums of aligned groups of four bins (lanes 4j..4j+3 hold a group), see norm_power.cuh
-            float* g = out.G + (long long)row * out.pitchG + (lo_bin >> 2) + (tid >> 2);
+            float* g = out.G + (long long)row * out.pitchG + (lo_bin >> 2) + (wb >> 2);
             if constexpr (EPT % 4 == 0) {
 #pragma unroll
                 for (int r0 = 0; r0 < EPT; r0 += 4) {
-                    const float e = quad_sums4(norm_power_value(sdat[tid + r0 * NT], a0, i0, k0, a1, i1, k1),
-                                               norm_power_value(sdat[tid + (r0 + 1) * NT], a0, i0, k0, a1, i1, k1),
-                                               norm_power_value(sdat[tid + (r0 + 2) * NT], a0, i0, k0, a1, i1, k1),
-                                               norm_power_value(sdat[tid + (r0 + 3) * NT], a0, i0, k0, a1, i1, k1));
-                    g[(r0 + (tid & 3)) * (NT / 4)] = e;
+                    const float e = quad_sums4(norm_power_value(sdat[wb + r0 * 32], a0, i0, k0, a1, i1, k1),
+                                               norm_power_value(sdat[wb + (r0 + 1) * 32], a0, i0, k0, a1, i1, k1),
+                                               norm_power_value(sdat[wb + (r0 + 2) * 32], a0, i0, k0, a1, i1, k1),
+                                               norm_power_value(sdat[wb + (r0 + 3) * 32], a0, i0, k0, a1, i1, k1));
+                    g[(r0 + (tid & 3)) * 8] = e;       // 32 consecutive group sums per warp and store: one 128-byte line
                 }
             } else {
 #pragma unroll
                 for (int r = 0; r < EPT; ++r) {
-                    const float e = quad_sum1(norm_power_value(sdat[tid + r * NT], a0, i0, k0, a1, i1, k1));
-                    if ((tid & 3) == 0) g[r * (NT / 4)] = e;
+                    const float e = quad_sum1(norm_power_value(sdat[wb + r * 32], a0, i0, k0, a1, i1, k1));
+                    if ((tid & 3) == 0) g[r * 8] = e;
                 }
             }
             if (tid == 0) {
