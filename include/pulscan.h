@@ -213,7 +213,7 @@ int64_t pulscan_plan_group_pitch(const pulscan_plan* plan);
  * h_stats[3] = cells dropped because the list was full (their tiles' blocks are all marked),
  * h_stats[4..8] = why blocks were handed over (geometry, search window, list capacity, verification,
  * degenerate sample), h_stats[9] = cover cells flagged by the sweep's cover sums before its second look,
- * h_stats[10..15] reserved.  h_stats must hold 16 values. */
+ * h_stats[10] = flagged lanes of the sweep whose blocks were marked directly (strong signals), h_stats[11..15] reserved.  h_stats must hold 16 values. */
 int pulscan_plan_get_thresholds(const pulscan_plan* plan, double* h_T);
 int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf_bytes);
 int pulscan_plan_get_stats(pulscan_plan* plan, uint32_t* h_stats, void* cuda_stream);

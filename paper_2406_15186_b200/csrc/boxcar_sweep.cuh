@@ -52,6 +52,10 @@ constexpr int kSweepBufs = PULSCAN_SWEEP_BUFS;   // landing buffers per CTA (cop
 constexpr int kRefineThreads = 128;        // sweep_refine_kernel: 4 warps, one listed cell per warp at a time
 constexpr int kMaxWarpTasks = 128;         // warp-tasks per tile (8 levels of at most tile/(256·g) each)
 constexpr int kPadG = 16;                  // replicated entries after each decimated prefix array (window over-read)
+#ifndef PULSCAN_SWEEP_DENSE_LANES
+#define PULSCAN_SWEEP_DENSE_LANES 5   /* cfg 4, sweep+refine / kernel (c) ms: 8: 0.398/0.193, 5: 0.355/0.202, 4: 0.348/0.258, 3: 0.320/0.490 (noise cells marked) */
+#endif
+constexpr int kSweepDenseLanes = PULSCAN_SWEEP_DENSE_LANES;        // flagged lanes of a warp-task from which its blocks are marked without listing cells
 constexpr float kSlackUlps = 96.f;         // ≥ 2·(2 + 4 + 5 + 7 + passes + 1) + 1 roundings, see above
 
 struct SweepLevel {
@@ -444,7 +448,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
 // Streaming filter, persistent: gridDim.x CTAs (a multiple of the SM count) stride over the n_items = tiles_per_row ·
 // batch tiles.  Two landing buffers: a tile's copy is issued as soon as the previous user of its buffer has read its
 // powers into registers, i.e. a whole tile ahead.  Two CTA barriers per tile (both inside the scan).
-// counters[2] = cells appended (the refine kernel's work count), counters[9] = cells flagged before the second look
+// counters[2] = cells appended (the refine kernel's work count), counters[9] = cells flagged before the second look,
+// counters[10] = flagged lanes whose blocks were marked directly (dense warp-tasks),
 // (sweep_confirm_cell), counters[3] = cells dropped because the list was full
 // (their tile's blocks are all marked instead, which is always allowed: kernel (c) decides).
 // Dynamic shared memory: [kSweepBufs × z_floats landing buffers][decimated arrays][ntau τ][SweepCtl].
@@ -519,6 +524,19 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             const int k0b = tb.y + lane * kSweepR;
             const unsigned mask = (k0b < tb.z) ? sweep_task(sG + ta.x, k0b, ta.z, ta.w, sTau + ta.y, slack) : 0u;
             unsigned lanes = __ballot_sync(0xffffffffu, mask != 0u);     // rare: 1.3 cells per tile in noise
+            // Many flagged lanes in one warp-task are a strong signal, not noise: every flagged lane marks the candidate blocks
+            // that own its 8·g start bins straight away (always allowed: kernel (c) decides) instead of the warp walking
+            // through hundreds of cells one at a time while the rest of its CTA waits at the next barrier.
+            if (lanes == 0u) continue;
+            if (__popc(lanes) >= kSweepDenseLanes && ((kSweepR << sp.lv[tb.x].lg) <= 16 * C)) {
+                if (mask != 0u) {
+                    const long long t0 = (long long)tix * sp.tile + ((long long)k0b << sp.lv[tb.x].lg);
+                    const long long last = min(t0 + (kSweepR << sp.lv[tb.x].lg) - 1, n - 1);
+                    for (long long c = t0 / C; c <= last / C; ++c) mark_block((unsigned long long)(row * nblk + c), bitmap, flagged, counters);
+                }
+                if (lane == 0) atomicAdd(counters + 10, (unsigned)__popc(lanes));
+                continue;
+            }
             while (lanes) {
                 const int src = __ffs(lanes) - 1;
                 lanes &= lanes - 1;
