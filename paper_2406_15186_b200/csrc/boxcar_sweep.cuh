@@ -94,6 +94,7 @@ struct SweepParams {
     int smem_floats; // two landing buffers + decimated arrays
     int ref_span;    // longest span of bins a listed cell covers (sweep_refine_kernel's shared memory per warp)
     int tp_monotone; // T'_w is finite and non-decreasing in w (every width searched, exact significance)
+    int dense_lanes; // flagged lanes of a warp-task from which its blocks are marked without listing cells; 33 = never
     SweepLevel lv[kMaxLevels];
 };
 
@@ -528,7 +529,7 @@ boxcar_sweep_kernel(const __grid_constant__ SweepParams sp, const float* __restr
             // that own its 8·g start bins straight away (always allowed: kernel (c) decides) instead of the warp walking
             // through hundreds of cells one at a time while the rest of its CTA waits at the next barrier.
             if (lanes == 0u) continue;
-            if (__popc(lanes) >= kSweepDenseLanes && ((kSweepR << sp.lv[tb.x].lg) <= 16 * C)) {
+            if (__popc(lanes) >= sp.dense_lanes && ((kSweepR << sp.lv[tb.x].lg) <= 16 * C)) {
                 if (mask != 0u) {
                     const long long t0 = (long long)tix * sp.tile + ((long long)k0b << sp.lv[tb.x].lg);
                     const long long last = min(t0 + (kSweepR << sp.lv[tb.x].lg) - 1, n - 1);
