@@ -329,10 +329,14 @@ def test_strong_signal_many_flagged_blocks(orc):
     wl = synth.CONFIGS[2].scaled(n_samples=1 << 18, zmax=200, norm_block=4096, block_width=200, n_fixed_random=0,
                                  fixed=(synth.Injection(0, 201.3, 0.3, 150.0), synth.Injection(0, 411.0, 0.2, 0.0)), seed=5)
     X, _ = synth.make_spectra(wl, device="cuda")
-    gpu, _ = gpu_search(X, wl.zmax, wl.norm_block, wl.block_width, 6.0)
+    gpu, stats = gpu_search(X, wl.zmax, wl.norm_block, wl.block_width, 6.0)
     ora = oracle_search(orc, X, wl.zmax, wl.norm_block, wl.block_width, 6.0)
     assert len(ora) >= 2
     assert_same_candidates(gpu, ora, "strong signals")
+    assert stats[10] > 0       # warp-tasks with many flagged lanes marked their blocks directly (the sweep's strong-signal shortcut)
+    # the same search with the shortcut off (a flag probability above 10^-3 disables it): identical candidates
+    slow, sstats = gpu_search(X, wl.zmax, wl.norm_block, wl.block_width, 6.0, log10_p_flag=-2.9)
+    assert sstats[10] == 0 and np.array_equal(gpu, slow)
 
 
 def test_batch_rows_independent_on_gpu():
