@@ -567,10 +567,6 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
                 hm[c] |= mm & ((1u << q) | (1u << (16 + q)));
             }
         }
-        auto hit_addr = [&](unsigned m, int c) {
-            const int b = __ffs(m) - 1;
-            return reinterpret_cast<const float*>(sdat + wb + (2 * (b & 15) + (b >> 4)) * 32) + c;
-        };
         auto put = [&](float val, int c) {
             const int tt = abs(2 * (int)(v2_bucket_bits(val, ctl.scale[c], ctl.off[c]) & 0xFFFFu) - ctl.c2[c]);
             const int k = tt <= ctl.tm[c] ? 0 : (tt >= ctl.t0[c] && tt <= ctl.tE[c]) ? 1 : -1;
@@ -579,13 +575,36 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
                 if (slot < (unsigned)kV2ClsCap) ctl.cls[c][k][slot] = val;
             }
         };
-        while (hm[0] | hm[1]) {
-            const bool h0 = hm[0] != 0, h1 = hm[1] != 0;
-            float v0 = 0.f, v1 = 0.f;
-            if (h0) v0 = *hit_addr(hm[0], 0);
-            if (h1) v1 = *hit_addr(hm[1], 1);
-            if (h0) { put(v0, 0); hm[0] &= hm[0] - 1; }
-            if (h1) { put(v1, 1); hm[1] &= hm[1] - 1; }
+        // The warp's hits (≈ 15) are dealt to its lanes, one each, so that their re-reads make ONE round trip instead of one
+        // per hit of the unluckiest lane: hit j belongs to the lane whose running count first exceeds j.
+        const int lane = tid & 31;
+        const int n0 = __popc(hm[0]), cnt = n0 + __popc(hm[1]);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        for (int j0 = 0; j0 < total; j0 += 32) {
+            const int j = j0 + lane;
+            int owner = 0;                                   // number of lanes whose running count is ≤ j (incl is non-decreasing)
+#pragma unroll
+            for (int step = 16; step > 0; step >>= 1) {
+                const int v = __shfl_sync(0xffffffffu, incl, min(owner + step - 1, 31));
+                if (v <= j) owner += step;
+            }
+            owner = min(owner, 31);
+            const int oi = __shfl_sync(0xffffffffu, incl, owner), oc = __shfl_sync(0xffffffffu, cnt, owner);
+            const int on0 = __shfl_sync(0xffffffffu, n0, owner);
+            const unsigned om0 = __shfl_sync(0xffffffffu, hm[0], owner), om1 = __shfl_sync(0xffffffffu, hm[1], owner);
+            if (j < total) {
+                const int k = j - (oi - oc);                 // my hit is the k-th of that lane: component 0's first
+                const int c = k < on0 ? 0 : 1;
+                const int b = (int)__fns(c ? om1 : om0, 0, (c ? k - on0 : k) + 1);
+                const float val = reinterpret_cast<const float*>(sdat + (wb - lane + owner) + (2 * (b & 15) + (b >> 4)) * 32)[c];
+                put(val, c);
+            }
         }
     }
     __syncthreads();                                                                     // S5
