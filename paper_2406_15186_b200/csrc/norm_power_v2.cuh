@@ -469,8 +469,10 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     }
 #endif
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(v2_smem(&ctl.mbar)));
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (STAGED) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(v2_smem(&ctl.mbar)));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
         if (use_tma) v2_tma_issue(stage, csrc, nbytes, &ctl.mbar);
         ctl.fail = 0; ctl.cls_n[0][0] = 0; ctl.cls_n[0][1] = 0; ctl.cls_n[1][0] = 0; ctl.cls_n[1][1] = 0;
     }
