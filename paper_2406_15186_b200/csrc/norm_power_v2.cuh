@@ -206,11 +206,13 @@ __device__ __forceinline__ void v2_locate(V2Ctl& ctl, const unsigned* __restrict
         const int w0 = ws + 32 * it;
         // upper ends jm+e1+w0+1+lane: exclusive scan from a uniform start; lower ends jm+e0−w0−lane: scan downwards
         const int H0 = min(jm + e1 + w0 + 1, kV2NB), L0 = max(jm + e0 - w0, 0);
-        const unsigned aH0 = v2_count_below_uniform(L, CE, H0), aL0 = v2_count_below_uniform(L, CE, L0);
+        // #values in buckets [L0, H0): two chunk prefixes and one warp sum of the two partial chunks (modulo 2³², like g below)
+        const unsigned partH = lane < (H0 & 15) ? L[(H0 & ~15) + lane] : 0u, partL = lane < (L0 & 15) ? L[(L0 & ~15) + lane] : 0u;
+        const unsigned a0 = CE[H0 >> 4] - CE[L0 >> 4] + __reduce_add_sync(0xffffffffu, partH - partL);
         const unsigned xh = (H0 + lane < kV2NB) ? L[H0 + lane] : 0u;
         const unsigned xl = (lane >= 1 && L0 - lane >= 0) ? L[L0 - lane] : 0u;
-        const unsigned sh = v2_incl_scan(xh), sl = v2_incl_scan(xl);
-        const unsigned g = (aH0 + sh - xh) - (aL0 - sl);
+        // G at σ = w0 + lane: a0 + (xh of the lanes below) + (xl up to this lane) = a0 + scan(xh + xl) − xh: one scan
+        const unsigned g = a0 + v2_incl_scan(xh + xl) - xh;
         const unsigned f1 = __ballot_sync(0xffffffffu, g >= kk + 1);
         const unsigned f2 = kEven ? __ballot_sync(0xffffffffu, g >= kk + 2) : f1;
         if (sg1 < 0 && f1) sg1 = w0 + __ffs(f1) - 1;
