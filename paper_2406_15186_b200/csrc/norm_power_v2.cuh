@@ -138,15 +138,6 @@ __device__ __forceinline__ unsigned v2_count_below(const unsigned* __restrict__ 
     return a;
 }
 
-// The same for a warp-uniform p: lanes share the ≤ 15 loads.
-__device__ __forceinline__ unsigned v2_count_below_uniform(const unsigned* __restrict__ L, const unsigned* __restrict__ CE,
-                                                           int p) {
-    const int lane = threadIdx.x & 31;
-    const int ch = p >> 4, rem = p & 15;
-    const unsigned part = lane < rem ? L[(ch << 4) + lane] : 0u;
-    return CE[ch] + __reduce_add_sync(0xffffffffu, part);
-}
-
 __device__ __forceinline__ unsigned v2_incl_scan(unsigned x) {
     const int lane = threadIdx.x & 31;
 #pragma unroll
