@@ -194,6 +194,29 @@ int pulscan_search_host(pulscan_plan* plan, const void* h_spectra, pulscan_candi
 int pulscan_normalise_power(pulscan_plan* plan, const void* d_spectra, float* d_power, void* cuda_stream);
 int64_t pulscan_plan_power_pitch(const pulscan_plan* plan);
 
+/* Steps 1-2 (L140-150, Eq. 8: exact median/MAD normalisation, then the power) for a caller that cannot allocate device memory.
+ * Who that is: a stage of a telescope back-end whose device memory was all handed out as ring buffers when the pipeline
+ * started, a plug-in inside a host application that owns the allocator and passes the plug-in nothing but its input and
+ * output buffers, code on a latency-critical path where cudaMalloc's device-wide synchronisation is not acceptable.  Such a
+ * caller has no workspace to give pulscan_plan_set_workspace, and without one pulscan_normalise_power falls back to its slower
+ * general kernels.  This entry point runs the same fast kernels as pulscan_search; the scratch they need (the list of blocks
+ * handed to the general kernel, a few counters) is a fixed array inside the library image instead of caller memory.
+ *   - It calls no cudaMalloc / cudaFree and no library routine that allocates; the plan needs NO workspace (an attached one is
+ *     ignored).  The caller passes d_spectra and d_power exactly as for pulscan_normalise_power (same layout, alignment, result).
+ *   - Limit: batch · max(1, n_bins div norm_block) ≤ PULSCAN_STATIC_MAX_NORM_BLOCKS, else PULSCAN_EINVAL (checked on the host
+ *     before anything is enqueued).  The array is 4 bytes per block + 256 bytes ≈ 1 MiB and stays resident on every GPU the
+ *     process uses with this library until the process exits, whether or not this function is ever called.
+ *   - The first call on each device looks the array's device address up and sets kernel attributes on that device (with the
+ *     target device current, as for every call).  Make that first call outside any stream capture; later calls only enqueue
+ *     one 256-byte memset and the kernels on `cuda_stream`.
+ *   - All calls on one device share the one array.  Every call zeroes the counters it needs before its kernels run, so
+ *     back-to-back calls on one stream are fine whatever the previous call left behind; two calls that can overlap on the GPU
+ *     (different streams, different host threads, different plans) race on it and corrupt each other's output.  Serialise them.
+ *   - PULSCAN_EINVAL for a plan set to the Alg. 1 normalisation: that kernel needs no scratch, pulscan_normalise_power already
+ *     allocates nothing for it. */
+#define PULSCAN_STATIC_MAX_NORM_BLOCKS 262144
+int pulscan_normalise_power_static(pulscan_plan* plan, const void* d_spectra, float* d_power, void* cuda_stream);
+
 /* Steps 1-2 in the form the default search keeps them in HBM (for unit tests and profiling): instead of the power of every
  * bin, d_group_sums receives float32 [batch][pulscan_plan_group_pitch()] with G[k] = (P[4k] + P[4k+1]) + (P[4k+2] + P[4k+3])
  * (bins ≥ n_bins count as 0; entries ≥ ceil(n_bins/4) are unspecified), and d_block_stats float32

@@ -49,6 +49,7 @@ SIGNATURES = {
     "pulscan_search_host": (ctypes.c_int, [_P, _P, _P, _P, _P]),
     "pulscan_normalise_power": (ctypes.c_int, [_P, _P, _P, _P]),
     "pulscan_plan_power_pitch": (ctypes.c_int64, [_P]),
+    "pulscan_normalise_power_static": (ctypes.c_int, [_P, _P, _P, _P]),
     "pulscan_normalise_group_sums": (ctypes.c_int, [_P, _P, _P, _P, _P]),
     "pulscan_plan_group_pitch": (ctypes.c_int64, [_P]),
     "pulscan_plan_get_thresholds": (ctypes.c_int, [_P, _P]),
@@ -255,6 +256,17 @@ class Plan:
         """Steps 1-2 only: float32 power [batch, n_bins] (a view of the padded [batch, power_pitch] buffer)."""
         out = torch.empty((self.batch, self.power_pitch), dtype=torch.float32, device=d_spectra.device)
         _check(self.lib.pulscan_normalise_power(self.handle, d_spectra.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
+        return out[:, : self.n_bins]
+
+    def normalise_power_static(self, d_spectra: torch.Tensor, out: torch.Tensor,
+                               stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        """pulscan_normalise_power_static: steps 1-2 for callers that cannot allocate device memory (all of it was given out
+        at start-up, or the host application owns the allocator).  The plan needs no workspace and nothing is allocated here
+        either: `out` is the caller's float32 [batch, power_pitch] buffer; the kernels' scratch is a fixed array inside the
+        library (limit: batch x normalisation blocks <= PULSCAN_STATIC_MAX_NORM_BLOCKS).  Calls share that array: do not let
+        two of them overlap on the GPU.  Returns the [batch, n_bins] view of `out`."""
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and out.shape == (self.batch, self.power_pitch)
+        _check(self.lib.pulscan_normalise_power_static(self.handle, d_spectra.data_ptr(), out.data_ptr(), _stream_ptr(stream)))
         return out[:, : self.n_bins]
 
     def normalise_group_sums(self, d_spectra: torch.Tensor, norm_block: int, stream: Optional[torch.cuda.Stream] = None):

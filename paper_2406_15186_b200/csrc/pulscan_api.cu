@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1228,6 +1229,71 @@ int pulscan_plan_destroy(pulscan_plan* plan) {
     release_profiling(*plan);
     delete plan;
     return PULSCAN_OK;
+}
+
+// ------------------------------------------------------------------------------------ static-scratch entry point
+// pulscan_normalise_power_static: steps 1-2 for callers that have no device memory to give beyond their input and output.
+// The exact normalisation's fast kernel needs a little scratch: a list of the blocks it hands to the general kernel and a few
+// counters.  Everywhere else in this library that scratch is part of the caller's workspace; here it is the array below, which
+// is part of the loaded library image on every GPU (≈ 1 MiB, held until the process exits).
+//
+// g_static_scratch is only a device address inside device code.  In the host code of this file the name is a handle for the
+// runtime, so the real address is asked for once per device (cudaGetSymbolAddress, with that device current) and remembered.
+namespace {
+
+constexpr unsigned kStaticCounterWords = 64;   // [1] = entries in the list, [4..8] = why blocks were handed over; 256 bytes
+static __device__ __align__(256) unsigned g_static_scratch[kStaticCounterWords + PULSCAN_STATIC_MAX_NORM_BLOCKS];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned* g_static_addr[kStaticMaxDevices] = {};   // per device ordinal; nullptr = not set up yet
+
+// Set-up on first use per device: architecture check, kernel attributes, address of the array on the CURRENT device.
+int static_scratch_on_current_device(unsigned** out) {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(PULSCAN_EINVAL, "device ordinal %d beyond the %d this entry point tracks", dev, kStaticMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        int major = 0;
+        CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return fail(PULSCAN_EARCH, "device %d is compute capability %d.x; libpulscan is built for sm_100a only", dev, major);
+        pulscan_plan none;
+        const int rc = set_kernel_attributes(none);
+        if (rc) return rc;
+        unsigned* addr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&addr), g_static_scratch);
+        if (e != cudaSuccess || !addr)
+            return fail(PULSCAN_ECUDA, "cudaGetSymbolAddress(g_static_scratch) failed on device %d: %s", dev, cudaGetErrorString(e));
+        g_static_addr[dev] = addr;
+    }
+    *out = g_static_addr[dev];
+    return PULSCAN_OK;
+}
+
+} // namespace
+
+int pulscan_normalise_power_static(pulscan_plan* plan, const void* d_spectra, float* d_power, void* cuda_stream) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    int rc = derive(*plan);
+    if (rc) return rc;
+    if (plan->norm_mode == 1)
+        return fail(PULSCAN_EINVAL, "the Alg. 1 normalisation uses no scratch: call pulscan_normalise_power (it allocates nothing either)");
+    const long long blocks = (long long)plan->batch * plan->nb;
+    if (blocks > (long long)PULSCAN_STATIC_MAX_NORM_BLOCKS)
+        return fail(PULSCAN_EINVAL, "batch x normalisation blocks per spectrum = %lld exceeds PULSCAN_STATIC_MAX_NORM_BLOCKS = %d: "
+                                    "pass fewer spectra per call or use a longer norm_block", blocks, (int)PULSCAN_STATIC_MAX_NORM_BLOCKS);
+    if (!d_spectra || !d_power) return fail(PULSCAN_EINVAL, "null pointer");
+    if (reinterpret_cast<uintptr_t>(d_spectra) & 7) return fail(PULSCAN_EINVAL, "d_spectra must be 8-byte aligned");
+    if (reinterpret_cast<uintptr_t>(d_power) & 15) return fail(PULSCAN_EINVAL, "d_power must be 16-byte aligned");
+    unsigned* scratch = nullptr;
+    if ((rc = static_scratch_on_current_device(&scratch))) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // the array still holds the previous call's counters and list: the counters must start at zero, the list is only read up
+    // to the new count
+    CUDA_TRY(cudaMemsetAsync(scratch, 0, kStaticCounterWords * sizeof(unsigned), st));
+    return enqueue_norm(*plan, d_spectra, NormOut{d_power, plan->pitchP, nullptr, 0, nullptr}, st, scratch + kStaticCounterWords,
+                        scratch + 1);
 }
 
 const char* pulscan_last_error(void) { return g_last_error.c_str(); }
