@@ -23,9 +23,11 @@
 //    double, re-tests the 32 covers and sums the ≤ g² windows of each passing cover against their own T'_w; blocks
 //    with a window that reaches T'_w are marked (bitmap + list).
 //
-// Float safety of the streaming kernel.  Every PG entry carries at most ~25 roundings of magnitude ≤ 2⁻²⁴·PP[len], so
-// a difference of two entries is off by < slack = kSlackUlps·2⁻²⁴·PP[len] from the exact sum of the float32 powers;
-// the cover test adds the slack on the keeping side.  The refine kernel works in double and compares with T'_w, which
+// Float safety of the streaming kernel.  Every PG entry carries at most D = scan_roundings(NQ, passes) roundings of magnitude
+// ≤ 2⁻²⁴·PP[len] (counted step by step at scan_roundings below: 26 for the one-pass scans of 11 quads per thread, 28 for five
+// passes of 5 quads), so a cover sum, the rounded difference of two entries, is off by at most (2·D + 1)·2⁻²⁴·PP[len] ≤ slack =
+// kSlackUlps·2⁻²⁴·PP[len] from the exact sum of the float32 powers (scan_tile asserts it for every NQ it is compiled for); the
+// cover test adds the slack on the keeping side.  The refine kernel works in double and compares with T'_w, which
 // the host rounds down by 2w·2⁻²⁴ + 2·10⁻⁶ relative.
 //
 // Exhaustive mode (the cross-check) evaluates every (i, w) by the paper's recursion instead.
@@ -56,7 +58,22 @@ constexpr int kPadG = 16;                  // replicated entries after each deci
 #define PULSCAN_SWEEP_DENSE_LANES 5   /* cfg 4, sweep+refine / kernel (c) ms: 8: 0.398/0.193, 5: 0.355/0.202, 4: 0.348/0.258, 3: 0.320/0.490 (noise cells marked) */
 #endif
 constexpr int kSweepDenseLanes = PULSCAN_SWEEP_DENSE_LANES;        // flagged lanes of a warp-task from which its blocks are marked without listing cells
-constexpr float kSlackUlps = 96.f;         // ≥ 2·(2 + 4 + 5 + 7 + passes + 1) + 1 roundings, see above
+constexpr float kSlackUlps = 96.f;         // ≥ 2·scan_roundings(NQ, passes) + 1, asserted in scan_tile
+// Longest landing buffer a plan can ask for: a 16384-bin tile + halo of zmax ≤ 4096 and two groups of ≤ 128 bins, rounded to 64.
+constexpr int kMaxSweepLen = 16384 + 4096 + 2 * 128 + 64;
+// Roundings on the way from the float32 powers to one entry PG[k] = PP[k·g] of scan_tile, each of magnitude ≤ 2⁻²⁴·PP[len]
+// (roundings of disjoint partial sums count once: each is relative to its own part of the total):
+//   3       the quad sum (((a + b) + c) + d in the full-resolution scan; (a + b) + (c + d), formed by kernel (a) as a group sum
+//           G or here, is 2)
+//   NQ − 1  the thread's serial prefix over its quads
+//   5       the warp's shuffle scan
+//   1       excl = incl − s[NQ−1]
+//   3       the butterfly sum of the totals of the warps below
+//   2       off = carry + (wbase + excl)
+//   1       s[q] += off
+//   1       the full-resolution entries x[3q+t] += s[q−1]
+//   2       per further pass: the carry, an entry of the pass before, goes through off and s[q] += off again
+constexpr int scan_roundings(int nq, int passes) { return 3 + (nq - 1) + 5 + 1 + 3 + 2 + 1 + 1 + 2 * (passes - 1); }
 
 struct SweepLevel {
     int lg;        // log2 of the group size g
@@ -192,6 +209,8 @@ __device__ __forceinline__ float scan_tile(const SweepParams& sp, const float* r
     static_assert(!(FINE && FROMG), "levels finer than four bins need the powers themselves");
     static_assert(NQ % 2 == 1 && NQ <= kScanTail / 4, "odd lane stride; zeros after the landing buffer");
     constexpr int kPer = 4 * NQ, kPass = kPer * kSweepThreads;
+    static_assert(2 * scan_roundings(NQ, (kMaxSweepLen + kPass - 1) / kPass) + 1 <= (int)kSlackUlps,
+                  "the cover test's slack no longer bounds the scan's rounding error: raise kSlackUlps or scan fewer quads per thread");
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int len = sp.len;
     float carry = 0.f;
