@@ -279,6 +279,8 @@ int derive(pulscan_plan& p) {
     sp.tile = tile;
     const int halo = (int)align_up((size_t)(p.zmax + 2 * (1 << lgmax)), 64);
     sp.len = tile + halo;
+    if (sp.len > kMaxSweepLen)   // the rounding bound of the scan (scan_roundings, boxcar_sweep.cuh) is asserted for this length
+        return fail(PULSCAN_EINVAL, "internal: sweep landing buffer of %d bins exceeds %d", sp.len, kMaxSweepLen);
     int off = 0, task = 0;
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = lvls[l];
@@ -471,7 +473,7 @@ int derive(pulscan_plan& p) {
         pulscan_plan* c = pulscan_plan_create(nH, p.batch, p.zmax, p.C, (float)p.sigma_thr);
         if (!c) return PULSCAN_EINVAL;
         c->is_child = true; c->shape_mult = H * (H + 1) / 2; c->numharm_tag = H; c->sigma_thr = p.sigma_thr; c->n_trials = p.n_trials;
-        c->signif_mode = p.signif_mode;
+        c->signif_mode = p.signif_mode; c->mode = p.mode;   // the mode is checked against the child's sweep levels at finalisation
         c->z_step = p.z_step; c->log_sampling = p.log_sampling; c->tile_user = p.tile_user;
         // a harmonic-summed spectrum has H(H+1)/2 of noise in every bin of a cover's slack: coarser groups at a higher flag rate
         // pay there (numharm 4, log-spaced widths, cfg 3: 8.92 ms at -3.25, 8.25 at -2.5, 8.35 at -2)
@@ -514,6 +516,10 @@ int finalize_device(pulscan_plan& p) {
     if (prop.major != 10)
         return fail(PULSCAN_EARCH, "device %s is compute capability %d.%d; libpulscan is built for sm_100a only", prop.name,
                     prop.major, prop.minor);
+    // all validation happens here ("Life of a plan"): a plan whose pruned sweep could not be sized must not get as far as a
+    // search (which would fail at enqueue time, possibly inside a stream capture)
+    if (p.mode == 0 && !p.pruned_error.empty())
+        return fail(PULSCAN_EINVAL, "%s; use mode 1 (exhaustive)", p.pruned_error.c_str());
     p.device = dev;
     p.sm_count = prop.multiProcessorCount;
     char* ws = static_cast<char*>(p.ws);
@@ -1155,6 +1161,10 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
                  q.sweep_fine ? ", full resolution" : "");
         s += line;
     };
+    if (!p.pruned_error.empty()) {
+        snprintf(line, sizeof line, "pruned sweep unavailable (pulscan_plan_set_workspace fails in mode 0): %s\n", p.pruned_error.c_str());
+        s += line;
+    }
     sweep_lines(p, "");
     for (size_t h = 0; h < p.harm.size(); ++h) {
         char tag[16];
