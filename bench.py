@@ -274,10 +274,10 @@ def run_ours(args):
         return 0
     prof = np.array([plan.profile(s) for s in range(warm, warm + steps)], dtype=np.float64).mean(axis=0)
     # Bytes per bin.  ALGORITHMIC: the path reads every complex64 bin once = 8 B/bin, and that is what the
-    # dominant kernel is held against too (any intermediate is the design's own cost); the boxcar stage on its own is defined
-    # on the 4 B/bin float32 power spectrum.  OWN TRAFFIC: what the kernel really moves — kernel (a) 8 read + 1 written as sums
-    # of 4-bin groups (4 with the per-bin array of --fast-norm), kernel (b) 1 (4) read.
-    keeps_p = bool(args.fast_norm)
+    # dominant kernel and the whole path are held against (any intermediate is the design's own cost).  OWN TRAFFIC: what a
+    # kernel really moves — kernel (a) 8 read + 1 written as sums of 4-bin groups (4 when the plan keeps the per-bin power
+    # array), the boxcar stage 1 (4) read.  Which of the two the plan keeps is read from the plan itself.
+    keeps_p = "intermediate in HBM: float32 power" in plan.describe()
     own = {"norm_power_kernel": 12 if keeps_p else 9, "boxcar_sweep_kernel": 4 if keeps_p else 1}
     ms = {"norm_power_kernel": prof[1], "boxcar_sweep_kernel": prof[2], "block_exact_kernel": prof[3]}
     dom = max(("norm_power_kernel", "boxcar_sweep_kernel"), key=lambda k: ms[k])
@@ -286,6 +286,25 @@ def run_ours(args):
     gbs = lambda nbytes, t_ms: nbytes / (t_ms * 1e-3) / 1e9
     achieved = gbs(8 * bins, dom_ms)
     traffic_per_bin = recorded_traffic(dom, args.config)
+    # The boxcar stage (sweep + refine, prof[2]) on its OWN traffic: the ncu-measured DRAM bytes per bin of the two kernels where
+    # the committed capture has them and the plan streams the group sums as in that capture, else the bytes it must read.
+    # §8's "fraction of HBM" for kernel (b) is this quantity; the stage is bound by instruction issue, so it also gets an issue
+    # roofline: warp-instructions per bin from the same capture (smsp__inst_executed.sum) against 4 schedulers x 1 instruction
+    # per clock x SMs at the SM clock sampled during the timed region.
+    sweep_ncu = None if keeps_p else recorded_traffic("boxcar_sweep_kernel", args.config)
+    if sweep_ncu is not None:
+        sweep_ncu += recorded_traffic("sweep_refine_kernel", args.config) or 0.0
+    sweep_bytes = sweep_ncu if sweep_ncu is not None else own["boxcar_sweep_kernel"]
+    sweep_instr = None if keeps_p else recorded_traffic("boxcar_stage_warp_instr_per_bin", args.config)
+    clocks = clk.summary()
+    sm_hz = 1e6 * (clocks.get("sm_mhz") or 1965.0)
+    issue_peak = 4.0 * torch.cuda.get_device_properties(dev).multi_processor_count * sm_hz
+    sweep_issue = None
+    if sweep_instr is not None:
+        rate = sweep_instr * bins / (prof[2] * 1e-3)
+        sweep_issue = {"bound": "alu", "achieved": rate, "peak": issue_peak, "unit": "warp-instr/s", "frac": rate / issue_peak,
+                       "warp_instr_per_bin": sweep_instr, "peak_source": "4 warp schedulers x SMs x sampled SM clock",
+                       "instr_source": "profiles/traffic.json (ncu smsp__inst_executed.sum of sweep + refine per bin)"}
     roofline = {
         "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "algorithmic_bytes_per_bin": 8, "algorithmic_bytes_per_launch": 8 * bins,
@@ -295,10 +314,13 @@ def run_ours(args):
         "kernel_ms": dom_ms,
         "kernel_ms_all": {"memsets": prof[0], "norm_power_kernel": prof[1], "boxcar_sweep_kernel": prof[2],
                           "block_exact_kernel": prof[3]},
-        "sweep_achieved": gbs(4 * bins, prof[2]), "sweep_frac": gbs(4 * bins, prof[2]) / peak,
-        "sweep_algorithmic_bytes_per_bin": 4, "sweep_own_bytes_per_bin": own["boxcar_sweep_kernel"],
         "path_algorithmic_GBps": gbs(8 * bins, ms_step) if world == 1 else None,
         "path_frac": gbs(8 * bins, ms_step) / peak if world == 1 else None,
+        "sweep_achieved": gbs(sweep_bytes * bins, prof[2]), "sweep_frac": gbs(sweep_bytes * bins, prof[2]) / peak,
+        "sweep_bytes_per_bin": sweep_bytes,
+        "sweep_bytes_source": "profiles/traffic.json (ncu, sweep + refine)" if sweep_ncu is not None else "bytes the stage must read",
+        "sweep_algorithmic_frac": gbs(4 * bins, prof[2]) / peak, "sweep_algorithmic_bytes_per_bin": 4,
+        "sweep_issue": sweep_issue,
     }
     launches = plan.launches_per_search * steps
 
@@ -335,7 +357,7 @@ def run_ours(args):
             "data": "synthetic", "config": config_dict(wl, world, args), "bin_widths_per_sec": value * wl.zmax,
             "latency_us_per_search": ms_step * 1e3 if n_copies > 1 else None,
             "candidates_per_step": n_cand, "blocks_flagged_by_sweep": flagged,
-            "sweep_cells_refined": int(stats[2]), "sweep_cells_flagged": int(stats[9]), "norm_blocks_redone": int(stats[1]), "clocks": clk.summary(),
+            "sweep_cells_refined": int(stats[2]), "sweep_cells_flagged": int(stats[9]), "norm_blocks_redone": int(stats[1]), "clocks": clocks,
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
         }
         print(json.dumps(out), flush=True)

@@ -84,9 +84,9 @@ __host__ __device__ inline double sigma_from_lnp(double lnp) {
 // Algorithm 3 (§2.6 Eq. 10-12): the paper's GPU approximation of ln p, a degree-16 polynomial
 // in x = 1500·dof/pow fitted by regression, in the paper's units (pow = |X'|² summed over the window = 2S, dof = its χ²
 // degrees of freedom = 2·shape; R31).  Horner form in double: the printed coefficients span 1e-46 … 1e2 and x
-// reaches 1428, so neither the coefficients nor the powers of x fit float32.
-__host__ __device__ inline double power_to_logp(double pw, double dof) {
-    if (dof >= pw * 1.05) return 0.0;
+// reaches 1575 (the branch dof ≥ 1.05·pow cuts it off there), so neither the coefficients nor the powers of x fit float32.
+// alg3_poly is the polynomial branch alone: pow·f(1500·dof/pow)/1500.
+__host__ __device__ inline double alg3_poly(double pw, double dof) {
     const double x = 1500.0 * dof / pw;
     double f = -4.4604059e-46;
     f = f * x + 9.4927863e-42;
@@ -107,6 +107,10 @@ __host__ __device__ inline double power_to_logp(double pw, double dof) {
     f = f * x - 755.24091;
     return pw * f / 1500.0;
 }
+__host__ __device__ inline double power_to_logp(double pw, double dof) {
+    if (dof >= pw * 1.05) return 0.0;
+    return alg3_poly(pw, dof);
+}
 
 // ln p of a sum S of Gamma shape `shape` (mean-1 units): mode 0 the exact χ² tail, mode 1 Alg. 3.
 __host__ __device__ inline double lnp_of(int signif_mode, int shape, double S) {
@@ -125,16 +129,40 @@ inline double power_threshold(int w, double lnp_target) {
 }
 
 // Host only: a lower bound of the smallest power S at which Alg. 3 reports ln p ≤ lnp_target for Gamma shape `shape`.  The
-// polynomial is not monotone in S (beyond x ≈ 1100 the printed coefficients do not determine it), so the first crossing is
-// found by a scan from the branch point S = shape/1.05 upwards and the last grid point before it is returned.
+// polynomial is not monotone in S (for x ≳ 1100, i.e. S ≲ 1.36·shape, the printed coefficients do not determine it, and at the
+// branch point x = 1575 it is already below −20 for shapes ≳ 110), so the first crossing is looked for from the branch point
+// S = shape/1.05 upwards: a coarse grid, and inside every grid interval where a crossing cannot be excluded — the lower of its
+// end values minus the largest change between neighbouring grid points is not above the target, a Lipschitz bound with a
+// factor 2 in hand — a bisection that keeps excluding halves the same way (slopes by central differences) down to 1e-9
+// relative.  What is returned is the lower end of the first interval that could not be excluded: never above the first
+// crossing, so no window the oracle's Alg. 3 would report is dropped by the power pre-threshold.  The scan evaluates the
+// polynomial branch itself from a hair below the branch point, where power_to_logp still returns 0.
+inline double alg3_first_crossing(double sh, double target, double a, double b, double ga, double gb, double la, double lb, int depth) {
+    // la, lb: |slope| estimates at the ends.  Nothing at or below the target inside [a, b]?
+    if (fmin(ga, gb) - (b - a) * fmax(la, lb) > target) return -1.0;
+    if (ga <= target || depth >= 48 || b - a <= 1e-9 * b) return a;
+    const double m = 0.5 * (a + b), h = 1e-7 * m;
+    const double gm = alg3_poly(2.0 * m, 2.0 * sh);
+    const double lm = fabs(alg3_poly(2.0 * (m + h), 2.0 * sh) - alg3_poly(2.0 * (m - h), 2.0 * sh)) / (2.0 * h);
+    const double r = alg3_first_crossing(sh, target, a, m, ga, gm, la, lm, depth + 1);
+    return r >= 0.0 ? r : alg3_first_crossing(sh, target, m, b, gm, gb, lm, lb, depth + 1);
+}
 inline double power_threshold_poly(int shape, double lnp_target) {
-    const double s0 = (double)shape / 1.05;
+    const double sh = (double)shape;
+    const double s0 = sh / 1.05 * (1.0 - 1e-12);
     const double hi = 4.0 * power_threshold(shape, lnp_target) + 64.0;
-    const double step = 0.01 + 0.01 * std::sqrt((double)shape);
-    double prev = s0 * (1.0 - 1e-12);
+    const double step = 0.01 + 0.01 * std::sqrt(sh);
+    auto g = [&](double S) { return alg3_poly(2.0 * S, 2.0 * sh); };
+    // sliding window over the grid: g at S − step, S, S + step, S + 2·step; the interval tested is [S, S + step]
+    double gm1 = g(s0), g0 = gm1, g1 = g(s0 + step), g2 = g(s0 + 2.0 * step);
     for (double S = s0; S <= hi; S += step) {
-        if (power_to_logp(2.0 * S, 2.0 * (double)shape) <= lnp_target) return prev;
-        prev = S;
+        const double d = fmax(fabs(g0 - gm1), fmax(fabs(g1 - g0), fabs(g2 - g1)));   // largest change per step nearby
+        if (fmin(g0, g1) - d <= lnp_target) {
+            const double l = d / step;
+            const double r = alg3_first_crossing(sh, lnp_target, S, S + step, g0, g1, l, l, 0);
+            if (r >= 0.0) return r;
+        }
+        gm1 = g0; g0 = g1; g1 = g2; g2 = g(S + 3.0 * step);
     }
     return hi;
 }

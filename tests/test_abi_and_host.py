@@ -202,3 +202,42 @@ def test_harmonics_sizes(binding):
     assert p4.workspace_bytes > p1.workspace_bytes              # room for Y_H and the scratch of its search
     with pytest.raises(binding.PulscanError):
         binding.Plan(100, 1, 30, 10, 6.0, numharm=4)            # zmax must be < floor(n/numharm)
+
+
+@pytest.mark.parametrize("sigma,zmax", [(6.0, 400), (3.5, 300), (10.0, 200), (4.5, 64)])
+def test_alg3_power_thresholds_never_sit_above_a_crossing(binding, sigma, zmax):
+    """With the polynomial ln p (Alg. 3) T_w is a power PRE-threshold: a window below it is never evaluated.
+    The polynomial is not monotone in S, so T_w must lie at or below the FIRST S at which Alg. 3 reports ln p <= the target —
+    the oracle evaluates every block maximum and would report such a window.  Dense scan of [w/1.05, T_w) with numpy.polyval on
+    the printed coefficients (typed in test_oracle_alg3.py from the paper; the oracle's own routine is checked on a sample):
+    nothing at or below the target.  w = 112 at sigma 6 and w = 45 at sigma 3.5 are the widths where the dip at the branch point
+    x = 1575 is narrower than one step of the library's coarse grid.  Where T_w is above the branch point it is also tight."""
+    import oracle
+    from test_oracle_alg3 import PRINTED
+
+    oracle.build()
+    coef = np.array([float(c) for c in PRINTED])
+    target = oracle.ln_sf(sigma)
+
+    def lnp(S, shape):
+        pw, dof = 2.0 * np.asarray(S, dtype=np.float64), 2.0 * shape
+        return np.where(dof >= 1.05 * pw, 0.0, pw * np.polyval(coef, 1500.0 * dof / pw) / 1500.0)
+
+    assert oracle.power_to_logp(2 * 30.0, 2 * 4.0) == pytest.approx(float(lnp(30.0, 4)), rel=1e-12)
+    p = binding.Plan(100000, 1, zmax, 50, sigma, poly_logp=True)
+    T = p.thresholds()
+    p.destroy()
+    at_branch = 0
+    for w in range(1, zmax + 1):
+        s0 = w / 1.05
+        assert T[w - 1] >= s0 * (1 - 1e-9)
+        S = np.linspace(s0, T[w - 1], 20001)[:-1]
+        S = S[S < T[w - 1] * (1 - 1e-12)]
+        if S.size:
+            bad = S[lnp(S, w) <= target]
+            assert bad.size == 0, f"w = {w}: ln p <= target at S = {bad[0]} < T_w = {T[w - 1]}"
+        if T[w - 1] > s0 * (1 + 1e-6):        # a real crossing: just above T_w the polynomial is at the target
+            assert float(lnp(T[w - 1] * (1 + 1e-6), w)) <= target + 1e-3, w
+        else:
+            at_branch += 1
+    assert (at_branch > 0) == (sigma in (6.0, 3.5))   # wide windows at low thresholds: Alg. 3 is already past the target at x = 1575
