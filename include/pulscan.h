@@ -31,6 +31,12 @@
  * graph).  A setter that changes derived state or the workspace layout (every setter except _set_r_block, and
  * _set_emission without host staging) returns the plan to step (1): searches then fail with PULSCAN_ENOWORKSPACE until
  * pulscan_plan_set_workspace is called again (pulscan_plan_workspace_bytes may have changed).
+ *
+ * One search at a time per plan.  The counters, the block bitmap, the cell and block lists, the intermediate arrays and the
+ * profiling slots all live in the plan's one workspace: two searches of the SAME plan that can overlap on the GPU (two streams)
+ * or that are enqueued from two host threads at once race with each other.  Searches on one stream, one after the other, are
+ * the supported use; for concurrent searches create one plan (and workspace) per stream.  Different plans are independent,
+ * except for pulscan_normalise_power_static, whose calls share one array per device.
  */
 #ifndef PULSCAN_H
 #define PULSCAN_H
@@ -153,6 +159,26 @@ int pulscan_plan_set_emission(pulscan_plan* plan, int32_t per_width, int64_t cap
 /* Tuning of the pruned sweep: tile_bins (multiple of 512, 1024..16384; 0 = default) and the per-cover false-flag
  * probability in noise as log10 (−1 … −9; 0 = default).  Affects speed only, never results. */
 int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_p_flag);
+
+/* Kernel variants: comparison and tuning switches that change which kernel variant runs or how the workspace is laid out,
+ * NEVER a result (the GPU tests run the parity suite's cases with them).  They replace the environment variables the library
+ * read until round 2; the only one left is PULSCAN_DEBUG_SYNC (any value: cudaDeviceSynchronize after every launch so that a
+ * device fault is reported by the launch that caused it; a debugging aid, never on a timed or captured path).
+ *   PULSCAN_VARIANT_SWEEP_SECOND_LOOK      1 (default) / 0: the sweep re-tests a flagged cell against half-group thresholds itself
+ *   PULSCAN_VARIANT_SCAN_QUADS             0 (default: 5, 9 or 11 quads per thread by tile length) / 5: the multi-pass scan
+ *   PULSCAN_VARIANT_NORM_KEEP_INDICES      -1 (default: by norm_block) / 0 / 1: kernel (a) keeps bucket indices in registers
+ *   PULSCAN_VARIANT_NORM_L2_AHEAD          -1 (default: 4 x SMs) / n >= 0: CTAs of L2 look-ahead of kernel (a), 0 = off
+ *   PULSCAN_VARIANT_NORM_SINGLE_HISTOGRAM  1 (default) / 0: every normalisation block through the general select kernel
+ *   PULSCAN_VARIANT_KEEP_POWER             0 (default) / 1: keep the float32 power of every bin in the workspace (4 B/bin)
+ *                                          even where the sums of 4-bin groups would do
+ * Like every setter that changes derived state: the workspace must be attached again (its size may change). */
+#define PULSCAN_VARIANT_SWEEP_SECOND_LOOK 1
+#define PULSCAN_VARIANT_SCAN_QUADS 2
+#define PULSCAN_VARIANT_NORM_KEEP_INDICES 3
+#define PULSCAN_VARIANT_NORM_L2_AHEAD 4
+#define PULSCAN_VARIANT_NORM_SINGLE_HISTOGRAM 5
+#define PULSCAN_VARIANT_KEEP_POWER 6
+int pulscan_plan_set_variant(pulscan_plan* plan, int32_t which, int32_t value);
 
 /* Capacity (in cells, 8 bytes each) of the list that carries flagged cover cells from the sweep to its refine kernel;
  * 0 = default (max(65536, batch·n_bins/256): ≈ 25× what noise flags at the default p_flag).  When the list is full the

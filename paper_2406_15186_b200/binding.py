@@ -41,6 +41,7 @@ SIGNATURES = {
     "pulscan_search_harmonics": (ctypes.c_int, [_P, _P, _P, _P, _P]),
     "pulscan_plan_set_tuning": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_double]),
     "pulscan_plan_set_cell_capacity": (ctypes.c_int, [_P, ctypes.c_int64]),
+    "pulscan_plan_set_variant": (ctypes.c_int, [_P, ctypes.c_int32, ctypes.c_int32]),
     "pulscan_plan_max_candidates": (ctypes.c_int64, [_P]),
     "pulscan_plan_workspace_bytes": (ctypes.c_size_t, [_P]),
     "pulscan_plan_enable_host_staging": (ctypes.c_int, [_P, ctypes.c_int32]),
@@ -62,6 +63,10 @@ SIGNATURES = {
     "pulscan_last_error": (ctypes.c_char_p, []),
     "pulscan_version": (ctypes.c_char_p, []),
 }
+
+# pulscan_plan_set_variant selectors (include/pulscan.h)
+VARIANT_SWEEP_SECOND_LOOK, VARIANT_SCAN_QUADS, VARIANT_NORM_KEEP_INDICES, VARIANT_NORM_L2_AHEAD = 1, 2, 3, 4
+VARIANT_NORM_SINGLE_HISTOGRAM, VARIANT_KEEP_POWER = 5, 6
 
 _lib = None
 
@@ -109,7 +114,8 @@ class Plan:
                  norm_block: Optional[int] = None, n_trials: Optional[float] = None, pitch: Optional[int] = None,
                  mode: int = 0, tile: int = 0, log10_p_flag: float = 0.0, host_staging: bool = False,
                  cell_capacity: int = 0, z_step: int = 1, log_sampling: bool = False, r_block: bool = False, numharm: int = 1,
-                 median_of_medians: bool = False, per_width_capacity: int = 0, poly_logp: bool = False):
+                 median_of_medians: bool = False, per_width_capacity: int = 0, poly_logp: bool = False,
+                 variants: Optional[dict] = None):
         self.lib = load_library()
         self.n_bins, self.batch, self.zmax, self.block_width = int(n_bins), int(batch), int(zmax), int(block_width)
         self.handle = self.lib.pulscan_plan_create(n_bins, batch, zmax, block_width, sigma_threshold)
@@ -144,6 +150,8 @@ class Plan:
         self.d_hcandidates = None
         if cell_capacity:
             _check(self.lib.pulscan_plan_set_cell_capacity(self.handle, cell_capacity))
+        for which, value in (variants or {}).items():
+            _check(self.lib.pulscan_plan_set_variant(self.handle, which, value))
         self.pitch = int(pitch) if pitch is not None else self.n_bins
         self.workspace = None
         self.d_candidates = None

@@ -42,15 +42,6 @@
 
 namespace pulscan {
 
-#ifdef PULSCAN_V2_TIMING
-__device__ unsigned long long g_v2_t[16];
-#define V2_TICK(k) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_v2_t[k], (unsigned long long)(now_ - tick_)); tick_ = now_; } } while (0)
-#define V2_RTICK(k) do { if (threadIdx.x == 0) { const long long now_ = clock64(); atomicAdd(&g_v2_t[k], (unsigned long long)(now_ - rt_)); rt_ = now_; } } while (0)
-#else
-#define V2_TICK(k) do { } while (0)
-#define V2_RTICK(k) do { } while (0)
-#endif
-
 constexpr int kV2NB = 2048;            // buckets per component
 constexpr int kV2KPT = 16;             // buckets per chunk
 constexpr int kV2NCH = kV2NB / kV2KPT; // chunks per component (128)
@@ -296,9 +287,6 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     constexpr int kk = (B - 1) >> 1;
     constexpr bool kEven = (B & 1) == 0;
     const int lane = threadIdx.x & 31;
-#ifdef PULSCAN_V2_TIMING
-    long long rt_ = clock64();
-#endif
     float* med = ctl.cls[c][0];
     float* shl = ctl.cls[c][1];
     const int nm = (int)ctl.cls_n[c][0], ns = (int)ctl.cls_n[c][1];   // the gather has split the members already
@@ -312,10 +300,8 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     }
     if (lane < 4) { med[nm + lane] = INFINITY; shl[ns + lane] = INFINITY; }
     __syncwarp();
-    V2_RTICK(8);
     float a, b;
     v2_rank_pair(med, nm, tmr, a, b);
-    V2_RTICK(9);
     if (!kEven) b = a;
     const float h = 0.5f * __fsub_rn(b, a);
     // deviations of the shell members, same arithmetic as the general path
@@ -325,7 +311,6 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
     float da, db;
     v2_rank_pair(shl, ns, tsr, da, db);
     if (!kEven) db = da;
-    V2_RTICK(10);
     // ---- verification.  vb(k) = value at the boundary between buckets k−1 and k.  Every value whose bucket lies
     // strictly inside the shells deviates by at most din, every value beyond them by at least dout; the margin of
     // 0.05 bucket covers the float rounding of the map and of its inverse (|off| ≤ 64).
@@ -349,7 +334,6 @@ __device__ __forceinline__ void v2_resolve(V2Ctl& ctl, int c) {
         ctl.a[c] = a; ctl.h[c] = h;
         ctl.inv[c] = (s > 0.0 && isfinite(s)) ? (float)(0.70710678118654752440 / s) : 0.f;
     }
-    V2_RTICK(11);
 }
 
 // Stage `bytes` (multiple of 16) global → shared with one TMA bulk copy; thread 0 only.  The mbarrier must have been
@@ -426,9 +410,6 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
     const long long lo_bin = (long long)jblk * B;
     const float2* src = spectra + (long long)row * pitch_in + lo_bin;
 
-#ifdef PULSCAN_V2_TIMING
-    long long tick_ = clock64();
-#endif
     // ---- stage the block; zero the histograms meanwhile; warp 0 derives the bucket map from a sample
     const unsigned shift = (unsigned)(reinterpret_cast<uintptr_t>(src) & 15);          // 0 or 8
     const char* csrc = reinterpret_cast<const char*>(src) - shift;
@@ -486,7 +467,6 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         v2_estimate<B>(sdat, ctl);
     }
     __syncthreads();                                                                     // S1
-    V2_TICK(0);
     if (use_tma) v2_mbar_wait(&ctl.mbar, 0);           // already complete: makes the copied bytes visible to this thread
     bool bad = ctl.fail != 0;
 
@@ -509,7 +489,6 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
     }
     __syncthreads();                                                                     // S2
-    V2_TICK(1);
     // ---- chunk totals (16 buckets each), rotated 16-byte reads so that a quarter-warp touches all bank groups
     if (!bad) {
         for (int id = tid; id < 2 * kV2NCH; id += NT) {
@@ -525,10 +504,8 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
     }
     __syncthreads();                                                                     // S3
-    V2_TICK(2);
     if (!bad && warp < 2) v2_locate<B>(ctl, hist + warp * kV2NB, warp);
     __syncthreads();                                                                     // S4
-    V2_TICK(3);
     bad = bad || ctl.fail != 0;
     // ---- gather: z = ||4·(idx − ⌊c2/2⌋)| − K| − K, member ⇔ |z| ≤ HW', on fp16 pairs (exact small-integer arithmetic).
     // The few hits (≈ 30 of 2·B values) are re-read, classified exactly (shell t = |2·bucket − c2|: median net t ≤ tm, MAD
@@ -603,10 +580,8 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
         }
     }
     __syncthreads();                                                                     // S5
-    V2_TICK(4);
     if (!bad && warp < 2) v2_resolve<B>(ctl, warp);
     __syncthreads();                                                                     // S6
-    V2_TICK(5);
     bad = bad || ctl.fail != 0;
     if (!bad) {
         // x' = ((v − a) − h)·inv evaluated as fma(v − a, inv, −h·inv), as in the general path (norm_power.cuh)
@@ -640,10 +615,6 @@ norm_power_v2_kernel(const float2* __restrict__ spectra, long long pitch_in, int
                 st[0] = a0; st[1] = i0; st[2] = k0; st[3] = a1; st[4] = i1; st[5] = k1;
             }
         }
-#ifdef PULSCAN_V2_TIMING
-        __syncthreads();
-        V2_TICK(6);
-#endif
     } else if (tid == 0) {
         redo[atomicAdd(redo_count, 1u)] = blockIdx.x;   // the general path will do this block
         atomicAdd(redo_count + 2 + min(max(ctl.fail, 1), 5), 1u);   // counters[4..8]: why (see V2Ctl::fail)

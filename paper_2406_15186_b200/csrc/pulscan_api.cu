@@ -88,6 +88,13 @@ struct pulscan_plan {
     int32_t tile_user = 0;
     double log10_p_flag = kDefaultLog10PFlag;
     bool host_staging = false;
+    // kernel variants (pulscan_plan_set_variant): comparison and tuning switches, none of which changes a result
+    int32_t v_second_look = 1;   // the sweep's second look at a flagged cell (half-group thresholds)
+    int32_t v_scan_quads = 0;    // 0 = automatic, 5 = the multi-pass scan of 5 quads per thread
+    int32_t v_keepidx = -1;      // single-histogram kernel keeps its bucket indices in registers: -1 = automatic, 0, 1
+    int32_t v_l2_ahead = -1;     // its L2 look-ahead in CTAs: -1 = automatic (4 x SMs), 0 = off
+    int32_t v_single_hist = 1;   // 0: every normalisation block goes through the general kernel
+    int32_t v_keep_power = 0;    // 1: the float32 power of every bin stays in the workspace even where the group sums would do
     // derived (host)
     bool dirty = true;         // derived tables need (re)building
     int64_t nblk = 0;          // candidate blocks per spectrum
@@ -328,7 +335,7 @@ int derive(pulscan_plan& p) {
     for (int l = 0; l < sp.nlevels; ++l) {
         SweepLevel& lv = sp.lv[l];
         lv.tauh_off = 0; lv.mh_start = 0; lv.nmh = 0;
-        if (lv.lg < 3 || lv.nsteps == 0 || std::getenv("PULSCAN_NO_CONFIRM") != nullptr) continue;
+        if (lv.lg < 3 || lv.nsteps == 0 || !p.v_second_look) continue;
         const int gh = 1 << (lv.lg - 1);
         lv.mh_start = std::max(0, 2 * lv.m_start - 2);
         const int mh_end = 2 * (lv.m_start + 4 * lv.nsteps - 1);
@@ -348,17 +355,13 @@ int derive(pulscan_plan& p) {
     // kernels rebuild the spans they need from the input spectrum (power_source.cuh).  It stays for: a child plan (its
     // "power" is the harmonic-summed spectrum Y_H), the exhaustive cross-check mode, levels finer than four bins
     // (full-resolution sweep), the harmonic search (Y_H is summed from P), the Alg. 1 normalisation kernel, and
-    // normalisation blocks that are not a multiple of four bins.  PULSCAN_KEEP_P forces it (comparison runs).
-    p.keep_P = p.is_child || p.mode == 1 || p.sweep_fine || p.numharm > 1 || p.norm_mode == 1 || (p.B & 3) != 0 ||
-               std::getenv("PULSCAN_KEEP_P") != nullptr;
+    // normalisation blocks that are not a multiple of four bins.  PULSCAN_VARIANT_KEEP_POWER forces it (comparison runs).
+    p.keep_P = p.is_child || p.mode == 1 || p.sweep_fine || p.numharm > 1 || p.norm_mode == 1 || (p.B & 3) != 0 || p.v_keep_power;
     sp.z_floats = p.keep_P ? (int)align_up((size_t)(sp.len + kScanTail), 4) : (int)align_up((size_t)(sp.len / 4 + kScanTail / 4), 4);
     // quads per thread per scan pass: a whole tile + halo in one pass where it fits 9 or 11 quads per thread (the
     // full-resolution scan keeps three more values per quad in registers and stays at 5)
     sp.scan_nq = (p.sweep_fine || sp.len <= 20 * kSweepThreads) ? 5 : (sp.len <= 36 * kSweepThreads ? 9 : (sp.len <= 44 * kSweepThreads && !p.keep_P ? 11 : 5));
-    {
-        const char* e = std::getenv("PULSCAN_SCAN_NQ");
-        if (e && std::atoi(e) == 5) sp.scan_nq = 5;
-    }
+    if (p.v_scan_quads == 5) sp.scan_nq = 5;
     sp.npass = (sp.len + 4 * sp.scan_nq * kSweepThreads - 1) / (4 * sp.scan_nq * kSweepThreads);
     if (task > kMaxWarpTasks) return fail(PULSCAN_EINVAL, "sweep tile of %d bins needs %d warp-tasks (limit %d)", tile, task, kMaxWarpTasks);
     sp.ntau = (int)p.tau.size();
@@ -418,21 +421,16 @@ int derive(pulscan_plan& p) {
         p.main_blocks_per_row = p.nb;
     }
 
-    p.norm_staged = std::getenv("PULSCAN_NORM_STAGED") != nullptr;
+    p.norm_staged = false;   // the TMA-staged variant lost its measurement (round 1) and is no longer dispatched
     // Bucket indices kept in registers between the histogram pass and the gather, or recomputed from a re-read of the block
     // (40 instead of 64 registers: more blocks per SM, one more read pass).  Measured (kernel (a), ms; kept / recomputed):
     // cfg 3 (B 4096, 128 threads, 8 -> 10 CTAs) 3.05 / 3.58; cfg 5 (B 2048) 7.53 / 8.05; cfg 4 (B 8192, 256 threads,
-    // 4 -> 6 CTAs) 0.864 / 0.830 — recomputed for blocks of 8192 bins only.  PULSCAN_NORM_NOIDX=0/1 overrides.
-    {
-        const char* e = std::getenv("PULSCAN_NORM_NOIDX");
-        p.norm_keepidx = e ? std::atoi(e) == 0 : p.B < 8192;
-    }
+    // 4 -> 6 CTAs) 0.864 / 0.830 — recomputed for blocks of 8192 bins only.  PULSCAN_VARIANT_NORM_KEEP_INDICES overrides.
+    p.norm_keepidx = p.v_keepidx >= 0 ? p.v_keepidx != 0 : p.B < 8192;
     // Fewer warps per CTA: the warp-serial phases keep two warps busy and idle the rest.  Measured: cfg 3 (B = 4096)
     // 256 threads 3.71 ms, 128 threads 3.41 ms; cfg 5 (B = 2048) 128 threads 9.06 ms, 64 threads 10.5 ms.
-    // PULSCAN_NORM_NT256 / PULSCAN_NORM_STAGED select the earlier variants for comparison.
-    p.norm_nt = (std::getenv("PULSCAN_NORM_NT256") == nullptr && !p.norm_staged && p.B >= 512 && p.B <= 4096) ? 128 : 256;
-    p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 &&
-                 std::getenv("PULSCAN_NO_FAST_NORM") == nullptr;
+    p.norm_nt = (p.B >= 512 && p.B <= 4096) ? 128 : 256;
+    p.use_fast = p.nt_main == 256 && p.B == p.ept_main * 256 && p.ept_main >= 2 && p.main_blocks_per_row > 0 && p.v_single_hist;
     }
 
     // ---- workspace layout
@@ -479,6 +477,7 @@ int derive(pulscan_plan& p) {
         // pay there (numharm 4, log-spaced widths, cfg 3: 8.92 ms at -3.25, 8.25 at -2.5, 8.35 at -2)
         c->log10_p_flag = (p.log10_p_flag == kDefaultLog10PFlag) ? -2.5 : p.log10_p_flag;
         c->cell_cap_user = p.cell_cap_user; c->B = p.B;
+        c->v_second_look = p.v_second_look; c->v_scan_quads = p.v_scan_quads;
         p.harm.push_back(c);
         const int rc = derive(*c);
         if (rc) return rc;
@@ -544,9 +543,8 @@ int finalize_device(pulscan_plan& p) {
     if (occ < 1) return fail(PULSCAN_ECUDA, "sweep_refine_kernel does not fit an SM with %zu bytes of shared memory", p.smem_refine);
     p.refine_grid = p.sm_count * std::min(occ, 16);
     {   // look-ahead of the single-histogram kernel's L2 prefetch in CTAs (short blocks only, see kV2L2Ahead): half a wave of
-        // resident CTAs measured best (592 and 1184: 7.61 ms at cfg 5; 2368: 8.0; off: 8.25); PULSCAN_NORM_L2_AHEAD overrides
-        const char* e = std::getenv("PULSCAN_NORM_L2_AHEAD");
-        p.norm_l2_ahead = e ? (unsigned)std::strtoul(e, nullptr, 10) : (unsigned)p.sm_count * 4u;
+        // resident CTAs measured best (592 and 1184: 7.61 ms at cfg 5; 2368: 8.0; off: 8.25); PULSCAN_VARIANT_NORM_L2_AHEAD overrides
+        p.norm_l2_ahead = p.v_l2_ahead >= 0 ? (unsigned)p.v_l2_ahead : (unsigned)p.sm_count * 4u;
     }
     p.finalized = true;
     return PULSCAN_OK;
@@ -581,10 +579,6 @@ int set_kernel_attributes(const pulscan_plan& p) {
     CUDA_TRY(cudaFuncSetAttribute(sweep_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(boxcar_exhaustive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
     CUDA_TRY(cudaFuncSetAttribute(block_exact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem));
-    CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<16, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)v2_smem_bytes<16, 256, true>()));
-    CUDA_TRY(cudaFuncSetAttribute(norm_power_v2_kernel<32, 256, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)v2_smem_bytes<32, 256, true>()));
     return PULSCAN_OK;
 }
 
@@ -635,8 +629,8 @@ int launch_norm_fast(pulscan_plan& p, int grid, cudaStream_t st, const float2* s
         case 256 * 64 + 2: PULSCAN_V2_LAUNCH(2, 256, false) break;
         case 256 * 64 + 4: PULSCAN_V2_LAUNCH(4, 256, false) break;
         case 256 * 64 + 8: PULSCAN_V2_LAUNCH(8, 256, false) break;
-        case 256 * 64 + 16: if (p.norm_staged) PULSCAN_V2_LAUNCH(16, 256, true) else PULSCAN_V2_LAUNCH(16, 256, false) break;
-        case 256 * 64 + 32: if (p.norm_staged) PULSCAN_V2_LAUNCH(32, 256, true) else PULSCAN_V2_LAUNCH(32, 256, false) break;
+        case 256 * 64 + 16: PULSCAN_V2_LAUNCH(16, 256, false) break;
+        case 256 * 64 + 32: PULSCAN_V2_LAUNCH(32, 256, false) break;
         case 128 * 64 + 32: PULSCAN_V2_LAUNCH(32, 128, false) break;
         case 128 * 64 + 16: PULSCAN_V2_LAUNCH(16, 128, false) break;
         case 128 * 64 + 8: PULSCAN_V2_LAUNCH(8, 128, false) break;
@@ -898,6 +892,33 @@ int pulscan_plan_set_tuning(pulscan_plan* plan, int32_t tile_bins, double log10_
         return fail(PULSCAN_EINVAL, "log10_p_flag must be 0 or in [-9, -1]");
     plan->tile_user = tile_bins;
     plan->log10_p_flag = (log10_p_flag == 0.0) ? kDefaultLog10PFlag : log10_p_flag;
+    invalidate(*plan);
+    return PULSCAN_OK;
+}
+
+int pulscan_plan_set_variant(pulscan_plan* plan, int32_t which, int32_t value) {
+    if (!plan) return fail(PULSCAN_EINVAL, "null plan");
+    switch (which) {
+        case PULSCAN_VARIANT_SWEEP_SECOND_LOOK:
+            if (value != 0 && value != 1) return fail(PULSCAN_EINVAL, "PULSCAN_VARIANT_SWEEP_SECOND_LOOK takes 0 or 1");
+            plan->v_second_look = value; break;
+        case PULSCAN_VARIANT_SCAN_QUADS:
+            if (value != 0 && value != 5) return fail(PULSCAN_EINVAL, "PULSCAN_VARIANT_SCAN_QUADS takes 0 (automatic) or 5");
+            plan->v_scan_quads = value; break;
+        case PULSCAN_VARIANT_NORM_KEEP_INDICES:
+            if (value < -1 || value > 1) return fail(PULSCAN_EINVAL, "PULSCAN_VARIANT_NORM_KEEP_INDICES takes -1 (automatic), 0 or 1");
+            plan->v_keepidx = value; break;
+        case PULSCAN_VARIANT_NORM_L2_AHEAD:
+            if (value < -1 || value > (1 << 20)) return fail(PULSCAN_EINVAL, "PULSCAN_VARIANT_NORM_L2_AHEAD takes -1 (automatic) or 0 … 2^20 CTAs");
+            plan->v_l2_ahead = value; break;
+        case PULSCAN_VARIANT_NORM_SINGLE_HISTOGRAM:
+            if (value != 0 && value != 1) return fail(PULSCAN_EINVAL, "PULSCAN_VARIANT_NORM_SINGLE_HISTOGRAM takes 0 or 1");
+            plan->v_single_hist = value; break;
+        case PULSCAN_VARIANT_KEEP_POWER:
+            if (value != 0 && value != 1) return fail(PULSCAN_EINVAL, "PULSCAN_VARIANT_KEEP_POWER takes 0 or 1");
+            plan->v_keep_power = value; break;
+        default: return fail(PULSCAN_EINVAL, "unknown variant %d", which);
+    }
     invalidate(*plan);
     return PULSCAN_OK;
 }
@@ -1310,11 +1331,3 @@ const char* pulscan_last_error(void) { return g_last_error.c_str(); }
 const char* pulscan_version(void) { return "pulscan-b200 0.1.0 (sm_100a)"; }
 
 } // extern "C"
-
-#ifdef PULSCAN_V2_TIMING
-extern "C" int pulscan_debug_v2_timing(unsigned long long* out, int reset) {
-    if (out) cudaMemcpyFromSymbol(out, pulscan::g_v2_t, sizeof(unsigned long long) * 16);
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(pulscan::g_v2_t, z, sizeof z); }
-    return 0;
-}
-#endif

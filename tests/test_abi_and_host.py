@@ -78,6 +78,14 @@ def test_setters_validate(binding):
     assert lib.pulscan_plan_set_emission(p.handle, 1, 1234) == binding.PULSCAN_OK and p.max_candidates == 1234
     assert lib.pulscan_plan_set_emission(p.handle, 0, 0) == binding.PULSCAN_OK and p.max_candidates == 2 * 200
     assert lib.pulscan_plan_set_harmonics(p.handle, 0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_variant(p.handle, 99, 0) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_variant(p.handle, binding.VARIANT_SCAN_QUADS, 7) == binding.PULSCAN_EINVAL
+    assert lib.pulscan_plan_set_variant(p.handle, binding.VARIANT_SWEEP_SECOND_LOOK, 2) == binding.PULSCAN_EINVAL
+    before = p.workspace_bytes
+    assert lib.pulscan_plan_set_variant(p.handle, binding.VARIANT_KEEP_POWER, 1) == binding.PULSCAN_OK
+    assert p.workspace_bytes > before and "float32 power of every bin" in p.describe()
+    assert lib.pulscan_plan_set_variant(p.handle, binding.VARIANT_KEEP_POWER, 0) == binding.PULSCAN_OK
+    assert p.workspace_bytes == before
     assert lib.pulscan_plan_set_harmonics(p.handle, 5) == binding.PULSCAN_EINVAL
     assert lib.pulscan_plan_set_cell_capacity(p.handle, -1) == binding.PULSCAN_EINVAL
     ws0 = p.workspace_bytes
