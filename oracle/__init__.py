@@ -16,7 +16,10 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "pulscan_oracle.c"
-_LIB = _HERE / "liboracle.so"
+# ORACLE_SANITIZE=1 in the environment: build and load an AddressSanitizer + UBSan copy instead (run the CPU tests with
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0; DESIGN.md §7 records the last such run)
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+_LIB = _HERE / ("liboracle_san.so" if _SANITIZE else "liboracle.so")
 
 CANDIDATE_DTYPE = np.dtype(
     [("spectrum", "<i4"), ("bin", "<i4"), ("width", "<i4"), ("numharm", "<i4"), ("power", "<f8"), ("sigma", "<f8"),
@@ -28,7 +31,8 @@ def build(force: bool = False) -> Path:
     """Compile the C oracle with gcc (-O2, OpenMP).  Building the checker is not using it."""
     if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
         tmp = _LIB.with_suffix(f".{os.getpid()}.tmp")
-        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-D_GNU_SOURCE", "-o", str(tmp), str(_SRC), "-lm"]
+        san = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if _SANITIZE else []
+        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-D_GNU_SOURCE", *san, "-o", str(tmp), str(_SRC), "-lm"]
         subprocess.run(cmd, check=True, capture_output=True)
         os.replace(tmp, _LIB)
     return _LIB
