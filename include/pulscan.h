@@ -57,7 +57,7 @@ extern "C" {
 /* Limits of this build (PULSCAN_EINVAL beyond them). */
 #define PULSCAN_MAX_ZMAX 4096
 #define PULSCAN_MAX_NORM_BLOCK 16384
-#define PULSCAN_MAX_BLOCK_PLUS_ZMAX 24576 /* block_width + zmax: one candidate block + halo in shared memory */
+#define PULSCAN_MAX_BLOCK_WIDTH (1 << 24) /* candidate blocks with block_width + zmax > 24576 are evaluated in segments */
 
 typedef struct pulscan_plan pulscan_plan; /* opaque */
 
@@ -89,7 +89,7 @@ typedef struct {
  * Gaussian-σ threshold (L361).  Host-only: touches no CUDA device.  Defaults: norm_block = next power of two
  * ≥ 16·block_width clamped to [1024, 8192]; n_trials = 1; pitch = n_bins.
  * Returns NULL on error (n_bins < 2, batch < 1, zmax < 1 or ≥ n_bins or > PULSCAN_MAX_ZMAX, block_width < 1,
- * block_width + zmax > PULSCAN_MAX_BLOCK_PLUS_ZMAX, sigma_threshold ≤ 0 or not finite, batch·blocks ≥ 2³¹). */
+ * or > PULSCAN_MAX_BLOCK_WIDTH, sigma_threshold ≤ 0 or not finite, batch·blocks ≥ 2³¹). */
 pulscan_plan* pulscan_plan_create(int64_t n_bins, int32_t batch, int32_t zmax, int32_t block_width,
                                   float sigma_threshold);
 
@@ -117,7 +117,9 @@ int pulscan_plan_set_width_sampling(pulscan_plan* plan, int32_t z_step, int32_t 
 
 /* "Pulscan R-Block" (L222-226 §2.4): save only the block index of a candidate, "an approximate frequency location".
  * enable ≠ 0: a record's `bin` is the first bin of its candidate block, block index × block_width (Table 3:
- * 360448 = 11 × 32768); width, power and sigma are unchanged.  Default 0: the exact first bin of the window. */
+ * 360448 = 11 × 32768); width, power and sigma are unchanged.  Default 0: the exact first bin of the window.
+ * The paper's own setting, block_width = 32768 (L224 "the default value of 32768 was used for all Pulscan R-Block tests"), is
+ * within range: kernel (c) walks such a block in segments. */
 int pulscan_plan_set_r_block(pulscan_plan* plan, int32_t enable);
 
 /* Harmonic sum (L201-220 §2.3; `-numharm`): numharm ∈ [1, 4].  pulscan_search_harmonics() then also searches the summed

@@ -68,16 +68,23 @@ struct alignas(8) ExactPartial {
 // their partial arg-minima meet in `partial` and the CTA that arrives last (`done` counter) reduces and emits — a few
 // hundred marked blocks then occupy the whole GPU instead of one CTA each.  Only the first `split_slots` marked blocks are
 // split (the size of `partial` / `done`); the rest is evaluated by one CTA per block.
+// seg < C (long candidate blocks, e.g. the paper's R-Block width 32768, L224): the block's start bins are walked in segments of
+// `seg` bins, each with its own prefix sum (+ zmax halo) in shared memory; the running maximum and arg-max of every width are
+// carried from segment to segment in shared memory behind the prefix array (a width always belongs to the same thread), a
+// later segment replaces them on `>` only (R14: the lowest bin wins ties), and ln p is evaluated after the last segment.
 __global__ void __launch_bounds__(kExactThreads)
 block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long long nblk,
                    const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int signif_mode, int numharm,
-                   pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity, int lg_split, int parts,
+                   pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity, int lg_split, int parts, int seg,
                    unsigned split_slots, ExactPartial* __restrict__ partial, unsigned* __restrict__ done,
                    const unsigned* __restrict__ flagged, const unsigned* __restrict__ counters,
                    pulscan_candidate* __restrict__ out, unsigned* __restrict__ out_count) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     ExactSmemHdr& hdr = *reinterpret_cast<ExactSmemHdr*>(smem_raw);
-    double* pre = reinterpret_cast<double*>(smem_raw + sizeof(ExactSmemHdr)); // [L + 1]
+    double* pre = reinterpret_cast<double*>(smem_raw + sizeof(ExactSmemHdr)); // [L + 1], L ≤ min(C, seg) + zmax − 1
+    const int Cs = min(C, seg);                                                 // start bins per segment
+    double* carry_s = pre + ((Cs + zmax + 2) & ~1);                             // [zmax + 1], only when seg < C
+    int* carry_i = reinterpret_cast<int*>(carry_s + zmax + 1);                  // [zmax + 1]
     const int tid = threadIdx.x, lane = tid & 31;
     const unsigned nflag = counters[0];
     if (tid == 0) { hdr.nlist[0] = 0; hdr.nlist[1] = 0; }
@@ -85,7 +92,7 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
     const int nsplit = 1 << lg_split, piece = tid & (nsplit - 1), w_per_round = kExactThreads >> lg_split;
     // start bins per chunk: even (16-byte loads of pairs of doubles), and ≡ 2 (mod 4) when there are several chunks, so that
     // the chunks' 16-byte loads of a warp (lanes of a chunk 32 bytes apart) interleave on the banks: 4 wavefronts per 512 bytes
-    int cs = (C + nsplit - 1) >> lg_split;
+    int cs = (Cs + nsplit - 1) >> lg_split;
     if (nsplit >= 2) cs += (2 - cs) & 3;
 
     const unsigned n_split = parts > 1 ? min(nflag, split_slots) : 0u;
@@ -100,17 +107,25 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
         const long long lo = c * C;
         long long hi = lo + C;
         if (hi > n) hi = n;
-        const int nstart = (int)(hi - lo);
-        long long end = hi + zmax - 1;              // last bin any window of the block can touch, exclusive: hi−1+zmax
+        const int nstart_all = (int)(hi - lo);
+        const int nseg = (nstart_all + Cs - 1) / Cs;
+        double my_lnp = INFINITY, my_s = 0.0;
+        int my_w = 0, my_i = 0;
+        for (int sg = 0; sg < nseg; ++sg) {
+        const bool last_seg = sg == nseg - 1;
+        const int seg_off = sg * Cs;                // first start bin of this segment, relative to the block
+        const long long slo = lo + seg_off;
+        const int nstart = min(Cs, nstart_all - seg_off);
+        long long end = slo + nstart + zmax - 1;    // last bin any window of the segment can touch, exclusive
         if (end > n) end = n;
-        const int L = (int)(end - lo);
+        const int L = (int)(end - slo);
         if (tid == 0) { hdr.nlist[0] = 0; hdr.nlist[1] = 0; }   // (barriers of the prefix build separate this from the first use)
 
         // double-precision prefix sum pre[j] = Σ_{t<j} P[lo+t]: coalesced loads (or rebuilds, power_source.cuh) into
         // pre[j+1], each thread then scans its own chunk in place and the chunk totals are scanned by one warp
         {
             PowerSource::Row src(src_pw, row);
-            for (int j = tid; j < L; j += kExactThreads) pre[j + 1] = (double)src(lo + j);
+            for (int j = tid; j < L; j += kExactThreads) pre[j + 1] = (double)src(slo + j);
             if (tid == 0) pre[0] = 0.0;
         }
         __syncthreads();
@@ -145,8 +160,6 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
         // needs pre[i..i+3] and pre[i+W4 .. i+W4+6]: 6 shared-memory loads for 16 window sums instead of 32 (the kernel is
         // bound by the rate of LDS instructions).  Per width the maximum and its lowest arg-max (strict >, ascending starts:
         // R14), combined over the chunks of a width by shuffles (adjacent lanes, the lower chunk holds the lower bins).
-        double my_lnp = INFINITY, my_s = 0.0;
-        int my_w = 0, my_i = 0;
         int rnd = 0;                                        // which of the two list counters this round uses
         const int nquads = zmax / 4 + 1;                    // width quads {4q, …, 4q+3}; width 0 does not exist
         for (int q0 = part * w_per_round; q0 < nquads; q0 += nparts * w_per_round) {
@@ -194,6 +207,17 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
                 // The widths whose maximum reaches T_w are collected and their ln p evaluated by all threads: the series of
                 // ln Q is a serial loop of up to w terms, and only one lane in 2^lg_split holds a width after the reduction.
                 const int w = W4 + b4;
+                if (nseg > 1) {                                // long block: merge with the segments before, hand on to the next
+                    if (piece == 0 && w >= 1 && w <= zmax) {
+                        if (arg[b4] >= 0) arg[b4] += seg_off;  // relative to the block from here on
+                        if (sg > 0) {
+                            const double cb = carry_s[w];
+                            if (!(best[b4] > cb)) { best[b4] = cb; arg[b4] = carry_i[w]; }
+                        }
+                        if (!last_seg) { carry_s[w] = best[b4]; carry_i[w] = arg[b4]; }
+                    }
+                    if (!last_seg) continue;                   // (uniform over the CTA) ln p after the last segment only
+                }
                 if (piece == 0 && arg[b4] >= 0 && best[b4] >= T_g[w - 1] * (1.0 - 1e-9)) {
                     const unsigned slot = atomicAdd(&hdr.nlist[rnd], 1u);
                     hdr.list_s[slot] = best[b4]; hdr.list_w[slot] = w; hdr.list_i[slot] = arg[b4];
@@ -215,6 +239,8 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
                 __syncthreads();
             }
         }
+        __syncthreads();                                    // the next segment overwrites the prefix array
+        }   // segments
         // block arg-min over (ln p, w)
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {

@@ -118,6 +118,7 @@ struct pulscan_plan {
     int exh_len = 0;
     int exact_lg_split = 0;    // kernel (c): 2^lg lanes share the start bins of a width
     int exact_parts = 1;       // kernel (c): CTAs that share the widths of one marked block
+    int exact_seg = 0;         // kernel (c): start bins per segment of a candidate block (= C unless the block is too long for shared memory)
     unsigned exact_slots = 0;  // marked blocks that can be split (size of the partial-result scratch)
     size_t off_partial = 0, off_done = 0;
     // normalisation launch shapes
@@ -384,7 +385,19 @@ int derive(pulscan_plan& p) {
     if (p.smem_sweep > 227 * 1024) return fail(PULSCAN_EINVAL, "sweep tile needs %zu bytes of shared memory", p.smem_sweep);
     p.exh_len = tile + (int)align_up((size_t)p.zmax, 64);
     p.smem_exh = (size_t)p.exh_len * 4 + align_up((size_t)p.zmax, 4) * 4 + 16 + flag_bytes;
-    p.smem_exact = sizeof(ExactSmemHdr) + (size_t)(p.C + p.zmax + 1) * 8;
+    {   // kernel (c) holds the prefix sum of a candidate block + halo in shared memory as doubles; a block too long for that
+        // (the paper's R-Block width 32768, L224) is walked in segments, with the per-width running maxima carried in
+        // (zmax + 1)·12 further bytes
+        constexpr long long kDyn = 227 * 1024;
+        if (p.C + p.zmax <= 24576) p.exact_seg = p.C;
+        else {
+            const long long room = (kDyn - (long long)sizeof(ExactSmemHdr) - (long long)(p.zmax + 1) * 12 - 16) / 8 - p.zmax - 2;
+            p.exact_seg = (int)(room / 64 * 64);
+            if (p.exact_seg < 1024) return fail(PULSCAN_EINVAL, "internal: no room for a segment of block_width = %d at zmax = %d", p.C, p.zmax);
+        }
+        const int cs = std::min(p.C, p.exact_seg);
+        p.smem_exact = sizeof(ExactSmemHdr) + (size_t)((cs + p.zmax + 2) & ~1) * 8 + (p.exact_seg < p.C ? (size_t)(p.zmax + 1) * 12 : 0);
+    }
     {   // kernel (c): a thread owns four consecutive widths; the start bins of a block are split over 2^lg adjacent lanes.  One
         // block costs zmax·C window sums on ONE SM (issue-bound: double-precision compare and select) plus ≈ 45 µs of
         // barrier-separated set-up per CTA (prefix sum rebuilt from the spectrum, ln p of the passing widths): only when the
@@ -739,7 +752,7 @@ int enqueue_sweep_exact(pulscan_plan& p, const float* d_in, const PowerSource& s
     const int grid_c = (int)std::min<long long>(total_blocks * p.exact_parts, (long long)p.sm_count * 4);
     if (p.exact_slots) CUDA_TRY(cudaMemsetAsync(ws + p.off_done, 0, (size_t)p.exact_slots * sizeof(unsigned), st));
     block_exact_kernel<<<grid_c, kExactThreads, p.smem_exact, st>>>(src, p.n, p.zmax, p.C, p.nblk, p.d_T, p.ln_trials,
-                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.signif_mode, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity, p.exact_lg_split, p.exact_parts,
+                                                                   p.lnp_thr, p.r_block, p.shape_mult, p.signif_mode, p.numharm_tag, d_hcandidates, p.per_width, p.out_capacity, p.exact_lg_split, p.exact_parts, p.exact_seg,
                                                                    p.exact_slots, reinterpret_cast<ExactPartial*>(ws + p.off_partial),
                                                                    reinterpret_cast<unsigned*>(ws + p.off_done),
                                                                    d_flagged, d_counters, d_candidates, d_count);
@@ -792,8 +805,7 @@ pulscan_plan* pulscan_plan_create(int64_t n_bins, int32_t batch, int32_t zmax, i
     if (zmax < 1 || zmax > PULSCAN_MAX_ZMAX) return bad("zmax = %d out of range [1, %d]", zmax, PULSCAN_MAX_ZMAX);
     if ((int64_t)zmax >= n_bins) return bad("zmax = %d must be < n_bins = %lld", zmax, (long long)n_bins);
     if (block_width < 1) return bad("block_width = %d < 1", block_width);
-    if ((int64_t)block_width + zmax > PULSCAN_MAX_BLOCK_PLUS_ZMAX)
-        return bad("block_width + zmax = %lld exceeds %d", (long long)block_width + zmax, PULSCAN_MAX_BLOCK_PLUS_ZMAX);
+    if (block_width > PULSCAN_MAX_BLOCK_WIDTH) return bad("block_width = %d exceeds %d", block_width, PULSCAN_MAX_BLOCK_WIDTH);
     if (!(sigma_threshold > 0.f) || !std::isfinite(sigma_threshold)) return bad("sigma_threshold must be finite and > 0");
     const int64_t nblk = (n_bins + block_width - 1) / block_width;
     if (nblk * batch >= 2147483648LL) return bad("batch · candidate blocks = %lld ≥ 2^31", (long long)(nblk * batch));
@@ -1195,8 +1207,8 @@ int64_t pulscan_plan_describe(const pulscan_plan* plan, char* h_buf, int64_t buf
     snprintf(line, sizeof line, "intermediate in HBM: %s\n",
              p.keep_P ? "float32 power of every bin (4 B/bin)" : "sums of 4-bin groups (1 B/bin) + 32 B per normalisation block");
     s += line;
-    snprintf(line, sizeof line, "exact: 4 widths per thread, start bins split over %d lanes, widths of a block dealt to %d CTA(s)\n",
-             1 << p.exact_lg_split, p.exact_parts);
+    snprintf(line, sizeof line, "exact: 4 widths per thread, start bins split over %d lanes, widths of a block dealt to %d CTA(s), %d segment(s) of %d start bins per block\n",
+             1 << p.exact_lg_split, p.exact_parts, (p.C + p.exact_seg - 1) / p.exact_seg, std::min(p.C, p.exact_seg));
     s += line;
     snprintf(line, sizeof line, "exact: smem=%zu B; workspace=%zu B; T_1=%.4f T_zmax=%.4f\n", p.smem_exact, p.need_bytes, p.T.front(), p.T.back());
     s += line;

@@ -46,7 +46,7 @@ def test_candidate_record_layout(binding):
     (100, 1, 100, 10, 6.0),       # zmax >= n_bins
     (100000, 1, 5000, 10, 6.0),   # zmax > PULSCAN_MAX_ZMAX
     (100, 1, 8, 0, 6.0),          # block_width < 1
-    (100000, 1, 4000, 30000, 6.0),  # block_width + zmax too large
+    (100000, 1, 4000, (1 << 24) + 1, 6.0),  # block_width > PULSCAN_MAX_BLOCK_WIDTH
     (100, 1, 8, 10, 0.0),         # sigma_threshold <= 0
     (100, 1, 8, 10, float("nan")),
     (2 ** 31 + 5, 1, 8, 10, 6.0),

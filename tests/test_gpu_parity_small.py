@@ -563,3 +563,74 @@ def test_kernel_variants_never_change_results(orc, which, value):
     got, _ = gpu_search(spec, zmax, B, C, thr, variants={which: value})
     assert np.array_equal(base, got) and len(got) > 0
     assert_same_candidates(got, oracle_search(orc, spec, zmax, B, C, thr), f"variant {which} = {value}")
+
+
+# ---- candidate blocks too long for one shared-memory prefix array: kernel (c) walks them in segments
+def _long_block_spectrum(n, zmax, seed):
+    """Noise + pulses in several segments of block 0 (segments are ≈ 15-25 k start bins), one in the last ragged block, and
+    two identical single-bin pulses in one normalisation block that fall in different segments when the block is cut at
+    25216 start bins (zmax 256): an exact tie across segments, which must go to the lower bin (R14)."""
+    spec = noise_spectra(1, n, seed=seed)
+    bump(spec, 0, 3000, min(zmax, 20), 1.9)
+    bump(spec, 0, 29000, min(zmax, 60), 1.6)
+    bump(spec, 0, n - 1500, 9, 2.2)
+    for i in (25000, 26000):
+        spec[0, i - 2:i + 3] *= 0.05
+    for i in (25000, 26000):
+        spec[0, i] = complex(12.0 * 50.0, 12.0 * 50.0)
+    return spec
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,zmax,B,C,thr,r_block", [
+    (200001, 256, 8192, 32768, 4.5, True),     # the paper's R-Block setting (PAPER.md:L224, Table 3 L516): 2 segments per block
+    (200001, 256, 8192, 32768, 4.5, False),
+    (100001, 4096, 8192, 30000, 4.5, False),   # 2 segments of 15616 start bins, the widths of a block dealt to 8 CTAs
+    (70001, 100, 4096, 70001, 4.0, False),     # one block = the whole spectrum, 3 segments
+])
+def test_long_candidate_blocks_are_walked_in_segments(orc, mode, n, zmax, B, C, thr, r_block):
+    from paper_2406_15186_b200 import binding
+    spec = _long_block_spectrum(n, zmax, seed=n + zmax)
+    plan = binding.Plan(n, 1, zmax, C, thr, norm_block=B)
+    assert "1 segment(s)" not in plan.describe().split("exact:")[1]
+    P = plan.normalise_power(spec).cpu().numpy()
+    plan.destroy()
+    assert P[0, 25000] == P[0, 26000] > 100
+    ref = oracle_search(orc, spec, zmax, B, C, thr, r_block=r_block)
+    got, _ = gpu_search(spec, zmax, B, C, thr, mode=mode, r_block=r_block)
+    assert len(ref) >= 1
+    assert_same_candidates(got, ref, f"C={C} zmax={zmax} mode={mode} r_block={r_block}")
+
+
+def test_long_candidate_blocks_tie_across_segments_and_per_width_emission(orc):
+    """Every width's maximum is carried over the segments before ln p is taken: per-(block, width) emission gives exactly one record per (block, width), and the width-1 record of block 0 names bin 25000,
+    the lower of the two tied bins, which sit in different segments."""
+    from paper_2406_15186_b200 import binding
+    n, zmax, B, C, thr = 120001, 64, 8192, 32768, 4.0
+    spec = _long_block_spectrum(n, zmax, seed=5)
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, 1, per_width=True)
+    ora = ora[np.lexsort((ora["width"], ora["bin"], ora["spectrum"]))]
+    plan = binding.Plan(n, 1, zmax, C, thr, norm_block=B, per_width_capacity=len(ora) + 16)
+    plan.attach("cuda")
+    plan.search(spec)
+    got = plan.candidates()
+    plan.destroy()
+    assert plan.last_count == len(ora) == len(got)
+    assert_same_candidates(got, ora, "per-width emission over segmented blocks")
+    w1 = got[(got["width"] == 1) & (got["bin"] // C == 0)]
+    assert len(w1) == 1 and w1["bin"][0] == 25000
+
+
+def test_long_candidate_blocks_with_polynomial_logp(orc):
+    """Alg. 3's ln p is not monotone in the power: it must be taken at the block maximum of a width, not per segment."""
+    from paper_2406_15186_b200 import binding
+    n, zmax, B, C, thr = 100001, 90, 8192, 32768, 6.0
+    spec = _long_block_spectrum(n, zmax, seed=8)
+    plan = binding.Plan(n, 1, zmax, C, thr, norm_block=B, poly_logp=True)
+    plan.attach("cuda")
+    plan.search_harmonics(spec)
+    gpu = plan.hcandidates()
+    plan.destroy()
+    ora = orc.search_harmonics(spec.cpu().numpy(), zmax, B, C, thr, 1, poly_logp=True)
+    assert len(ora) >= 2
+    _assert_same_hcandidates(gpu, ora, "Alg. 3 over segmented blocks")
