@@ -261,13 +261,62 @@ def run_ours(args):
     flagged = int(stats[0])
 
     # per-kernel device times of the timed steps (CUDA events recorded by the library on the launching stream)
-    if args.numharm > 1:   # the per-stage events belong to pulscan_search: report the whole step only
+    if args.numharm > 1:   # the per-stage events belong to pulscan_search: the whole step is held against the roofline
+        peak, peak_src = measured_hbm_peak()
+        gbs = lambda nbytes, t_ms: nbytes / (t_ms * 1e-3) / 1e9
+        H = args.numharm
+        # least own traffic of the harmonic path, per input bin: 8 read + 4 (P written) + 4 (P read by the sweep of Y_1) + the
+        # decimation pass (P read at least once: 4; each Y_H written: 4/H) + each Y_H read by its sweep (4/H).  A lower bound:
+        # the decimation pass re-reads P from DRAM where a row's reuse distance exceeds the L2
+        own = 8 + 4 + 4 + 4 + sum(8.0 / h for h in range(2, H + 1))
+        roofline = {"bound": "hbm", "kernel": "whole step (pulscan_search_harmonics: kernel (a), harmonic_sum_kernel, sweep + refine "
+                    "+ exact per Y_H)", "achieved": gbs(8 * bins, ms_step), "peak": peak, "unit": "GB/s",
+                    "frac": gbs(8 * bins, ms_step) / peak, "algorithmic_bytes_per_bin": 8, "algorithmic_bytes_per_launch": 8 * bins,
+                    "own_bytes_per_bin": own, "frac_own_traffic": gbs(own * bins, ms_step) / peak, "traffic": None,
+                    "peak_source": peak_src, "path_frac": gbs(8 * bins, ms_step) / peak if world == 1 else None}
+        e2e = None
+        if not args.no_e2e:   # host buffer -> H2D -> pulscan_search_harmonics -> D2H of count and records, wall clock
+            Xh = torch.empty(X.shape, dtype=X.dtype, pin_memory=True)
+            Xh.copy_(X)
+            Xd = torch.empty_like(X)
+            def one():
+                Xd.copy_(Xh, non_blocking=True)
+                plan.search_harmonics(Xd, stream)
+                return plan.hcandidates()
+            rec = one()
+            torch.cuda.synchronize(); pdist.barrier()
+            t0 = time.perf_counter()
+            for _ in range(args.e2e_steps):
+                rec = one()
+            dt = pdist.max_over_ranks(time.perf_counter() - t0)
+            assert len(rec) == n_cand, "host-buffer search disagrees with device-buffer search"
+            e2e = {"value": total_bins * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(Xh.numel() * 8),
+                   "d2h_bytes_per_step": int(4 + 24 * len(rec)), "steps": args.e2e_steps, "ms_per_step": 1e3 * dt / args.e2e_steps}
+            del Xd
+        cpu = None
+        if rank == 0 and world == 1 and not args.no_cpu_baseline:
+            import oracle
+            oracle.build()
+            rows = X[: min(wl.batch, 16)].cpu().numpy()
+            t0 = time.perf_counter()
+            oracle.search_harmonics(rows[:1], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold, H, z_step=args.z_step,
+                                    log_sampling=args.log_sampling, median_of_medians=args.fast_norm)
+            t1 = time.perf_counter() - t0
+            extra = int(max(0, min(len(rows) - 1, round(15.0 / max(t1, 1e-3)) - 1)))
+            if extra:
+                t0 = time.perf_counter()
+                oracle.search_harmonics(rows[1:1 + extra], wl.zmax, wl.norm_block, wl.block_width, wl.sigma_threshold, H,
+                                        z_step=args.z_step, log_sampling=args.log_sampling, median_of_medians=args.fast_norm)
+                t1 += time.perf_counter() - t0
+            cpu = {"value": (1 + extra) * wl.n_bins / t1, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                   "sample": f"{1 + extra} of {wl.batch} spectra of the workload, harmonic sums up to {H}, {t1:.1f} s wall"}
         if rank == 0:
             print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
                               "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                               "dtype": "f32", "data": "synthetic", "config": dict(config_dict(wl, world, args), numharm=args.numharm),
                               "bin_widths_per_sec": value * wl.zmax, "candidates_per_step": n_cand, "clocks": clk.summary(),
-                              "gpu_launches": (plan.launches_per_search + 1 + 3 * (args.numharm - 1)) * steps}), flush=True)
+                              "e2e": e2e, "gpu_launches": (plan.launches_per_search + 1 + 3 * (args.numharm - 1)) * steps,
+                              "roofline": roofline, "cpu_baseline": cpu}), flush=True)
         plan.destroy()
         if world > 1:
             tdist.destroy_process_group()
@@ -295,7 +344,8 @@ def run_ours(args):
     if sweep_ncu is not None:
         sweep_ncu += recorded_traffic("sweep_refine_kernel", args.config) or 0.0
     sweep_bytes = sweep_ncu if sweep_ncu is not None else own["boxcar_sweep_kernel"]
-    sweep_instr = None if keeps_p else recorded_traffic("boxcar_stage_warp_instr_per_bin", args.config)
+    default_sweep = not (keeps_p or args.log_sampling or args.z_step != 1 or args.tile or args.log10_p_flag)   # as captured
+    sweep_instr = recorded_traffic("boxcar_stage_warp_instr_per_bin", args.config) if default_sweep else None
     clocks = clk.summary()
     sm_hz = 1e6 * (clocks.get("sm_mhz") or 1965.0)
     issue_peak = 4.0 * torch.cuda.get_device_properties(dev).multi_processor_count * sm_hz

@@ -22,7 +22,17 @@
 
 namespace pulscan {
 
-constexpr int kExactThreads = 1024;
+// Threads per CTA / resident CTAs per SM.  Two CTAs of 512 threads let one block's barrier-separated set-up (prefix build, ln p
+// of the passing widths) overlap another block's window sums.  Measured on a B200, kernel (c) ms at cfg 2 / 3 / 4 / 5:
+// 1024 x 1: 0.058 / 0.065 / 0.209 / 0.061; 512 x 2: 0.055 / 0.062 / 0.196 / 0.057; 512 x 1: 0.053 / 0.061 / 0.215 / 0.055;
+// 256 x 4: 0.053 / 0.061 / 0.243 / 0.055.
+#ifndef PULSCAN_EXACT_THREADS
+#define PULSCAN_EXACT_THREADS 512
+#endif
+#ifndef PULSCAN_EXACT_MIN_CTAS
+#define PULSCAN_EXACT_MIN_CTAS 2
+#endif
+constexpr int kExactThreads = PULSCAN_EXACT_THREADS;
 
 struct alignas(16) ExactSmemHdr {   // the prefix array behind it is read with 16-byte loads
     double part[kExactThreads];   // per-thread chunk sums for the prefix scan
@@ -63,7 +73,7 @@ struct alignas(8) ExactPartial {
 };
 
 // lg_split: the start bins of a block are cut into 2^lg_split chunks handled by adjacent lanes, so that zmax·2^lg_split
-// (width, chunk) pairs keep all 1024 threads busy when zmax is small and balance the rounds when it is large (host choice).
+// (width, chunk) pairs keep all kExactThreads threads busy when zmax is small and balance the rounds when it is large (host choice).
 // parts > 1 (large zmax): the rounds of widths of one block are dealt to `parts` CTAs (each rebuilds the block's prefix sum),
 // their partial arg-minima meet in `partial` and the CTA that arrives last (`done` counter) reduces and emits — a few
 // hundred marked blocks then occupy the whole GPU instead of one CTA each.  Only the first `split_slots` marked blocks are
@@ -72,7 +82,7 @@ struct alignas(8) ExactPartial {
 // `seg` bins, each with its own prefix sum (+ zmax halo) in shared memory; the running maximum and arg-max of every width are
 // carried from segment to segment in shared memory behind the prefix array (a width always belongs to the same thread), a
 // later segment replaces them on `>` only (R14: the lowest bin wins ties), and ln p is evaluated after the last segment.
-__global__ void __launch_bounds__(kExactThreads)
+__global__ void __launch_bounds__(kExactThreads, PULSCAN_EXACT_MIN_CTAS)
 block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long long nblk,
                    const double* __restrict__ T_g, double ln_trials, double lnp_thr, int r_block, int shape_mult, int signif_mode, int numharm,
                    pulscan_hcandidate* __restrict__ out_h, int per_width, unsigned capacity, int lg_split, int parts, int seg,
@@ -137,7 +147,7 @@ block_exact_kernel(const PowerSource src_pw, long long n, int zmax, int C, long 
             hdr.part[tid] = run;
         }
         __syncthreads();
-        if (tid < 32) { // exclusive scan of the 1024 chunk sums by one warp, 32 each
+        if (tid < 32) { // exclusive scan of the kExactThreads chunk sums by one warp, kExactThreads/32 each
             double run = 0.0;
             for (int q = 0; q < kExactThreads / 32; ++q) { const double v = hdr.part[tid * (kExactThreads / 32) + q]; hdr.part[tid * (kExactThreads / 32) + q] = run; run += v; }
             double inc = run;

@@ -402,7 +402,7 @@ int derive(pulscan_plan& p) {
         // block costs zmax·C window sums on ONE SM (issue-bound: double-precision compare and select) plus ≈ 45 µs of
         // barrier-separated set-up per CTA (prefix sum rebuilt from the spectrum, ln p of the passing widths): only when the
         // window sums are several times that (measured at cfg 4, 1.44 M sums per block: 1 CTA 0.245 ms, 8 CTAs 0.387 ms) are
-        // the widths of a block dealt to several CTAs; lg is then chosen to give that many rounds of 1024 threads.
+        // the widths of a block dealt to several CTAs; lg is then chosen to give that many rounds of kExactThreads threads.
         const long long nquads = p.zmax / 4 + 1;
         const long long want_parts = std::min<long long>(8, std::max<long long>(1, (long long)p.zmax * p.C / 3000000));
         long long best = -1;
